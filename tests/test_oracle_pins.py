@@ -1,0 +1,371 @@
+"""Pins for the CPU oracle (no GPU): every oracle function is checked against something
+other than itself -- closed forms, invariants, brute force, a long-double evaluation of the
+plain definition, the survey's independent counts -- so that a dropped term, a wrong sign
+or a transposed index anywhere in oracle/rpim_oracle.cpp fails a test here.
+
+Citations: SURVEY.md section 8(c) "Pins" table; readings R1..R12.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+import scipy.sparse as sp
+import scipy.sparse.linalg as spla
+
+import oracle
+import workloads
+
+EPS = np.finfo(np.float64).eps
+
+
+# ------------------------------------------------------------------ R5: power function
+@pytest.mark.parametrize("q,tol_eps", [(1.03, 4.0), (0.5, 6.0), (1.5, 6.0), (1.99, 8.0), (-0.5, 8.0)])
+def test_pow_qm1_against_long_double(q, tol_eps):
+    rng = np.random.default_rng(7)
+    t = np.concatenate([np.exp(rng.uniform(np.log(1e-3), np.log(1e6), 4000)),
+                        [16.0, 1.0, 2.0, 0.5, 17.0, 41.0, 1.0 + 2 ** -52, 2.0 - 2 ** -52]])
+    got = np.array([oracle.pow_qm1(x, q) for x in t])
+    ref = np.power(t.astype(np.longdouble), np.longdouble(q) - np.longdouble(1.0))
+    rel = np.abs((got.astype(np.longdouble) - ref) / ref).astype(np.float64)
+    assert rel.max() <= tol_eps * EPS, rel.max() / EPS
+
+
+def test_pow_qm1_domain():
+    assert np.isnan(oracle.pow_qm1(0.0, 1.03))
+    assert np.isnan(oracle.pow_qm1(-1.0, 1.03))
+    assert np.isnan(oracle.pow_qm1(np.inf, 1.03))
+    assert np.isnan(oracle.pow_qm1(2.0 ** 64, 1.03))
+    assert np.isnan(oracle.pow_qm1(2.0 ** -65, 1.03))
+    assert oracle.pow_qm1(2.0 ** -64, 1.03) == pytest.approx((2.0 ** -64) ** 0.03, rel=1e-15)
+    # exact cases of the definition: 1^a = 1, t^0 = 1
+    assert oracle.pow_qm1(1.0, 1.03) == pytest.approx(1.0, rel=4 * EPS)
+    assert oracle.pow_qm1(37.5, 1.0) == pytest.approx(1.0, rel=4 * EPS)
+
+
+# ------------------------------------------------------------------ R1: support search
+def _numpy_knn(nodes, qpts, k):
+    out = np.empty((len(qpts), k), dtype=np.int32)
+    ids = np.arange(len(nodes))
+    for i, x in enumerate(qpts):
+        d = nodes - x
+        d2 = (d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]) + d[:, 2] * d[:, 2]
+        order = np.lexsort((ids, d2))[:k]
+        out[i] = np.sort(order)
+    return out
+
+
+@pytest.mark.parametrize("name", ["patch", "cantilever"])
+def test_knn_regular_grids_with_exact_ties(name):
+    w = workloads.config(name)
+    sel = np.arange(0, w.Nq, max(1, w.Nq // 700))
+    ref = _numpy_knn(w.nodes, w.qpts[sel], w.k)
+    assert (oracle.knn(w.nodes, w.qpts[sel], w.k, "brute") == ref).all()
+    assert (oracle.knn(w.nodes, w.qpts[sel], w.k, "grid") == ref).all()
+    # H7: ties between the k-th and (k+1)-th neighbour really occur on regular grids
+    d = w.nodes[None, :, :] - w.qpts[sel][:64, None, :]
+    d2 = np.sort((d[..., 0] ** 2 + d[..., 1] ** 2) + d[..., 2] ** 2, axis=1)
+    assert (d2[:, w.k - 1] == d2[:, w.k]).any()
+
+
+@pytest.mark.parametrize("k", [8, 40, 60])
+def test_knn_jittered_block_grid_equals_brute(k):
+    w = workloads.make_block("t", 14, 11, 9, 1.0, 2, k, 1e9, 0.3, jitter=0.3, seed=11)
+    sel = np.arange(0, w.Nq, 7)
+    ref = _numpy_knn(w.nodes, w.qpts[sel], k)
+    assert (oracle.knn(w.nodes, w.qpts[sel], k, "grid") == ref).all()
+    assert (oracle.knn(w.nodes, w.qpts[sel], k, "brute") == ref).all()
+    # query points outside the node bounding box and exactly on nodes
+    far = np.array([[-3.0, -2.0, -1.0], [20.0, 5.0, 4.0], *w.nodes[[0, 5, 77]]])
+    assert (oracle.knn(w.nodes, far, k, "grid") == _numpy_knn(w.nodes, far, k)).all()
+
+
+def test_knn_k_equals_N():
+    w = workloads.make_block("t", 3, 3, 3, 1.0, 1, 27, 1e9, 0.3)
+    s = oracle.knn(w.nodes, w.qpts, 27, "grid")
+    assert (s == np.arange(27)[None, :]).all()
+
+
+# ------------------------------------------------------------------ R2: pattern
+def _check_pattern_invariants(row_ptr, col_idx, support, N):
+    assert row_ptr[0] == 0 and (np.diff(row_ptr) >= 0).all()
+    nnz = row_ptr[-1]
+    assert nnz == len(col_idx) and nnz % 9 == 0
+    A = sp.csr_matrix((np.ones(nnz), col_idx, row_ptr), shape=(3 * N, 3 * N))
+    for r in range(0, 3 * N, max(1, 3 * N // 400)):
+        c = col_idx[row_ptr[r]:row_ptr[r + 1]]
+        assert (np.diff(c) > 0).all()                       # strictly sorted
+        assert r in c                                       # diagonal present
+    assert (A != A.T).nnz == 0                              # structurally symmetric
+    lens = np.diff(row_ptr).reshape(N, 3)
+    assert (lens[:, 0] == lens[:, 1]).all() and (lens[:, 0] == lens[:, 2]).all()
+    # brute-force union on the block level
+    blocks = set()
+    for s in support:
+        for i in s:
+            for j in s:
+                blocks.add((int(i), int(j)))
+    assert len(blocks) * 9 == nnz
+    rows = np.repeat(np.arange(3 * N), np.diff(row_ptr))
+    got = set(zip((rows // 3).tolist(), (col_idx // 3).tolist()))
+    assert got == blocks
+
+
+def test_pattern_invariants_and_counts(golden_dir):
+    counts = json.load(open(os.path.join(golden_dir, "pattern_counts.json")))
+    w = workloads.config("patch")
+    s = oracle.knn(w.nodes, w.qpts, w.k, "grid")
+    rp, ci = oracle.pattern(s, w.N)
+    _check_pattern_invariants(rp, ci, s, w.N)
+    assert rp[-1] == counts["patch"]["nnz"] == 91575          # SURVEY.md 8(c) pins: 10,175 blocks
+    w = workloads.make_block("t", 7, 6, 5, 1.0, 2, 20, 1e9, 0.3, jitter=0.3, seed=2)
+    s = oracle.knn(w.nodes, w.qpts, w.k, "grid")
+    rp, ci = oracle.pattern(s, w.N)
+    _check_pattern_invariants(rp, ci, s, w.N)
+
+
+def test_pattern_counts_cantilever(golden_dir):
+    counts = json.load(open(os.path.join(golden_dir, "pattern_counts.json")))
+    w = workloads.config("cantilever")
+    s = oracle.knn(w.nodes, w.qpts, w.k, "grid")
+    rp, ci = oracle.pattern(s, w.N)
+    assert rp[-1] == counts["cantilever"]["nnz"] == 1186893   # SURVEY.md 8(c) pins: 131,877 blocks
+    assert rp[-1] // 9 == counts["cantilever"]["blocks"] == 131877
+
+
+# ------------------------------------------------------------------ R3-R7: shape functions
+CASES = [
+    ("patch", dict()),
+    ("jit40", dict(nx=9, ny=8, nz=7, h=1.0, gauss=2, k=40, jitter=0.3, seed=5)),
+    ("jit60", dict(nx=9, ny=9, nz=8, h=1.0, gauss=2, k=60, jitter=0.3, seed=6)),
+    ("jit30h", dict(nx=8, ny=8, nz=8, h=0.5, gauss=1, k=30, jitter=0.25, seed=7)),
+]
+
+
+def _case(name, kw):
+    if name == "patch":
+        return workloads.config("patch")
+    return workloads.make_block(name, kw["nx"], kw["ny"], kw["nz"], kw["h"], kw["gauss"], kw["k"], 1e9, 0.3,
+                                jitter=kw["jitter"], seed=kw["seed"])
+
+
+@pytest.mark.parametrize("name,kw", CASES)
+def test_shape_function_invariants(name, kw):
+    w = _case(name, kw)
+    sel = np.arange(0, w.Nq, max(1, w.Nq // 400))
+    pts = w.qpts[sel]
+    s = oracle.knn(w.nodes, pts, w.k, "grid")
+    phi, dphi, sing = oracle.shape(w.nodes, pts, s, w.alpha_c, w.d_c, w.q)
+    assert sing.sum() == 0
+    X = w.nodes[s]
+    assert np.abs(phi.sum(1) - 1.0).max() < 1e-12                               # partition of unity
+    assert np.abs(dphi.sum(2)).max() * w.h < 1e-12                              # sum grad phi = 0
+    assert np.abs(np.einsum("mk,mkb->mb", phi, X) - pts).max() < 1e-11 * max(1.0, np.abs(pts).max())
+    assert np.abs(np.einsum("mak,mkb->mab", dphi, X) - np.eye(3)).max() < 1e-11  # linear reproduction
+    # the definition in long double (plain G in global coordinates, powl, textbook LU):
+    pr, dr = oracle.shape_dense_ref(w.nodes, pts, s, w.alpha_c, w.d_c, w.q)
+    assert np.abs(phi - pr).max() / np.abs(pr).max() < 2e-7      # cond(G) ~ 1e8..4e9 times eps
+    assert np.abs(dphi - dr).max() / np.abs(dr).max() < 2e-7
+
+
+def test_shape_kronecker_delta():
+    w = _case(*CASES[1])
+    nodes_sel = np.arange(0, w.N, 9)
+    pts = w.nodes[nodes_sel]
+    s = oracle.knn(w.nodes, pts, w.k, "grid")
+    phi, _, sing = oracle.shape(w.nodes, pts, s, w.alpha_c, w.d_c, w.q)
+    assert sing.sum() == 0
+    expect = (s == nodes_sel[:, None].astype(np.int32)).astype(float)
+    assert expect.sum() == len(nodes_sel)
+    assert np.abs(phi - expect).max() < 1e-9
+
+
+def test_shape_translation_and_scale_invariance():
+    # shape functions depend only on relative, dimensionless geometry
+    w = _case(*CASES[3])
+    pts = w.qpts[::37]
+    s = oracle.knn(w.nodes, pts, w.k, "grid")
+    phi, dphi, _ = oracle.shape(w.nodes, pts, s, w.alpha_c, w.d_c, w.q)
+    phi2, dphi2, _ = oracle.shape(w.nodes * 4.0, pts * 4.0, s, w.alpha_c, w.d_c * 4.0, w.q)
+    assert np.array_equal(phi, phi2)                 # scaling by a power of two is exact
+    assert np.array_equal(dphi, dphi2 * 4.0)
+    off = np.array([100.0, -50.0, 25.0])
+    phi3, dphi3, _ = oracle.shape(w.nodes + off, pts + off, s, w.alpha_c, w.d_c, w.q)
+    assert np.abs(phi - phi3).max() < 1e-6 and np.abs(dphi - dphi3).max() < 1e-5
+
+
+def test_shape_singular_support_is_flagged():
+    # all support nodes in one plane: P has rank 3, the moment matrix is singular
+    nodes = np.array([[i, j, 0.0] for i in range(4) for j in range(4)])
+    s = np.arange(16, dtype=np.int32)[None, :]
+    phi, dphi, sing = oracle.shape(nodes, np.array([[1.3, 1.6, 0.0]]), s, 4.0, 1.0, 1.03)
+    assert sing[0] == 1 and not phi.any() and not dphi.any()
+
+
+# ------------------------------------------------------------------ R8-R10: assembly, loads, penalty
+def _assemble(w, support=None):
+    s = oracle.knn(w.nodes, w.qpts, w.k, "grid") if support is None else support
+    rp, ci = oracle.pattern(s, w.N)
+    vals, f, ns = oracle.assemble(w.nodes, w.qpts, w.qw, s, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, rp, ci)
+    assert ns == 0
+    return s, rp, ci, vals, f
+
+
+def _rigid_modes(nodes):
+    N = len(nodes)
+    R = np.zeros((3 * N, 6))
+    x, y, z = nodes.T
+    for c in range(3):
+        R[c::3, c] = 1.0
+    R[0::3, 3], R[1::3, 3] = -y, x
+    R[1::3, 4], R[2::3, 4] = -z, y
+    R[0::3, 5], R[2::3, 5] = z, -x
+    return R
+
+
+def _elastic_D(E, nu):
+    lam = E * nu / ((1 + nu) * (1 - 2 * nu))
+    mu = E / (2 * (1 + nu))
+    D = np.zeros((6, 6))
+    D[:3, :3] = lam
+    D[np.arange(3), np.arange(3)] += 2 * mu
+    D[np.arange(3, 6), np.arange(3, 6)] = mu
+    return D
+
+
+@pytest.mark.parametrize("which", ["patch", "jit"])
+def test_stiffness_invariants(which):
+    if which == "patch":
+        w = workloads.config("patch")
+    else:
+        w = workloads.make_block("jit", 7, 6, 6, 1.0, 2, 30, 5e9, 0.3, jitter=0.3, seed=9,
+                                 body=(0.0, 0.0, -2500 * 9.81))
+    s, rp, ci, vals, f = _assemble(w)
+    K = sp.csr_matrix((vals, ci, rp), shape=(3 * w.N, 3 * w.N))
+    kmax = K.diagonal().max()
+    assert abs(w.qw.sum() - w.volume) < 1e-12 * w.volume
+    assert abs(K - K.T).max() / kmax < 1e-15                                   # symmetry (A2)
+    assert np.abs(K @ _rigid_modes(w.nodes)).max() / (kmax * np.abs(w.nodes).max()) < 1e-13
+    assert (K.diagonal() > 0).all()
+    # energy identity for linear fields (A3 (ii)): v^T K u = Vol * eps_v^T D eps_u
+    D = _elastic_D(w.E, w.nu)
+    rng = np.random.default_rng(3)
+    for _ in range(6):
+        Hu, Hv = rng.standard_normal((3, 3)), rng.standard_normal((3, 3))
+        u = (w.nodes @ Hu.T).reshape(-1)
+        v = (w.nodes @ Hv.T).reshape(-1)
+
+        def voigt(H):
+            e = 0.5 * (H + H.T)
+            return np.array([e[0, 0], e[1, 1], e[2, 2], 2 * e[0, 1], 2 * e[1, 2], 2 * e[2, 0]])
+        expect = w.volume * voigt(Hv) @ D @ voigt(Hu)
+        got = v @ (K @ u)
+        scale = w.volume * np.abs(D).max() * np.abs(Hu).max() * np.abs(Hv).max()
+        assert abs(got - expect) / scale < 1e-11
+    # load resultants: sum_I f_I = b * Vol ; sum_I x_I x f_I = sum_q w x_q x b
+    F = f.reshape(-1, 3)
+    assert np.abs(F.sum(0) - w.body * w.volume).max() <= 1e-12 * max(1.0, np.abs(w.body).max() * w.volume)
+    mom = np.cross(w.nodes, F).sum(0)
+    mom_ref = np.cross((w.qw[:, None] * w.qpts).sum(0), w.body)
+    assert np.abs(mom - mom_ref).max() <= 1e-11 * max(1.0, np.abs(mom_ref).max())
+
+
+def test_assembly_is_sum_of_point_contributions_and_row_restriction():
+    w = workloads.make_block("jit", 6, 6, 5, 1.0, 2, 20, 5e9, 0.3, jitter=0.3, seed=1, body=(1.0, 2.0, 3.0))
+    s, rp, ci, vals, f = _assemble(w)
+    # closed form of w*B^T D B for an isotropic D from the oracle's own phi / grad phi
+    phi, dphi, _ = oracle.shape(w.nodes, w.qpts, s, w.alpha_c, w.d_c, w.q)
+    lam = w.E * w.nu / ((1 + w.nu) * (1 - 2 * w.nu))
+    mu = w.E / (2 * (1 + w.nu))
+    Kd = np.zeros((3 * w.N, 3 * w.N))
+    for p in range(w.Nq):
+        g = dphi[p].T                                  # (k, 3)
+        gg = g @ g.T
+        blk = lam * np.einsum("ia,jb->iajb", g, g) + mu * np.einsum("ib,ja->iajb", g, g) \
+            + mu * np.einsum("ij,ab->iajb", gg, np.eye(3))
+        idx = (3 * s[p][:, None] + np.arange(3)[None, :]).reshape(-1)
+        Kd[np.ix_(idx, idx)] += w.qw[p] * blk.reshape(3 * w.k, 3 * w.k)
+    K = sp.csr_matrix((vals, ci, rp), shape=(3 * w.N, 3 * w.N)).toarray()
+    assert np.abs(K - Kd).max() / np.abs(np.diag(K)).max() < 1e-14
+    # restriction to a node range gives exactly the same rows
+    lo, hi = 40, 77
+    sub_rp = rp[3 * lo:3 * hi + 1] - rp[3 * lo]
+    sub_ci = ci[rp[3 * lo]:rp[3 * hi]]
+    v2, f2, _ = oracle.assemble(w.nodes, w.qpts, w.qw, s, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body,
+                                sub_rp, sub_ci, lo, hi)
+    assert np.array_equal(v2, vals[rp[3 * lo]:rp[3 * hi]])
+    assert np.array_equal(f2, f[3 * lo:3 * hi])
+
+
+def test_penalty_changes_exactly_the_constrained_diagonals():
+    w = workloads.make_block("jit", 6, 5, 5, 1.0, 2, 20, 5e9, 0.3, jitter=0.2, seed=4,
+                             body=(0.0, 0.0, -1.0), bc="bottom+roller")
+    s, rp, ci, vals, f = _assemble(w)
+    rng = np.random.default_rng(0)
+    ubar = rng.standard_normal((len(w.bc_nodes), 3))
+    v2, f2 = vals.copy(), f.copy()
+    K0 = sp.csr_matrix((vals, ci, rp), shape=(3 * w.N, 3 * w.N))
+    alpha = oracle.penalty(w.bc_nodes, w.bc_mask, ubar, 1e8, True, w.N, rp, ci, v2, f2)
+    assert alpha == 1e8 * K0.diagonal().max()
+    dv, df = v2 - vals, f2 - f
+    K1 = sp.csr_matrix((v2, ci, rp), shape=(3 * w.N, 3 * w.N))
+    dof_mask = np.zeros(3 * w.N, dtype=bool)
+    ub = np.zeros(3 * w.N)
+    for i, (nd, m) in enumerate(zip(w.bc_nodes, w.bc_mask)):
+        for c in range(3):
+            if (m >> c) & 1:
+                dof_mask[3 * nd + c] = True
+                ub[3 * nd + c] = ubar[i, c]
+    assert np.count_nonzero(dv) == dof_mask.sum()
+    assert np.array_equal(K1.diagonal()[dof_mask], K0.diagonal()[dof_mask] + alpha)
+    assert np.array_equal(K1.diagonal()[~dof_mask], K0.diagonal()[~dof_mask])
+    assert np.array_equal(f2[dof_mask], f[dof_mask] + alpha * ub[dof_mask])
+    assert not df[~dof_mask].any()
+    # absolute alpha, no mask = all three DOFs
+    v3, f3 = vals.copy(), f.copy()
+    a3 = oracle.penalty(w.bc_nodes[:3], None, ubar[:3], 123.0, False, w.N, rp, ci, v3, f3)
+    assert a3 == 123.0 and np.count_nonzero(v3 - vals) == 9
+
+
+def test_cantilever_tip_deflection_closed_form():
+    """BASELINE.json configs[1]: 10 x 1 x 1 beam, x = 0 clamped by penalty, end shear 1e6 Pa.
+    Euler-Bernoulli P L^3 / (3 E I) = 0.13333 m, with Timoshenko shear term about 0.1343 m
+    (SURVEY.md 8(c) pins: within 1 %)."""
+    w = workloads.config("cantilever")
+    s, rp, ci, vals, f = _assemble(w)
+    ls = oracle.knn(w.nodes, w.load_pts, w.k, "grid")
+    oracle.point_loads(w.nodes, w.load_pts, w.load_w, w.load_t, ls, w.alpha_c, w.d_c, w.q, f)
+    F = f.reshape(-1, 3)
+    assert np.abs(F.sum(0) - np.array([0.0, 0.0, -1e6])).max() < 1e-6       # total load = t * area
+    oracle.penalty(w.bc_nodes, w.bc_mask, w.bc_ubar, w.penalty_alpha, True, w.N, rp, ci, vals, f)
+    K = sp.csc_matrix(sp.csr_matrix((vals, ci, rp), shape=(3 * w.N, 3 * w.N)))
+    u = spla.spsolve(K, f).reshape(-1, 3)
+    tip = u[np.isclose(w.nodes[:, 0], 10.0), 2].mean()
+    P, L, E, I = 1e6, 10.0, w.E, 1.0 / 12.0
+    euler = -P * L ** 3 / (3 * E * I)
+    G = E / (2 * (1 + w.nu))
+    timo = euler - P * L / ((5.0 / 6.0) * G * 1.0)
+    assert abs(tip - euler) / abs(euler) < 0.01 or abs(tip - timo) / abs(timo) < 0.01, (tip, euler, timo)
+    assert np.abs(u[w.bc_nodes]).max() < 1e-6 * abs(tip)                    # clamped face
+
+
+def test_patch_test_solved_field_is_close_not_exact():
+    """Gauss-integrated RPIM does not pass the solved patch test exactly; the
+    error is ~1e-2 (reported), while reproduction at quadrature points is exact (above)."""
+    w = workloads.config("patch")
+    s, rp, ci, vals, f = _assemble(w)
+    oracle.penalty(w.bc_nodes, w.bc_mask, w.bc_ubar, w.penalty_alpha, True, w.N, rp, ci, vals, f)
+    K = sp.csc_matrix(sp.csr_matrix((vals, ci, rp), shape=(3 * w.N, 3 * w.N)))
+    u = spla.spsolve(K, f).reshape(-1, 3)
+    exact = 1e-3 * (w.nodes[:, 0] + 2 * w.nodes[:, 1] + 3 * w.nodes[:, 2])
+    err = np.abs(u - exact[:, None]).max() / np.abs(exact).max()
+    assert err < 0.05
+    assert np.abs(u[w.bc_nodes] - w.bc_ubar).max() / np.abs(exact).max() < 1e-6
+
+
+def test_paper_example1_closed_form(golden_dir):
+    g = json.load(open(os.path.join(golden_dir, "paper_example1.json")))
+    # the paper's "theoretical" value is rho * g * H; context only
+    sigma = g["density_kg_m3"] * g["inferred"]["g"] * g["inferred"]["height_m"] / 1e6
+    assert sigma == pytest.approx(g["theoretical_bottom_stress_MPa"], abs=5e-4)
+    assert g["numerical_bottom_stress_MPa"] / g["theoretical_bottom_stress_MPa"] == pytest.approx(1 - 0.0675, abs=1e-3)

@@ -1,0 +1,382 @@
+#!/usr/bin/env python
+"""bench.py -- RPIM assembly throughput on B200 (quad-points/s, fp64), the BASELINE.json metric.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config large] [--impl reference]
+
+A "step" is one pass of the whole hot path over one synthetic
+workload: rpim_build_pattern (kNN + CSR pattern) -> rpim_get_pattern -> rpim_assemble (shape functions,
+B^T D B, deterministic reduction into CSR, body force) -> rpim_apply_penalty.  `value` = quadrature
+points processed per second, inputs resident in HBM, timed with CUDA events on the launching stream,
+max over ranks.  Extra keys give the assemble+penalty-only rate (the paper's stage 1+2, DESIGN.md
+R12), the per-phase kernel times, the roofline of the dominant kernel, the end-to-end rate through
+the host-buffer C ABI calls (pinned host buffers, H2D/D2H inside the timed region), and the CPU
+oracle timed on a bounded sample of the same workload (a reported baseline, not the target).
+
+N > 1 (torchrun, one rank per GPU): the path partitions (quadrature points and matrix rows are
+independent per spatial partition), so every rank assembles its own partition of the
+same size with no data-path collective: weak scaling, value = total points / max-over-ranks time.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands, one host core) on bounded samples
+of the same workload; under torchrun only rank 0 runs it.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads  # noqa: E402
+
+METRIC = "rpim_assembly_quad_points_per_sec"
+UNIT = "quad-points/s"
+FP64_LANES_PER_SM = 64            # DFMA lanes per SM per clock (4 SMSP x 16), DESIGN.md section 5
+N_SM = 148
+
+
+def read_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+def flops_per_point(k: int):
+    """Algorithmic fp64 flops per quadrature point of THIS implementation,
+    fma = 2.  Returns (shape_flops, reduce_flops)."""
+    n = k + 4
+    pairs = k * (k + 1) // 2
+    build = pairs * (7 + 2 * 10 + 3 + 1) + k * (6 + 2 * 10 + 3 + 5)   # t, pow (1+9 fma, 2 mul), t*P; rhs
+    m = n - 8
+    factor = 0
+    for i in range(4):                      # 2x2 pivots: 2 fma per trailing element + multipliers
+        r = n - 2 * (i + 1)
+        factor += 2 * 2 * (r * (r + 1) // 2) + 5 * r + 16 * r
+    factor += sum(2 * (j * (j + 1) // 2) + j + 8 * j for j in range(m))      # 1x1 pivots (+ 4 rhs)
+    back = 8 * (n * (n - 1) // 2) + 8 * n
+    shape = build + factor + back
+    reduce_ = k * k * 18 + k * 3                                              # S += (w g_I) x g_J : 9 fma
+    return shape, reduce_
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            parts = [p.strip() for p in r.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": float(max(mx)) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample_rate(w, budget_s: float = 15.0):
+    """CPU oracle (one core) on a bounded sample: the first S quadrature points of the workload, all
+    hot-path rows (kNN, pattern, shape functions, B^T D B assembly, penalty).  Returns (points/s, S, seconds)."""
+    import oracle
+
+    def run(S):
+        pts, qw = np.ascontiguousarray(w.qpts[:S]), np.ascontiguousarray(w.qw[:S])
+        t0 = time.perf_counter()
+        s = oracle.knn(w.nodes, pts, w.k, "grid")
+        # rows touched by the sample: a contiguous node range keeps the sample's pattern small
+        lo, hi = int(s.min()), int(s.max()) + 1
+        sub = (s - lo).astype(np.int32)
+        rp_, ci = oracle.pattern(sub, hi - lo)
+        vals, f, _ = oracle.assemble(w.nodes[lo:hi], pts, qw, sub, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, rp_, ci)
+        sel = (w.bc_nodes >= lo) & (w.bc_nodes < hi)
+        sel[sel] = np.diff(rp_)[3 * (w.bc_nodes[sel] - lo)] > 0      # only nodes the sample touches have rows
+        if sel.any():
+            oracle.penalty(w.bc_nodes[sel] - lo, w.bc_mask[sel], w.bc_ubar[sel], w.penalty_alpha, True, hi - lo,
+                           rp_, ci, vals, f)
+        return time.perf_counter() - t0
+
+    S = min(w.Nq, 256)
+    t = run(S)
+    S2 = int(min(w.Nq, max(S, S * budget_s / max(t, 1e-3))))
+    if S2 > S:
+        S, t = S2, run(S2)
+    return S / t, S, t
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    rates = []
+    S = 0
+    per_step = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for i in range(args.warmup + args.steps):
+        r, S, t = oracle_sample_rate(w, budget_s=per_step)
+        if i >= args.warmup:
+            rates.append((S, t))
+    tot_pts = sum(s for s, _ in rates)
+    tot_t = sum(t for _, t in rates)
+    value = tot_pts / tot_t
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / max(1, args.steps),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "N": w.N, "Nq": w.Nq, "k": w.k, "sample_points_per_step": S},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": f"first {S} quadrature points per step, all hot-path rows"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="large", choices=workloads.CONFIG_NAMES)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        args.warmup = max(args.warmup, 3) if os.environ.get("RPIM_BENCH_STRICT_WARMUP", "1") == "1" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    w = workloads.config(args.config)
+    if world > 1:
+        # weak scaling: every rank assembles its own partition (same size, its own jitter stream)
+        seed = int(w.meta.get("seed", 0)) + 1000 * rank
+        if w.meta.get("jitter", 0.0) > 0:
+            nx, ny, nz = w.grid
+            w = workloads.make_block(w.name, nx, ny, nz, w.h, w.meta["gauss"], w.k, w.E, w.nu, jitter=w.meta["jitter"],
+                                     seed=seed, body=tuple(w.body), bc=w.meta["bc"], index_bits=w.index_bits)
+
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_1802_04256_b200 as rp
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    hbm_gbs, sm_max_mhz, peak_src = read_peaks()
+    ctx = rp.Context(local_rank)
+    d_nodes = torch.from_numpy(w.nodes).to(dev)
+    d_qpts = torch.from_numpy(w.qpts).to(dev)
+    d_qw = torch.from_numpy(w.qw).to(dev)
+    d_bcn = torch.from_numpy(w.bc_nodes).to(dev)
+    d_bcm = torch.from_numpy(w.bc_mask).to(dev)
+    d_bcu = torch.from_numpy(w.bc_ubar).to(dev)
+
+    # first pass sizes the outputs (pattern is data dependent)
+    nnz, bits = ctx.build_pattern(d_nodes, d_qpts, w.k, w.index_bits)
+    idt = torch.int32 if bits == 32 else torch.int64
+    d_rp = torch.empty(3 * w.N + 1, dtype=idt, device=dev)
+    d_ci = torch.empty(nnz, dtype=idt, device=dev)
+    d_vals = torch.empty(nnz, dtype=torch.float64, device=dev)
+    d_f = torch.empty(3 * w.N, dtype=torch.float64, device=dev)
+
+    def step():
+        n2, _ = ctx.build_pattern(d_nodes, d_qpts, w.k, w.index_bits)
+        assert n2 == nnz
+        ctx.get_pattern(d_rp, d_ci, None)
+        ctx.assemble(d_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f, want_singular=False)
+        ctx.apply_penalty(d_bcn, d_bcm, d_bcu, w.penalty_alpha, True, d_vals, d_f)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    ctx.phase_totals(reset=True)
+    launches0 = ctx.launch_count()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    stream = torch.cuda.current_stream(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else None
+    launches = ctx.launch_count() - launches0
+    phase_ms, calls = ctx.phase_totals(reset=True)
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * w.Nq / (ms_step * 1e-3)
+
+    # assemble + penalty only (paper stages 1 + 2), same timing discipline
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        ctx.assemble(d_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f, want_singular=False)
+        ctx.apply_penalty(d_bcn, d_bcm, d_bcu, w.penalty_alpha, True, d_vals, d_f)
+    e1.record(stream)
+    barrier()
+    ms_asm = e0.elapsed_time(e1) / args.steps
+
+    # ------------------------------------------------ roofline of the dominant kernel (live CUDA events)
+    n_asm = max(1, calls[1])
+    shape_ms, reduce_ms = phase_ms[3] / n_asm, phase_ms[4] / n_asm
+    fl_shape, fl_reduce = flops_per_point(w.k)
+    peak_tflops = N_SM * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    if shape_ms >= reduce_ms:
+        dom, dom_ms, dom_fl = "shape_functions", shape_ms, fl_shape * w.Nq
+    else:
+        dom, dom_ms, dom_fl = "reduce_into_csr", reduce_ms, fl_reduce * w.Nq
+    achieved = dom_fl / (dom_ms * 1e-3) / 1e12
+    roofline = {
+        "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+        "frac": achieved / peak_tflops, "traffic": None,
+        "peak_source": f"derived: {N_SM} SM x {FP64_LANES_PER_SM} DFMA/clk x 2 x {sm_max_mhz:.0f} MHz (DESIGN.md section 5)",
+        "kernel_ms": {"shape_functions": shape_ms, "reduce_into_csr": reduce_ms,
+                      "knn": phase_ms[0] / max(1, calls[0]), "incidence": phase_ms[1] / max(1, calls[0]),
+                      "block_pattern": phase_ms[2] / max(1, calls[0])},
+        "assemble_flops_per_point": fl_shape + fl_reduce,
+        "assemble_fp64_frac": (fl_shape + fl_reduce) * w.Nq / (ms_asm * 1e-3) / 1e12 / peak_tflops,
+        "assemble_hbm_min_bytes": nnz * 8 + w.Nq * w.k * 4 + w.Nq * 32 + w.N * 24 + 3 * w.N * 8,
+        "assemble_hbm_frac": (nnz * 8 + w.Nq * w.k * 4 + w.Nq * 32 + w.N * 24 + 3 * w.N * 8) / (ms_asm * 1e-3) / 1e9 / hbm_gbs,
+        "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": peak_src,
+    }
+
+    # ------------------------------------------------ end to end through the host-buffer C ABI calls
+    e2e = None
+    if not args.no_e2e:
+        try:
+            np_idt = np.int32 if bits == 32 else np.int64
+            pin = lambda a: torch.from_numpy(a).pin_memory().numpy()  # noqa: E731
+            h_nodes, h_qpts, h_qw = pin(w.nodes), pin(w.qpts), pin(w.qw)
+            h_bcn, h_bcm, h_bcu = pin(w.bc_nodes), pin(w.bc_mask), pin(w.bc_ubar)
+            h_rp = torch.empty(3 * w.N + 1, dtype=idt).pin_memory().numpy()
+            h_ci = torch.empty(nnz, dtype=idt).pin_memory().numpy()
+            h_vals = torch.empty(nnz, dtype=torch.float64).pin_memory().numpy()
+            h_f = torch.empty(3 * w.N, dtype=torch.float64).pin_memory().numpy()
+            assert h_rp.dtype == np_idt
+
+            def e2e_step():
+                n2, _ = ctx.host_pattern(h_nodes, h_qpts, w.k, w.index_bits)
+                assert n2 == nnz
+                ctx.host_assemble(h_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, h_bcn, h_bcm, h_bcu,
+                                  w.penalty_alpha, True, h_rp, h_ci, h_vals, h_f)
+
+            e2e_step()
+            n_e2e = max(1, min(args.steps, 3))
+            barrier()
+            e0.record(stream)
+            for _ in range(n_e2e):
+                e2e_step()
+            e1.record(stream)
+            barrier()
+            ms_e2e = e0.elapsed_time(e1) / n_e2e
+            if world > 1:
+                t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                ms_e2e = float(t.item())
+            h2d = h_nodes.nbytes + h_qpts.nbytes + h_qw.nbytes + h_bcn.nbytes + h_bcm.nbytes + h_bcu.nbytes
+            d2h = h_rp.nbytes + h_ci.nbytes + h_vals.nbytes + h_f.nbytes
+            e2e = {"value": world * w.Nq / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                   "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e, "steps": n_e2e,
+                   "api": "rpim_host_pattern + rpim_host_assemble (pinned host buffers)"}
+            del h_ci, h_vals
+        except Exception as ex:  # report, never fake
+            e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        r, S, t = oracle_sample_rate(w, budget_s=15.0)
+        cpu_baseline = {"value": r, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": t,
+                        "sample": f"first {S} quadrature points of '{w.name}', all hot-path rows (kNN, pattern, "
+                                  f"shape functions, B^T D B assembly, penalty); host has {os.cpu_count()} cores"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{w.name} (BASELINE.json configs[{workloads.CONFIG_NAMES.index(w.name)}])",
+                       "N": w.N, "Nq": w.Nq, "k": w.k, "nnz": nnz, "index_bits": bits,
+                       "step": "build_pattern + get_pattern + assemble + apply_penalty",
+                       "l2": "inputs and outputs larger than L2 (no flush needed)" if nnz * 8 > 2.5e8 else
+                             "working set may fit L2; no flush",
+                       "parallelism": f"{world} independent partitions" if world > 1 else "single GPU"},
+            "assemble_penalty": {"value": world * w.Nq / (ms_asm * 1e-3), "unit": UNIT, "ms_per_step": ms_asm,
+                                 "gdof_entries_per_s": 9.0 * w.k * w.k * w.Nq * world / (ms_asm * 1e-3) / 1e9},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "cpu_baseline": cpu_baseline,
+        }
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

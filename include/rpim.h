@@ -1,0 +1,138 @@
+/*
+ * rpim.h -- C ABI of librpim: B200-native (sm_100a) RPIM global stiffness assembly with
+ * penalty enforcement of displacement boundary conditions (GeoMFree3D, arXiv 1802.04256).
+ *
+ * The calls follow the paper's stage split ("assemble the global stiffness
+ * matrix ... enforce the boundary conditions ... solve") and the names BASELINE.json
+ * north_star fixes: rpim_build_pattern, rpim_assemble, rpim_apply_penalty.  The exact
+ * arithmetic of every step is the set of readings R1..R12 in DESIGN.md section 2.
+ *
+ * Conventions
+ *   - "d_" arguments are DEVICE pointers (caller-owned, e.g. torch tensors); "h_" and
+ *     "out_" arguments and small by-value arrays are HOST pointers.
+ *   - All coordinate / value arrays are fp64, row-major, densely packed.
+ *   - DOF id = 3*node + component.  CSR rows are strictly ascending, every structural 3x3
+ *     block stores all nine entries, the diagonal is always present (R2).
+ *   - Every call returns 0 (RPIM_OK) or a negative rpim_status; rpim_last_error() gives a
+ *     text for the last failure on that context.  No call aborts, throws or prints.
+ *   - Work is enqueued on the stream given to rpim_create.  Calls that return host scalars
+ *     (out_*) synchronise that stream before returning; the others are asynchronous.
+ *   - The context owns only its internal workspace (cell grid, supports, incidence lists,
+ *     block pattern, staged shape functions); it is freed by rpim_destroy.  The node and
+ *     point arrays passed to rpim_build_pattern must stay valid and unchanged until the
+ *     last rpim_assemble / rpim_add_point_loads that uses the pattern has completed.
+ *   - There is no CPU fallback anywhere: without a CUDA device rpim_create fails.
+ */
+#ifndef RPIM_H
+#define RPIM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rpim_ctx rpim_ctx;
+
+typedef enum rpim_status {
+    RPIM_OK = 0,
+    RPIM_ERR_INVALID_ARG = -1,     /* null pointer, k < 4, k > N, k > RPIM_MAX_K, bad index_bits, ... */
+    RPIM_ERR_ALLOC = -2,           /* device or host allocation failed */
+    RPIM_ERR_CUDA = -3,            /* a CUDA runtime call or kernel failed */
+    RPIM_ERR_STATE = -4,           /* call order violated (e.g. assemble before build_pattern) */
+    RPIM_ERR_BC_NODE_INVALID = -5, /* boundary node id out of range */
+    RPIM_ERR_INDEX_OVERFLOW = -6,  /* 32-bit indices forced but nnz >= 2^31 */
+    RPIM_ERR_CAPACITY = -7         /* an on-chip work buffer would overflow (pathological node cloud) */
+} rpim_status;
+
+#define RPIM_MAX_K 124  /* moment systems up to 128 x 128 */
+
+/* Create a context on CUDA device `device`; all work goes to `cuda_stream` (a cudaStream_t,
+ * may be NULL for the default stream).  Fails with RPIM_ERR_CUDA when no device exists. */
+int rpim_create(rpim_ctx** out_ctx, int device, void* cuda_stream);
+int rpim_destroy(rpim_ctx* ctx);
+const char* rpim_last_error(const rpim_ctx* ctx);
+
+/* Bytes of device workspace currently owned by the context. */
+int64_t rpim_workspace_bytes(const rpim_ctx* ctx);
+
+/* Stage 0 (R1, R2; hot-path steps a1, a2): exact k-nearest-neighbour supports on a
+ * uniform cell grid and the CSR pattern of the 3N x 3N stiffness matrix.
+ *   d_nodes  N x 3 field-node coordinates        d_qpts  Nq x 3 quadrature points
+ *   k        support size (4 <= k <= min(N, RPIM_MAX_K))
+ *   index_bits  0 = auto (64 iff nnz > 2^31 - 1), 32 or 64: width of row_ptr AND col_idx
+ *   out_nnz, out_index_bits  host scalars (number of stored scalar entries, chosen width)
+ * Synchronises the stream. */
+int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const double* d_qpts,
+                       int64_t Nq, int k, int index_bits, int64_t* out_nnz, int* out_index_bits);
+
+/* Write the pattern built by rpim_build_pattern.
+ *   d_row_ptr  3N+1 entries, d_col_idx  nnz entries, both int32_t or int64_t per index_bits
+ *   d_support  Nq x k int32 node ids, ascending per point; may be NULL
+ * Any of the three may be NULL to skip it.  Asynchronous. */
+int rpim_get_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx, int32_t* d_support);
+
+/* Stage 1 (R3-R8; steps a3-a6): per quadrature point build and factor the
+ * (k+4)x(k+4) moment matrix, solve for the shape functions and their derivatives, form
+ * w * B^T D B and reduce it deterministically (fixed order, no floating-point atomics) into
+ * the CSR values; body-force load f_{3I+c} = sum_q w phi_I b_c.
+ *   d_qw    Nq quadrature weights           E, nu   isotropic elastic constants
+ *   alpha_c, d_c, q   multiquadric R(r) = (r^2 + (alpha_c*d_c)^2)^q
+ *   body    host array of 3 (force per unit volume)
+ *   d_vals  nnz fp64 values (overwritten)   d_f  3N fp64 (overwritten)
+ *   out_singular  host scalar: number of points whose moment matrix was singular (they
+ *                 contribute nothing); may be NULL, in which case the call is asynchronous. */
+int rpim_assemble(rpim_ctx* ctx, const double* d_qw, double E, double nu, double alpha_c,
+                  double d_c, double q, const double body[3], double* d_vals, double* d_f,
+                  int64_t* out_singular);
+
+/* Step a5b (R9): f_{3I+c} += w * phi_I(x) * t_c at M given points (face Gauss
+ * points of a traction boundary) using the shape parameters of the last rpim_assemble.
+ *   d_pts M x 3, d_w M, d_t M x 3, d_f 3N (updated in place).  Synchronises the stream. */
+int rpim_add_point_loads(rpim_ctx* ctx, const double* d_pts, const double* d_w, const double* d_t,
+                         int64_t M, double* d_f);
+
+/* Stage 2 (R10; step a7): penalty method, in place.
+ *   d_bc_nodes  m unique node ids            d_bc_mask  m bytes, bit c = constrain DOF c (NULL = all)
+ *   d_u_bar     m x 3 prescribed displacements
+ *   alpha, alpha_is_relative   alpha_used = alpha * max_d K_dd (before penalty) if relative
+ *   out_alpha_used  host scalar, may be NULL (then asynchronous unless an error check is needed) */
+int rpim_apply_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* d_bc_mask,
+                       const double* d_u_bar, int64_t m, double alpha, int alpha_is_relative,
+                       double* d_vals, double* d_f, double* out_alpha_used);
+
+/* Test / inspection accessor: shape functions staged by the last rpim_assemble.
+ *   d_phi Nq x k, d_dphi Nq x 3 x k (d/dx, d/dy, d/dz), d_singular Nq bytes; any may be NULL. */
+int rpim_get_shape(rpim_ctx* ctx, double* d_phi, double* d_dphi, uint8_t* d_singular);
+
+/* End-to-end variants with HOST buffers (pageable or pinned): copy inputs to the device,
+ * run the same kernels, copy results back, all on the context's stream, then synchronise.
+ * rpim_host_pattern builds the pattern and reports nnz so the caller can size the outputs of
+ * rpim_host_assemble, which runs get_pattern + assemble + apply_penalty and returns the CSR
+ * arrays, values and load vector.  bc arrays may be NULL with m = 0. */
+int rpim_host_pattern(rpim_ctx* ctx, const double* h_nodes, int64_t N, const double* h_qpts,
+                      int64_t Nq, int k, int index_bits, int64_t* out_nnz, int* out_index_bits);
+int rpim_host_assemble(rpim_ctx* ctx, const double* h_qw, double E, double nu, double alpha_c,
+                       double d_c, double q, const double body[3], const int64_t* h_bc_nodes,
+                       const uint8_t* h_bc_mask, const double* h_u_bar, int64_t m, double alpha,
+                       int alpha_is_relative, void* h_row_ptr, void* h_col_idx, double* h_vals,
+                       double* h_f, int64_t* out_singular, double* out_alpha_used);
+
+/* Per-phase device times (ms, CUDA events) of the last rpim_build_pattern / rpim_assemble:
+ * [0] grid+kNN  [1] incidence  [2] block pattern  [3] shape functions  [4] reduction into CSR.
+ * Host array of 5.  Synchronises. */
+int rpim_last_phase_ms(rpim_ctx* ctx, float out_ms[5]);
+
+/* Sum of the per-phase device times (ms, same five phases) over all rpim_build_pattern /
+ * rpim_assemble calls since the last reset, measured with CUDA events recorded on the context's
+ * stream around the kernels; out_calls = {build_pattern calls, assemble calls} (may be NULL).
+ * Synchronises.  reset != 0 clears the totals afterwards. */
+int rpim_phase_totals(rpim_ctx* ctx, double out_ms[5], int64_t out_calls[2], int reset);
+
+/* Number of kernels this library has launched on the context since creation. */
+int64_t rpim_launch_count(const rpim_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RPIM_H */

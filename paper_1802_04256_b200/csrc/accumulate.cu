@@ -1,0 +1,210 @@
+// Steps a5 + a6 (R8): w * B^T D B blocks and their deterministic reduction into the
+// CSR values, body-force load; step a5b (R9) point loads; step a7 (R10) penalty BCs.
+//
+// Reduction design: ROW OWNER.  Block row I (node I) is owned by one warp; it walks the node's
+// incidence list (points q whose support contains I, ascending q) and accumulates, for every
+// column J of supp(q), S_IJ += (w g_I) (x) g_J into an on-chip accumulator row.  Every CSR entry
+// is therefore summed in ascending q by exactly one warp: no floating-point atomics, bitwise
+// run-to-run reproducible, and K is written to HBM exactly once (never read).  The isotropic
+// closed form K_IJ = lambda S + mu S^T + mu tr(S) I is applied once per block at write-out.
+#include "common.cuh"
+
+namespace {
+
+__global__ void __launch_bounds__(256)
+accumulate_generic_kernel(int64_t N, int k, int Lcap, const int64_t* __restrict__ inc_ptr,
+                          const int32_t* __restrict__ inc_q, const uint8_t* __restrict__ inc_j,
+                          const int32_t* __restrict__ support, const double* __restrict__ stage,
+                          const double* __restrict__ qw, const int64_t* __restrict__ brow_ptr,
+                          const int32_t* __restrict__ bcol, double lambda, double mu, double bx, double by,
+                          double bz, double* __restrict__ vals, double* __restrict__ f) {
+    extern __shared__ double smem_d[];
+    const int nwarps = blockDim.x >> 5;
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double* acc = smem_d + (size_t)wid * ((size_t)Lcap * 9 + (Lcap + 1) / 2);
+    int* cols = (int*)(acc + (size_t)Lcap * 9);
+
+    for (int64_t I = (int64_t)blockIdx.x * nwarps + wid; I < N; I += (int64_t)gridDim.x * nwarps) {
+        const int64_t o = brow_ptr[I];
+        const int L = (int)(brow_ptr[I + 1] - o);
+        for (int s = lane; s < L; s += 32) cols[s] = bcol[o + s];
+        for (int s = lane; s < 9 * L; s += 32) acc[s] = 0.0;
+        __syncwarp();
+        double fI = 0.0;
+        const int64_t pa = inc_ptr[I], pb = inc_ptr[I + 1];
+        for (int64_t p = pa; p < pb; ++p) {
+            const int64_t q = inc_q[p];
+            const int i = inc_j[p];
+            const double w = qw[q];
+            const double* st = stage + q * 4 * (int64_t)k;
+            const double wgx = w * st[k + i], wgy = w * st[2 * k + i], wgz = w * st[3 * k + i];
+            fI += w * st[i];
+            const int32_t* sp = support + q * k;
+            for (int j = lane; j < k; j += 32) {
+                const int J = sp[j];
+                const double gx = st[k + j], gy = st[2 * k + j], gz = st[3 * k + j];
+                int lo = 0, hi = L - 1;   // J is always present in the row
+                while (lo < hi) {
+                    const int mid = (lo + hi) >> 1;
+                    if (cols[mid] < J) lo = mid + 1; else hi = mid;
+                }
+                double* a = acc + 9 * lo;
+                a[0] = fma(wgx, gx, a[0]); a[1] = fma(wgx, gy, a[1]); a[2] = fma(wgx, gz, a[2]);
+                a[3] = fma(wgy, gx, a[3]); a[4] = fma(wgy, gy, a[4]); a[5] = fma(wgy, gz, a[5]);
+                a[6] = fma(wgz, gx, a[6]); a[7] = fma(wgz, gy, a[7]); a[8] = fma(wgz, gz, a[8]);
+            }
+            __syncwarp();
+        }
+        // K_IJ = lambda S + mu S^T + mu tr(S) I, written row by row (each scalar row is contiguous)
+        for (int s = lane; s < L; s += 32) {
+            const double* a = acc + 9 * s;
+            const double mtr = mu * ((a[0] + a[4]) + a[8]);
+#pragma unroll
+            for (int r = 0; r < 3; ++r) {
+                double* dst = vals + 9 * o + (int64_t)r * 3 * L + 3 * s;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    double v = fma(lambda, a[3 * r + c], mu * a[3 * c + r]);
+                    if (r == c) v += mtr;
+                    dst[c] = v;
+                }
+            }
+        }
+        if (lane == 0) { f[3 * I] = fI * bx; f[3 * I + 1] = fI * by; f[3 * I + 2] = fI * bz; }
+        __syncwarp();
+    }
+}
+
+// one warp, points in order: f_{3J+c} += (w phi_J) t_c  (deterministic; M is small: face points)
+__global__ void point_loads_kernel(const int32_t* __restrict__ support, const double* __restrict__ stage,
+                                   const double* __restrict__ w, const double* __restrict__ t, int64_t M, int k,
+                                   double* __restrict__ f) {
+    const int lane = threadIdx.x;
+    for (int64_t p = 0; p < M; ++p) {
+        const double* st = stage + p * 4 * (int64_t)k;
+        const double wp = w[p], tx = t[3 * p], ty = t[3 * p + 1], tz = t[3 * p + 2];
+        for (int j = lane; j < k; j += 32) {
+            const int64_t J = support[p * k + j];
+            const double wphi = wp * st[j];
+            f[3 * J] += wphi * tx;
+            f[3 * J + 1] += wphi * ty;
+            f[3 * J + 2] += wphi * tz;
+        }
+        __syncwarp();
+        __threadfence_block();
+    }
+}
+
+// ------------------------------------------------------------------ penalty
+__global__ void diag_max_partial_kernel(int64_t N, const int64_t* __restrict__ brow_ptr,
+                                        const int* __restrict__ bdiag, const double* __restrict__ vals,
+                                        double* __restrict__ part) {
+    double m = 0.0;
+    for (int64_t I = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; I < N; I += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t o = brow_ptr[I];
+        const int64_t L = brow_ptr[I + 1] - o;
+        if (L == 0) continue;
+        const int64_t d = bdiag[I];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) m = fmax(m, vals[9 * o + a * 3 * L + 3 * d + a]);
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, d));
+    __shared__ double s[32];
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        m = (threadIdx.x < (blockDim.x >> 5)) ? s[threadIdx.x] : 0.0;
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, d));
+        if (threadIdx.x == 0) part[blockIdx.x] = m;
+    }
+}
+
+__global__ void diag_max_final_kernel(double* part, int nparts, double alpha, int relative) {
+    double m = 0.0;
+    for (int b = threadIdx.x; b < nparts; b += 32) m = fmax(m, part[b]);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, d));
+    __syncwarp();
+    if (threadIdx.x == 0) part[0] = relative ? alpha * m : alpha;
+}
+
+__global__ void penalty_apply_kernel(int64_t N, const int64_t* __restrict__ bc_nodes,
+                                     const uint8_t* __restrict__ bc_mask, const double* __restrict__ ubar, int64_t m,
+                                     const double* __restrict__ alpha_used, const int64_t* __restrict__ brow_ptr,
+                                     const int* __restrict__ bdiag, double* __restrict__ vals, double* __restrict__ f,
+                                     long long* __restrict__ flags) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m) return;
+    const int64_t I = bc_nodes[i];
+    if (I < 0 || I >= N || brow_ptr[I + 1] == brow_ptr[I]) {
+        atomicAdd((unsigned long long*)&flags[FLAG_BC_BAD], 1ull);
+        return;
+    }
+    const double a = alpha_used[0];
+    const int mask = bc_mask ? bc_mask[i] : 7;
+    const int64_t o = brow_ptr[I], L = brow_ptr[I + 1] - o, d = bdiag[I];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        if (!((mask >> c) & 1)) continue;
+        vals[9 * o + c * 3 * L + 3 * d + c] += a;
+        f[3 * I + c] += a * ubar[3 * i + c];
+    }
+}
+
+}  // namespace
+
+int rpim_stage_accumulate(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
+                          double* d_vals, double* d_f) {
+    const int Lcap = std::max(ctx->max_blen, 1);
+    const size_t per_warp = ((size_t)Lcap * 9 + (Lcap + 1) / 2) * sizeof(double);
+    int warps = 8;
+    while (warps > 1 && per_warp * warps > 200 * 1024) --warps;
+    if (per_warp * warps > 220 * 1024) RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "block row of %d columns does not fit on chip", Lcap);
+    const size_t smem = per_warp * warps;
+    CUDA_TRY(ctx, cudaFuncSetAttribute(accumulate_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int per_sm = (int)std::max<size_t>(1, (220 * 1024) / (smem + 1024));
+    int64_t blocks = (ctx->N + warps - 1) / warps;
+    blocks = std::min<int64_t>(blocks, 148LL * per_sm * 8);
+    accumulate_generic_kernel<<<(unsigned)blocks, warps * 32, smem, ctx->stream>>>(
+        ctx->N, ctx->k, Lcap, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_support, ctx->d_stage, d_qw,
+        ctx->d_brow_ptr, ctx->d_bcol, lambda, mu, body[0], body[1], body[2], d_vals, d_f);
+    KERNEL_CHECK(ctx);
+    return RPIM_OK;
+}
+
+int rpim_stage_point_loads(rpim_ctx* ctx, const int32_t* d_support, const double* d_stage, const double* d_w,
+                           const double* d_t, int64_t M, double* d_f) {
+    if (M == 0) return RPIM_OK;
+    point_loads_kernel<<<1, 32, 0, ctx->stream>>>(d_support, d_stage, d_w, d_t, M, ctx->k, d_f);
+    KERNEL_CHECK(ctx);
+    return RPIM_OK;
+}
+
+int rpim_stage_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* d_bc_mask, const double* d_u_bar,
+                       int64_t m, double alpha, int relative, double* d_vals, double* d_f, double* out_alpha) {
+    cudaStream_t st = ctx->stream;
+    const int nparts = 592;
+    diag_max_partial_kernel<<<nparts, 256, 0, st>>>(ctx->N, ctx->d_brow_ptr, ctx->d_bdiag, d_vals, ctx->d_scratch);
+    KERNEL_CHECK(ctx);
+    diag_max_final_kernel<<<1, 32, 0, st>>>(ctx->d_scratch, nparts, alpha, relative);
+    KERNEL_CHECK(ctx);
+    if (m > 0) {
+        penalty_apply_kernel<<<(unsigned)((m + 127) / 128), 128, 0, st>>>(ctx->N, d_bc_nodes, d_bc_mask, d_u_bar, m,
+                                                                          ctx->d_scratch, ctx->d_brow_ptr,
+                                                                          ctx->d_bdiag, d_vals, d_f, ctx->d_flags);
+        KERNEL_CHECK(ctx);
+    }
+    double a = 0.0;
+    long long bad = 0;
+    CUDA_TRY(ctx, cudaMemcpyAsync(&a, ctx->d_scratch, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaMemcpyAsync(&bad, ctx->d_flags + FLAG_BC_BAD, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    if (out_alpha) *out_alpha = a;
+    if (bad) {
+        CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_BC_BAD, 0, sizeof(long long), st));
+        RPIM_FAIL(ctx, RPIM_ERR_BC_NODE_INVALID, "%lld boundary node ids are out of range or have no matrix row", bad);
+    }
+    return RPIM_OK;
+}

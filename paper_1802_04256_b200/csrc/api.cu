@@ -1,0 +1,353 @@
+// C ABI of librpim (include/rpim.h): argument checks, workspace ownership, stage sequencing.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+
+namespace {
+
+// DESIGN.md R5: coefficients and tables of the reproducible power function, evaluated on the
+// host in the library's own code (the oracle has its own, independent copy of this recipe).
+void fill_shape_params(double alpha_c, double d_c, double q, ShapeParams& P) {
+    P.inv_dc = 1.0 / d_c;
+    P.ac2 = alpha_c * alpha_c;
+    P.twoq = 2.0 * q;
+    const double a = q - 1.0;
+    P.pw.b[0] = 1.0;
+    for (int j = 1; j <= 9; ++j) P.pw.b[j] = (P.pw.b[j - 1] * (a - (double)(j - 1))) / (double)j;
+    for (int i = 0; i < 32; ++i) {
+        const double c = 1.0 + (double)(2 * i + 1) / 64.0;
+        P.pw.invc[i] = 1.0 / c;
+        P.pw.E[i] = (double)powl((long double)P.pw.invc[i], -(long double)a);
+    }
+    for (int e = -64; e <= 63; ++e) P.pw.F[e + 64] = (double)powl(2.0L, (long double)e * (long double)a);
+}
+
+void free_all(rpim_ctx* c) {
+    ws_free(c, &c->d_cell_of); ws_free(c, &c->d_cell_start); ws_free(c, &c->d_cell_cursor);
+    ws_free(c, &c->d_node_order); ws_free(c, &c->d_sorted_xyz); ws_free(c, &c->d_support);
+    ws_free(c, &c->d_inc_count); ws_free(c, &c->d_inc_ptr); ws_free(c, &c->d_inc_q); ws_free(c, &c->d_inc_j);
+    ws_free(c, &c->d_blen); ws_free(c, &c->d_brow_ptr); ws_free(c, &c->d_bcol); ws_free(c, &c->d_bdiag);
+    ws_free(c, &c->d_stage); ws_free(c, &c->d_singular); ws_free(c, &c->d_scratch);
+    ws_free(c, &c->h2d_nodes); ws_free(c, &c->h2d_qpts);
+    { int64_t* t = (int64_t*)c->d_scan_tmp; ws_free(c, &t); c->d_scan_tmp = nullptr; c->scan_tmp_elems = 0; }
+    c->have_pattern = c->have_shape = false;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rpim_create(rpim_ctx** out_ctx, int device, void* cuda_stream) {
+    if (!out_ctx) return RPIM_ERR_INVALID_ARG;
+    *out_ctx = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return RPIM_ERR_CUDA;
+    }
+    rpim_ctx* c = new (std::nothrow) rpim_ctx();
+    if (!c) return RPIM_ERR_ALLOC;
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    if (cudaSetDevice(device) != cudaSuccess) { delete c; return RPIM_ERR_CUDA; }
+    if (cudaMalloc((void**)&c->d_flags, NUM_FLAGS * sizeof(long long)) != cudaSuccess) { delete c; return RPIM_ERR_ALLOC; }
+    cudaMemset(c->d_flags, 0, NUM_FLAGS * sizeof(long long));
+    for (auto& e : c->ev) cudaEventCreate(&e);
+    *out_ctx = c;
+    return RPIM_OK;
+}
+
+int rpim_destroy(rpim_ctx* ctx) {
+    if (!ctx) return RPIM_OK;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    free_all(ctx);
+    if (ctx->d_flags) cudaFree(ctx->d_flags);
+    for (auto& e : ctx->ev) if (e) cudaEventDestroy(e);
+    for (auto& e : ctx->phase_events) cudaEventDestroy(e);
+    delete ctx;
+    return RPIM_OK;
+}
+
+const char* rpim_last_error(const rpim_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+int64_t rpim_workspace_bytes(const rpim_ctx* ctx) { return ctx ? ctx->ws_bytes : 0; }
+int64_t rpim_launch_count(const rpim_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const double* d_qpts, int64_t Nq, int k,
+                       int index_bits, int64_t* out_nnz, int* out_index_bits) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    if (!d_nodes || !d_qpts || N <= 0 || Nq <= 0) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "null pointer or empty input");
+    if (k < 4 || k > RPIM_MAX_K || k > N) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "k = %d must satisfy 4 <= k <= min(N, %d)", k, RPIM_MAX_K);
+    if (index_bits != 0 && index_bits != 32 && index_bits != 64) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "index_bits must be 0, 32 or 64");
+    if (N > 700000000 || Nq * (int64_t)k > 0x7fffffff00LL || Nq > 0x7fffffff) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "problem too large for 32-bit node / point ids");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    ctx->have_pattern = ctx->have_shape = false;
+    ws_free(ctx, &ctx->d_stage);
+    ws_free(ctx, &ctx->d_singular);
+    ctx->d_nodes = d_nodes; ctx->d_qpts = d_qpts; ctx->N = N; ctx->Nq = Nq; ctx->k = k;
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags, 0, NUM_FLAGS * sizeof(long long), st));
+    int rc;
+    if ((rc = ws_alloc(ctx, &ctx->d_support, Nq * k))) return rc;
+    cudaEventRecord(ctx->ev[0], st);
+    if ((rc = rpim_stage_grid_knn(ctx, d_qpts, Nq, k, ctx->d_support, true))) return rc;
+    cudaEventRecord(ctx->ev[1], st);
+    if ((rc = rpim_stage_incidence(ctx))) return rc;
+    cudaEventRecord(ctx->ev[2], st);
+    if ((rc = rpim_stage_block_pattern(ctx))) return rc;
+    cudaEventRecord(ctx->ev[3], st);
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    for (int i = 0; i < 3; ++i) {
+        cudaEventElapsedTime(&ctx->phase_ms[i], ctx->ev[i], ctx->ev[i + 1]);
+        ctx->phase_total_ms[i] += ctx->phase_ms[i];
+    }
+    ctx->phase_calls[0]++;
+    const int64_t nnz = 9 * ctx->nnzb;
+    int bits = index_bits ? index_bits : (nnz > 0x7fffffffLL ? 64 : 32);
+    if (bits == 32 && nnz > 0x7fffffffLL) RPIM_FAIL(ctx, RPIM_ERR_INDEX_OVERFLOW, "nnz = %lld does not fit 32-bit indices", (long long)nnz);
+    ctx->index_bits = bits;
+    ctx->have_pattern = true;
+    if (out_nnz) *out_nnz = nnz;
+    if (out_index_bits) *out_index_bits = bits;
+    return RPIM_OK;
+}
+
+int rpim_get_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx, int32_t* d_support) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    if (!ctx->have_pattern) RPIM_FAIL(ctx, RPIM_ERR_STATE, "rpim_get_pattern before rpim_build_pattern");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    int rc;
+    if ((rc = rpim_stage_emit_pattern(ctx, d_row_ptr, d_col_idx))) return rc;
+    if (d_support)
+        CUDA_TRY(ctx, cudaMemcpyAsync(d_support, ctx->d_support, (size_t)ctx->Nq * ctx->k * sizeof(int32_t),
+                                      cudaMemcpyDeviceToDevice, ctx->stream));
+    return RPIM_OK;
+}
+
+int rpim_assemble(rpim_ctx* ctx, const double* d_qw, double E, double nu, double alpha_c, double d_c, double q,
+                  const double body[3], double* d_vals, double* d_f, int64_t* out_singular) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    if (!ctx->have_pattern) RPIM_FAIL(ctx, RPIM_ERR_STATE, "rpim_assemble before rpim_build_pattern");
+    if (!d_qw || !body || !d_vals || !d_f) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "null pointer");
+    if (!(d_c > 0.0) || !(alpha_c > 0.0) || !std::isfinite(q) || !std::isfinite(E) || !(nu > -1.0 && nu < 0.5))
+        RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "need d_c > 0, alpha_c > 0, finite q and E, -1 < nu < 0.5");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    fill_shape_params(alpha_c, d_c, q, ctx->sp);
+    ctx->have_sp = true;
+    int rc;
+    if (!ctx->d_stage) {
+        if ((rc = ws_alloc(ctx, &ctx->d_stage, ctx->Nq * 4 * (int64_t)ctx->k))) return rc;
+        if ((rc = ws_alloc(ctx, &ctx->d_singular, ctx->Nq))) return rc;
+    }
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_SINGULAR, 0, sizeof(long long), st));
+    // a triple of pooled events per call so that a caller can sum kernel times over many calls
+    cudaEvent_t pe[3] = {nullptr, nullptr, nullptr};
+    if (ctx->phase_events_used + 3 <= 3 * 4096) {
+        while (ctx->phase_events.size() < ctx->phase_events_used + 3) {
+            cudaEvent_t e;
+            CUDA_TRY(ctx, cudaEventCreate(&e));
+            ctx->phase_events.push_back(e);
+        }
+        for (int i = 0; i < 3; ++i) pe[i] = ctx->phase_events[ctx->phase_events_used + i];
+        ctx->phase_events_used += 3;
+    }
+    cudaEventRecord(ctx->ev[4], st);
+    if (pe[0]) cudaEventRecord(pe[0], st);
+    if ((rc = rpim_stage_shape(ctx, ctx->d_qpts, ctx->d_support, ctx->Nq, ctx->d_stage, ctx->d_singular))) return rc;
+    cudaEventRecord(ctx->ev[5], st);
+    if (pe[1]) cudaEventRecord(pe[1], st);
+    const double lambda = E * nu / ((1.0 + nu) * (1.0 - 2.0 * nu));
+    const double mu = E / (2.0 * (1.0 + nu));
+    if ((rc = rpim_stage_accumulate(ctx, d_qw, lambda, mu, body, d_vals, d_f))) return rc;
+    cudaEventRecord(ctx->ev[6], st);
+    if (pe[2]) cudaEventRecord(pe[2], st);
+    ctx->phase_calls[1]++;
+    ctx->have_shape = true;
+    if (out_singular) {
+        long long ns = 0;
+        CUDA_TRY(ctx, cudaMemcpyAsync(&ns, ctx->d_flags + FLAG_SINGULAR, sizeof(ns), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(ctx, cudaStreamSynchronize(st));
+        *out_singular = ns;
+    }
+    return RPIM_OK;
+}
+
+int rpim_add_point_loads(rpim_ctx* ctx, const double* d_pts, const double* d_w, const double* d_t, int64_t M,
+                         double* d_f) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    if (!ctx->have_pattern || !ctx->have_sp) RPIM_FAIL(ctx, RPIM_ERR_STATE, "rpim_add_point_loads before rpim_assemble");
+    if (M < 0 || (M > 0 && (!d_pts || !d_w || !d_t || !d_f))) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "null pointer");
+    if (M == 0) return RPIM_OK;
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    int32_t* d_sup = nullptr;
+    double* d_stage = nullptr;
+    uint8_t* d_sing = nullptr;
+    int rc = RPIM_OK;
+    if ((rc = ws_alloc(ctx, &d_sup, M * ctx->k)) == RPIM_OK && (rc = ws_alloc(ctx, &d_stage, M * 4 * (int64_t)ctx->k)) == RPIM_OK &&
+        (rc = ws_alloc(ctx, &d_sing, M)) == RPIM_OK) {
+        if ((rc = rpim_stage_grid_knn(ctx, d_pts, M, ctx->k, d_sup, false)) == RPIM_OK &&
+            (rc = rpim_stage_shape(ctx, d_pts, d_sup, M, d_stage, d_sing)) == RPIM_OK)
+            rc = rpim_stage_point_loads(ctx, d_sup, d_stage, d_w, d_t, M, d_f);
+    }
+    cudaError_t e = cudaStreamSynchronize(st);
+    long long capf = 0;
+    cudaMemcpy(&capf, ctx->d_flags + FLAG_KNN_CAP, sizeof(capf), cudaMemcpyDeviceToHost);
+    ws_free(ctx, &d_sup);
+    ws_free(ctx, &d_stage);
+    ws_free(ctx, &d_sing);
+    if (rc) return rc;
+    if (e != cudaSuccess) RPIM_FAIL(ctx, RPIM_ERR_CUDA, "point loads failed: %s", cudaGetErrorString(e));
+    if (capf) RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "kNN capacity exceeded for %lld load points", capf);
+    return RPIM_OK;
+}
+
+int rpim_apply_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* d_bc_mask, const double* d_u_bar,
+                       int64_t m, double alpha, int alpha_is_relative, double* d_vals, double* d_f,
+                       double* out_alpha_used) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    if (!ctx->have_pattern) RPIM_FAIL(ctx, RPIM_ERR_STATE, "rpim_apply_penalty before rpim_build_pattern");
+    if (m < 0 || !d_vals || !d_f || (m > 0 && (!d_bc_nodes || !d_u_bar))) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "null pointer");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    return rpim_stage_penalty(ctx, d_bc_nodes, d_bc_mask, d_u_bar, m, alpha, alpha_is_relative, d_vals, d_f,
+                              out_alpha_used);
+}
+
+namespace {
+__global__ void split_stage_kernel(const double* __restrict__ stage, int64_t M, int k, double* __restrict__ phi,
+                                   double* __restrict__ dphi) {
+    const int64_t total = M * 4 * (int64_t)k;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t q = e / (4 * k);
+        const int r = (int)(e % (4 * k));
+        if (r < k) { if (phi) phi[q * k + r] = stage[e]; }
+        else if (dphi) dphi[q * 3 * (int64_t)k + (r - k)] = stage[e];
+    }
+}
+}  // namespace
+
+int rpim_get_shape(rpim_ctx* ctx, double* d_phi, double* d_dphi, uint8_t* d_singular) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    if (!ctx->have_shape) RPIM_FAIL(ctx, RPIM_ERR_STATE, "rpim_get_shape before rpim_assemble");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    if (d_phi || d_dphi) {
+        const int64_t total = ctx->Nq * 4 * (int64_t)ctx->k;
+        split_stage_kernel<<<(unsigned)std::min<int64_t>((total + 255) / 256, 148 * 32), 256, 0, ctx->stream>>>(
+            ctx->d_stage, ctx->Nq, ctx->k, d_phi, d_dphi);
+        KERNEL_CHECK(ctx);
+    }
+    if (d_singular)
+        CUDA_TRY(ctx, cudaMemcpyAsync(d_singular, ctx->d_singular, (size_t)ctx->Nq, cudaMemcpyDeviceToDevice, ctx->stream));
+    return RPIM_OK;
+}
+
+int rpim_last_phase_ms(rpim_ctx* ctx, float out_ms[5]) {
+    if (!ctx || !out_ms) return RPIM_ERR_INVALID_ARG;
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    if (ctx->have_shape) {
+        cudaEventElapsedTime(&ctx->phase_ms[3], ctx->ev[4], ctx->ev[5]);
+        cudaEventElapsedTime(&ctx->phase_ms[4], ctx->ev[5], ctx->ev[6]);
+    }
+    for (int i = 0; i < 5; ++i) out_ms[i] = ctx->phase_ms[i];
+    return RPIM_OK;
+}
+
+int rpim_phase_totals(rpim_ctx* ctx, double out_ms[5], int64_t out_calls[2], int reset) {
+    if (!ctx || !out_ms) return RPIM_ERR_INVALID_ARG;
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    double shape = 0.0, reduce = 0.0;
+    for (size_t i = 0; i + 2 < ctx->phase_events_used + 0 && i + 2 < ctx->phase_events.size() + 0; i += 3) {
+        float a = 0.f, b = 0.f;
+        if (cudaEventElapsedTime(&a, ctx->phase_events[i], ctx->phase_events[i + 1]) == cudaSuccess) shape += a;
+        if (cudaEventElapsedTime(&b, ctx->phase_events[i + 1], ctx->phase_events[i + 2]) == cudaSuccess) reduce += b;
+    }
+    cudaGetLastError();
+    for (int i = 0; i < 3; ++i) out_ms[i] = ctx->phase_total_ms[i];
+    out_ms[3] = shape;
+    out_ms[4] = reduce;
+    if (out_calls) { out_calls[0] = ctx->phase_calls[0]; out_calls[1] = ctx->phase_calls[1]; }
+    if (reset) {
+        ctx->phase_events_used = 0;
+        for (int i = 0; i < 5; ++i) ctx->phase_total_ms[i] = 0.0;
+        ctx->phase_calls[0] = ctx->phase_calls[1] = 0;
+    }
+    return RPIM_OK;
+}
+
+// ------------------------------------------------------------------ host-buffer (end-to-end) entry points
+int rpim_host_pattern(rpim_ctx* ctx, const double* h_nodes, int64_t N, const double* h_qpts, int64_t Nq, int k,
+                      int index_bits, int64_t* out_nnz, int* out_index_bits) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    if (!h_nodes || !h_qpts || N <= 0 || Nq <= 0) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "null pointer or empty input");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    int rc;
+    if ((rc = ws_alloc(ctx, &ctx->h2d_nodes, 3 * N))) return rc;
+    if ((rc = ws_alloc(ctx, &ctx->h2d_qpts, 3 * Nq))) return rc;
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h2d_nodes, h_nodes, (size_t)3 * N * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h2d_qpts, h_qpts, (size_t)3 * Nq * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    return rpim_build_pattern(ctx, ctx->h2d_nodes, N, ctx->h2d_qpts, Nq, k, index_bits, out_nnz, out_index_bits);
+}
+
+int rpim_host_assemble(rpim_ctx* ctx, const double* h_qw, double E, double nu, double alpha_c, double d_c, double q,
+                       const double body[3], const int64_t* h_bc_nodes, const uint8_t* h_bc_mask,
+                       const double* h_u_bar, int64_t m, double alpha, int alpha_is_relative, void* h_row_ptr,
+                       void* h_col_idx, double* h_vals, double* h_f, int64_t* out_singular, double* out_alpha_used) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    if (!ctx->have_pattern) RPIM_FAIL(ctx, RPIM_ERR_STATE, "rpim_host_assemble before rpim_host_pattern");
+    if (!h_qw || !h_vals || !h_f || m < 0 || (m > 0 && (!h_bc_nodes || !h_u_bar))) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "null pointer");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const int64_t nnz = 9 * ctx->nnzb, n3 = 3 * ctx->N;
+    const size_t iw = ctx->index_bits / 8;
+    double *d_qw = nullptr, *d_vals = nullptr, *d_f = nullptr, *d_ub = nullptr;
+    int64_t* d_bn = nullptr;
+    uint8_t* d_bm = nullptr;
+    void *d_rp = nullptr, *d_ci = nullptr;
+    int rc = RPIM_OK;
+    auto cleanup = [&]() {
+        cudaFree(d_qw); cudaFree(d_vals); cudaFree(d_f); cudaFree(d_ub); cudaFree(d_bn); cudaFree(d_bm); cudaFree(d_rp); cudaFree(d_ci);
+    };
+#define HOST_TRY(expr)                                                                           \
+    do {                                                                                         \
+        cudaError_t _e = (expr);                                                                 \
+        if (_e != cudaSuccess) {                                                                 \
+            cleanup();                                                                           \
+            RPIM_FAIL(ctx, (_e == cudaErrorMemoryAllocation ? RPIM_ERR_ALLOC : RPIM_ERR_CUDA),   \
+                      "%s failed: %s", #expr, cudaGetErrorString(_e));                           \
+        }                                                                                        \
+    } while (0)
+    HOST_TRY(cudaMalloc((void**)&d_qw, (size_t)ctx->Nq * sizeof(double)));
+    HOST_TRY(cudaMalloc((void**)&d_vals, (size_t)std::max<int64_t>(nnz, 1) * sizeof(double)));
+    HOST_TRY(cudaMalloc((void**)&d_f, (size_t)n3 * sizeof(double)));
+    HOST_TRY(cudaMemcpyAsync(d_qw, h_qw, (size_t)ctx->Nq * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (m > 0) {
+        HOST_TRY(cudaMalloc((void**)&d_bn, (size_t)m * sizeof(int64_t)));
+        HOST_TRY(cudaMalloc((void**)&d_ub, (size_t)3 * m * sizeof(double)));
+        HOST_TRY(cudaMemcpyAsync(d_bn, h_bc_nodes, (size_t)m * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+        HOST_TRY(cudaMemcpyAsync(d_ub, h_u_bar, (size_t)3 * m * sizeof(double), cudaMemcpyHostToDevice, st));
+        if (h_bc_mask) {
+            HOST_TRY(cudaMalloc((void**)&d_bm, (size_t)m));
+            HOST_TRY(cudaMemcpyAsync(d_bm, h_bc_mask, (size_t)m, cudaMemcpyHostToDevice, st));
+        }
+    }
+    if (h_row_ptr) HOST_TRY(cudaMalloc(&d_rp, (size_t)(n3 + 1) * iw));
+    if (h_col_idx) HOST_TRY(cudaMalloc(&d_ci, (size_t)std::max<int64_t>(nnz, 1) * iw));
+    if ((rc = rpim_get_pattern(ctx, d_rp, d_ci, nullptr))) { cleanup(); return rc; }
+    if (h_row_ptr) HOST_TRY(cudaMemcpyAsync(h_row_ptr, d_rp, (size_t)(n3 + 1) * iw, cudaMemcpyDeviceToHost, st));
+    if (h_col_idx) HOST_TRY(cudaMemcpyAsync(h_col_idx, d_ci, (size_t)nnz * iw, cudaMemcpyDeviceToHost, st));
+    if ((rc = rpim_assemble(ctx, d_qw, E, nu, alpha_c, d_c, q, body, d_vals, d_f, out_singular))) { cleanup(); return rc; }
+    if ((rc = rpim_apply_penalty(ctx, d_bn, d_bm, d_ub, m, alpha, alpha_is_relative, d_vals, d_f, out_alpha_used))) { cleanup(); return rc; }
+    HOST_TRY(cudaMemcpyAsync(h_vals, d_vals, (size_t)nnz * sizeof(double), cudaMemcpyDeviceToHost, st));
+    HOST_TRY(cudaMemcpyAsync(h_f, d_f, (size_t)n3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    HOST_TRY(cudaStreamSynchronize(st));
+#undef HOST_TRY
+    cleanup();
+    return RPIM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,230 @@
+// Internal declarations of librpim (sm_100a).  Not part of the C ABI (include/rpim.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <cstdio>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+#include "../../include/rpim.h"
+
+#define RPIM_WARP 32
+
+// device-side error / counter slots (ctx->d_flags, int64 each)
+enum { FLAG_KNN_CAP = 0, FLAG_PAT_CAP = 1, FLAG_BC_BAD = 2, FLAG_SINGULAR = 3, FLAG_INC_CAP = 4, NUM_FLAGS = 8 };
+
+struct GridParams {
+    double lo[3];
+    double cell;      // cell edge
+    double inv_cell;  // 1.0 / cell
+    int nc[3];
+    int64_t ncell;
+};
+
+// Reproducible power t^(q-1): tables and coefficients (R5), filled on the host.
+struct PowTables {
+    double b[10];
+    double invc[32];
+    double E[32];
+    double F[128];
+};
+
+struct ShapeParams {
+    double inv_dc, ac2, twoq;
+    PowTables pw;
+};
+
+struct rpim_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    int64_t launches = 0;
+    int64_t ws_bytes = 0;
+    std::unordered_map<void*, int64_t> ws_sizes;
+
+    // problem
+    const double* d_nodes = nullptr;
+    const double* d_qpts = nullptr;
+    int64_t N = 0, Nq = 0;
+    int k = 0;
+    bool have_pattern = false, have_shape = false;
+    int index_bits = 64;
+    int64_t nnzb = 0;   // number of 3x3 blocks
+    int max_blen = 0;   // longest block row
+    int max_inc = 0;    // longest incidence list
+
+    // cell grid
+    GridParams grid{};
+    int* d_cell_of = nullptr;        // N
+    int64_t* d_cell_start = nullptr; // ncell + 1
+    int* d_cell_cursor = nullptr;    // ncell
+    int* d_node_order = nullptr;     // N   (node ids in cell order)
+    double* d_sorted_xyz = nullptr;  // 3 x N (SoA, cell order)
+
+    // supports and incidence
+    int32_t* d_support = nullptr;    // Nq x k
+    int* d_inc_count = nullptr;      // N
+    int64_t* d_inc_ptr = nullptr;    // N + 1
+    int32_t* d_inc_q = nullptr;      // Nq*k  (point id, ascending per node)
+    uint8_t* d_inc_j = nullptr;      // Nq*k  (position of the node in that point's support)
+
+    // block pattern
+    int* d_blen = nullptr;           // N
+    int64_t* d_brow_ptr = nullptr;   // N + 1
+    int32_t* d_bcol = nullptr;       // nnzb
+    int* d_bdiag = nullptr;          // N (slot of the diagonal block in its row)
+
+    // staged shape functions: Nq x 4 x k  (phi, dphi/dx, dphi/dy, dphi/dz)
+    double* d_stage = nullptr;
+    uint8_t* d_singular = nullptr;   // Nq
+    ShapeParams sp{};
+    bool have_sp = false;
+
+    // misc
+    long long* d_flags = nullptr;    // NUM_FLAGS
+    double* d_scratch = nullptr;     // small reductions (>= 4096 doubles)
+    void* d_scan_tmp = nullptr;      // scan block sums
+    int64_t scan_tmp_elems = 0;
+
+    cudaEvent_t ev[8] = {};
+    float phase_ms[5] = {0, 0, 0, 0, 0};
+    // per-call event triples (begin shape, end shape = begin reduce, end reduce) since the last reset
+    std::vector<cudaEvent_t> phase_events;
+    size_t phase_events_used = 0;
+    double phase_total_ms[5] = {0, 0, 0, 0, 0};   // accumulated pattern-stage times (measured at sync points)
+    int64_t phase_calls[2] = {0, 0};              // build_pattern calls, assemble calls since reset
+
+    // device buffers of the host-buffer entry points
+    double *h2d_nodes = nullptr, *h2d_qpts = nullptr;
+};
+
+#define RPIM_FAIL(ctx, code, ...)                          \
+    do {                                                   \
+        char _b[512];                                      \
+        snprintf(_b, sizeof(_b), __VA_ARGS__);             \
+        (ctx)->err = _b;                                   \
+        return (code);                                     \
+    } while (0)
+
+#define CUDA_TRY(ctx, expr)                                                                     \
+    do {                                                                                        \
+        cudaError_t _e = (expr);                                                                \
+        if (_e != cudaSuccess)                                                                  \
+            RPIM_FAIL(ctx, (_e == cudaErrorMemoryAllocation ? RPIM_ERR_ALLOC : RPIM_ERR_CUDA),  \
+                      "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+    } while (0)
+
+#define KERNEL_CHECK(ctx)                                                                       \
+    do {                                                                                        \
+        (ctx)->launches++;                                                                      \
+        cudaError_t _e = cudaGetLastError();                                                    \
+        if (_e != cudaSuccess)                                                                  \
+            RPIM_FAIL(ctx, RPIM_ERR_CUDA, "kernel launch failed: %s (%s:%d)",                   \
+                      cudaGetErrorString(_e), __FILE__, __LINE__);                              \
+    } while (0)
+
+template <typename T>
+void ws_free(rpim_ctx* ctx, T** p) {
+    if (*p) {
+        auto it = ctx->ws_sizes.find((void*)*p);
+        if (it != ctx->ws_sizes.end()) { ctx->ws_bytes -= it->second; ctx->ws_sizes.erase(it); }
+        cudaFree(*p);
+    }
+    *p = nullptr;
+}
+template <typename T>
+int ws_alloc(rpim_ctx* ctx, T** p, int64_t count) {
+    ws_free(ctx, p);
+    if (count <= 0) count = 1;
+    cudaError_t e = cudaMalloc((void**)p, (size_t)count * sizeof(T));
+    if (e != cudaSuccess) {
+        *p = nullptr;
+        cudaGetLastError();
+        RPIM_FAIL(ctx, RPIM_ERR_ALLOC, "device allocation of %lld bytes failed: %s",
+                  (long long)(count * (int64_t)sizeof(T)), cudaGetErrorString(e));
+    }
+    ctx->ws_sizes[(void*)*p] = count * (int64_t)sizeof(T);
+    ctx->ws_bytes += count * (int64_t)sizeof(T);
+    return RPIM_OK;
+}
+
+// ---- stages implemented in the other translation units
+int rpim_scan_i32_to_i64(rpim_ctx* ctx, const int* d_in, int64_t* d_out, int64_t n);  // exclusive, writes n+1
+int rpim_stage_grid_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, int32_t* d_support, bool build_grid);
+int rpim_stage_incidence(rpim_ctx* ctx);
+int rpim_stage_block_pattern(rpim_ctx* ctx);
+int rpim_stage_emit_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx);
+int rpim_stage_shape(rpim_ctx* ctx, const double* d_pts, const int32_t* d_support, int64_t M, double* d_stage,
+                     uint8_t* d_singular);
+int rpim_stage_accumulate(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
+                          double* d_vals, double* d_f);
+int rpim_stage_point_loads(rpim_ctx* ctx, const int32_t* d_support, const double* d_stage, const double* d_w,
+                           const double* d_t, int64_t M, double* d_f);
+int rpim_stage_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* d_bc_mask, const double* d_u_bar,
+                       int64_t m, double alpha, int relative, double* d_vals, double* d_f, double* out_alpha);
+
+// ---- small device helpers
+__device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
+
+// In-place ascending bitonic sort of n (power of two) 64-bit keys in shared memory by one warp.
+__device__ __forceinline__ void warp_bitonic_u64(unsigned long long* key, int n) {
+    const int lane = lane_id();
+    for (int size = 2; size <= n; size <<= 1) {
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            __syncwarp();
+            for (int t = lane; t < (n >> 1); t += 32) {
+                int lo = 2 * t - (t & (stride - 1));
+                int hi = lo + stride;
+                bool up = ((lo & size) == 0);
+                unsigned long long a = key[lo], b = key[hi];
+                if ((a > b) == up) { key[lo] = b; key[hi] = a; }
+            }
+        }
+    }
+    __syncwarp();
+}
+
+// Same for (key, value) pairs ordered by (key, value).
+__device__ __forceinline__ void warp_bitonic_u64_i32(unsigned long long* key, int* val, int n) {
+    const int lane = lane_id();
+    for (int size = 2; size <= n; size <<= 1) {
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            __syncwarp();
+            for (int t = lane; t < (n >> 1); t += 32) {
+                int lo = 2 * t - (t & (stride - 1));
+                int hi = lo + stride;
+                bool up = ((lo & size) == 0);
+                unsigned long long a = key[lo], b = key[hi];
+                int va = val[lo], vb = val[hi];
+                bool gt = (a > b) || (a == b && va > vb);
+                if (gt == up) { key[lo] = b; key[hi] = a; val[lo] = vb; val[hi] = va; }
+            }
+        }
+    }
+    __syncwarp();
+}
+
+__device__ __forceinline__ void warp_bitonic_i32(int* key, int n) {
+    const int lane = lane_id();
+    for (int size = 2; size <= n; size <<= 1) {
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            __syncwarp();
+            for (int t = lane; t < (n >> 1); t += 32) {
+                int lo = 2 * t - (t & (stride - 1));
+                int hi = lo + stride;
+                bool up = ((lo & size) == 0);
+                int a = key[lo], b = key[hi];
+                if ((a > b) == up) { key[lo] = b; key[hi] = a; }
+            }
+        }
+    }
+    __syncwarp();
+}
+
+__host__ __device__ __forceinline__ int next_pow2(int v) {
+    int p = 1;
+    while (p < v) p <<= 1;
+    return p;
+}

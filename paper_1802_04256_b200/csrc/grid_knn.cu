@@ -1,0 +1,379 @@
+// Step a1 (R1): exact k-nearest-neighbour support search on a uniform cell grid.
+// Integer / exact-order work: the result is unique (keys (d2, node id) are distinct), so the
+// cell size, scan order and thread mapping below are free implementation choices.
+#include <cfloat>
+#include <cmath>
+
+#include "common.cuh"
+
+// ------------------------------------------------------------------ exclusive scan int32 -> int64
+namespace {
+constexpr int SCAN_THREADS = 1024;
+constexpr int SCAN_ITEMS = 4;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+
+__global__ void scan_tile_kernel(const int* __restrict__ in, int64_t* __restrict__ out, int64_t n,
+                                 int64_t* __restrict__ tile_sum) {
+    __shared__ int64_t warp_tot[32];
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    int64_t v[SCAN_ITEMS];
+    int64_t s = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) {
+        int64_t x = (base + i < n) ? (int64_t)in[base + i] : 0;
+        v[i] = s;
+        s += x;
+    }
+    // warp inclusive scan of s
+    int64_t inc = s;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int64_t t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    if (lane == 31) warp_tot[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        int64_t w = warp_tot[lane];
+        int64_t winc = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            int64_t t = __shfl_up_sync(0xffffffffu, winc, d);
+            if (lane >= d) winc += t;
+        }
+        warp_tot[lane] = winc - w;   // exclusive
+        if (lane == 31) tile_sum[blockIdx.x] = winc;
+    }
+    __syncthreads();
+    const int64_t off = warp_tot[wid] + (inc - s);
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i)
+        if (base + i < n) out[base + i] = off + v[i];
+}
+
+__global__ void scan_sums_kernel(int64_t* tile_sum, int64_t ntiles) {
+    // single block, sequential over chunks of blockDim.x with a running carry
+    __shared__ int64_t buf[1024];
+    __shared__ int64_t carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int64_t c0 = 0; c0 < ntiles; c0 += blockDim.x) {
+        int64_t i = c0 + threadIdx.x;
+        int64_t x = (i < ntiles) ? tile_sum[i] : 0;
+        buf[threadIdx.x] = x;
+        __syncthreads();
+        for (int d = 1; d < (int)blockDim.x; d <<= 1) {
+            int64_t t = (threadIdx.x >= (unsigned)d) ? buf[threadIdx.x - d] : 0;
+            __syncthreads();
+            buf[threadIdx.x] += t;
+            __syncthreads();
+        }
+        if (i < ntiles) tile_sum[i] = carry + buf[threadIdx.x] - x;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry += buf[threadIdx.x];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) tile_sum[ntiles] = carry;   // grand total
+}
+
+__global__ void scan_add_kernel(int64_t* __restrict__ out, int64_t n, const int64_t* __restrict__ tile_sum,
+                                int64_t ntiles) {
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    const int64_t add = tile_sum[blockIdx.x];
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i)
+        if (base + i < n) out[base + i] += add;
+    if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = tile_sum[ntiles];
+}
+}  // namespace
+
+int rpim_scan_i32_to_i64(rpim_ctx* ctx, const int* d_in, int64_t* d_out, int64_t n) {
+    const int64_t ntiles = (n + SCAN_TILE - 1) / SCAN_TILE;
+    if (ctx->scan_tmp_elems < ntiles + 1) {
+        int64_t* p = (int64_t*)ctx->d_scan_tmp;
+        int rc = ws_alloc(ctx, &p, ntiles + 1);
+        ctx->d_scan_tmp = p;
+        if (rc) return rc;
+        ctx->scan_tmp_elems = ntiles + 1;
+    }
+    int64_t* tmp = (int64_t*)ctx->d_scan_tmp;
+    if (n == 0) {
+        CUDA_TRY(ctx, cudaMemsetAsync(d_out, 0, sizeof(int64_t), ctx->stream));
+        return RPIM_OK;
+    }
+    scan_tile_kernel<<<(unsigned)ntiles, SCAN_THREADS, 0, ctx->stream>>>(d_in, d_out, n, tmp);
+    KERNEL_CHECK(ctx);
+    scan_sums_kernel<<<1, 1024, 0, ctx->stream>>>(tmp, ntiles);
+    KERNEL_CHECK(ctx);
+    scan_add_kernel<<<(unsigned)ntiles, SCAN_THREADS, 0, ctx->stream>>>(d_out, n, tmp, ntiles);
+    KERNEL_CHECK(ctx);
+    return RPIM_OK;
+}
+
+// ------------------------------------------------------------------ bounding box + cell binning
+namespace {
+__global__ void bbox_partial_kernel(const double* __restrict__ nodes, int64_t N, double* __restrict__ part) {
+    double lo[3] = {DBL_MAX, DBL_MAX, DBL_MAX}, hi[3] = {-DBL_MAX, -DBL_MAX, -DBL_MAX};
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double v = nodes[3 * i + c];
+            lo[c] = fmin(lo[c], v);
+            hi[c] = fmax(hi[c], v);
+        }
+    __shared__ double s[6][256];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { s[c][threadIdx.x] = lo[c]; s[3 + c][threadIdx.x] = hi[c]; }
+    __syncthreads();
+    for (int d = blockDim.x >> 1; d > 0; d >>= 1) {
+        if ((int)threadIdx.x < d)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                s[c][threadIdx.x] = fmin(s[c][threadIdx.x], s[c][threadIdx.x + d]);
+                s[3 + c][threadIdx.x] = fmax(s[3 + c][threadIdx.x], s[3 + c][threadIdx.x + d]);
+            }
+        __syncthreads();
+    }
+    if (threadIdx.x < 6) part[blockIdx.x * 6 + threadIdx.x] = s[threadIdx.x][0];
+}
+
+__global__ void bbox_final_kernel(double* part, int nparts) {
+    // one warp; result in part[0..5]
+    const int lane = threadIdx.x;
+    double lo[3] = {DBL_MAX, DBL_MAX, DBL_MAX}, hi[3] = {-DBL_MAX, -DBL_MAX, -DBL_MAX};
+    for (int b = lane; b < nparts; b += 32)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            lo[c] = fmin(lo[c], part[b * 6 + c]);
+            hi[c] = fmax(hi[c], part[b * 6 + 3 + c]);
+        }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            lo[c] = fmin(lo[c], __shfl_xor_sync(0xffffffffu, lo[c], d));
+            hi[c] = fmax(hi[c], __shfl_xor_sync(0xffffffffu, hi[c], d));
+        }
+    __syncwarp();
+    if (lane == 0)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { part[c] = lo[c]; part[3 + c] = hi[c]; }
+}
+
+__device__ __forceinline__ void cell_coords(const GridParams& g, double x, double y, double z, int* c) {
+    double p[3] = {x, y, z};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        int v = (int)floor((p[a] - g.lo[a]) * g.inv_cell);
+        c[a] = min(max(v, 0), g.nc[a] - 1);
+    }
+}
+
+__global__ void cell_count_kernel(GridParams g, const double* __restrict__ nodes, int64_t N,
+                                  int* __restrict__ cell_of, int* __restrict__ count) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int c[3];
+    cell_coords(g, nodes[3 * i], nodes[3 * i + 1], nodes[3 * i + 2], c);
+    int id = c[0] + g.nc[0] * (c[1] + g.nc[1] * c[2]);
+    cell_of[i] = id;
+    atomicAdd(&count[id], 1);
+}
+
+__global__ void cell_fill_kernel(const double* __restrict__ nodes, int64_t N, const int* __restrict__ cell_of,
+                                 const int64_t* __restrict__ cell_start, int* __restrict__ cursor,
+                                 int* __restrict__ node_order) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int id = cell_of[i];
+    int p = atomicAdd(&cursor[id], 1);
+    node_order[cell_start[id] + p] = (int)i;
+}
+
+// make the order inside every cell deterministic (ascending node id) and gather coordinates
+__global__ void cell_sort_gather_kernel(const double* __restrict__ nodes, int64_t ncell,
+                                        const int64_t* __restrict__ cell_start, int* __restrict__ node_order,
+                                        double* __restrict__ sx, double* __restrict__ sy, double* __restrict__ sz) {
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncell) return;
+    int64_t a = cell_start[c], b = cell_start[c + 1];
+    for (int64_t i = a + 1; i < b; ++i) {   // insertion sort, cells hold a handful of nodes
+        int v = node_order[i];
+        int64_t j = i - 1;
+        while (j >= a && node_order[j] > v) { node_order[j + 1] = node_order[j]; --j; }
+        node_order[j + 1] = v;
+    }
+    for (int64_t i = a; i < b; ++i) {
+        int64_t id = node_order[i];
+        sx[i] = nodes[3 * id];
+        sy[i] = nodes[3 * id + 1];
+        sz[i] = nodes[3 * id + 2];
+    }
+}
+
+// ------------------------------------------------------------------ the search: one warp per query point
+constexpr int KNN_CAP = 2048;          // candidates held on chip per query
+constexpr int KNN_WARPS = 4;
+
+__global__ void __launch_bounds__(KNN_WARPS * 32)
+knn_kernel(GridParams g, const double* __restrict__ sx, const double* __restrict__ sy,
+           const double* __restrict__ sz, const int* __restrict__ node_order,
+           const int64_t* __restrict__ cell_start, const double* __restrict__ pts, int64_t M, int k, int R0,
+           int32_t* __restrict__ support, long long* __restrict__ flags) {
+    extern __shared__ unsigned char smem_raw[];
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned long long* key = (unsigned long long*)smem_raw + (size_t)wid * KNN_CAP;
+    int* val = (int*)((unsigned long long*)smem_raw + (size_t)KNN_WARPS * KNN_CAP) + (size_t)wid * KNN_CAP;
+
+    for (int64_t q = (int64_t)blockIdx.x * KNN_WARPS + wid; q < M; q += (int64_t)gridDim.x * KNN_WARPS) {
+        const double xq = pts[3 * q], yq = pts[3 * q + 1], zq = pts[3 * q + 2];
+        int cq[3];
+        cell_coords(g, xq, yq, zq, cq);
+        int R = R0;
+        int npad = 0;
+        bool fail = false;
+        while (true) {
+            int a[3], b[3];
+            bool whole = true;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                a[c] = max(cq[c] - R, 0);
+                b[c] = min(cq[c] + R, g.nc[c] - 1);
+                if (a[c] > 0 || b[c] < g.nc[c] - 1) whole = false;
+            }
+            const int ny = b[1] - a[1] + 1, nz = b[2] - a[2] + 1;
+            const int nrows = ny * nz;
+            // count candidates (cells of one x-row are contiguous in cell order)
+            int cnt = 0;
+            for (int r = lane; r < nrows; r += 32) {
+                int y = a[1] + r % ny, z = a[2] + r / ny;
+                int64_t c0 = a[0] + (int64_t)g.nc[0] * (y + (int64_t)g.nc[1] * z);
+                int64_t c1 = c0 + (b[0] - a[0]);
+                cnt += (int)(cell_start[c1 + 1] - cell_start[c0]);
+            }
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, d);
+            if (cnt < k) {
+                if (whole) { fail = true; break; }
+                ++R;
+                continue;
+            }
+            if (cnt > KNN_CAP) { fail = true; break; }
+            // gather candidates with their squared distances (R1: no fma, fixed association)
+            int base = 0;
+            for (int r = 0; r < nrows; ++r) {
+                int y = a[1] + r % ny, z = a[2] + r / ny;
+                int64_t c0 = a[0] + (int64_t)g.nc[0] * (y + (int64_t)g.nc[1] * z);
+                int64_t s0 = cell_start[c0], s1 = cell_start[c0 + (b[0] - a[0]) + 1];
+                for (int64_t p = s0 + lane; p < s1; p += 32) {
+                    double dx = __dsub_rn(sx[p], xq), dy = __dsub_rn(sy[p], yq), dz = __dsub_rn(sz[p], zq);
+                    double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+                    key[base + (int)(p - s0)] = (unsigned long long)__double_as_longlong(d2);
+                    val[base + (int)(p - s0)] = node_order[p];
+                }
+                base += (int)(s1 - s0);
+            }
+            npad = next_pow2(cnt);
+            for (int i = cnt + lane; i < npad; i += 32) { key[i] = 0xFFFFFFFFFFFFFFFFull; val[i] = 0x7FFFFFFF; }
+            __syncwarp();
+            warp_bitonic_u64_i32(key, val, npad);
+            if (whole) break;
+            // distance from the query to the part of space not covered by the scanned cells
+            double bound = DBL_MAX;
+            const double xyz[3] = {xq, yq, zq};
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                if (a[c] > 0) bound = fmin(bound, xyz[c] - (g.lo[c] + a[c] * g.cell));
+                if (b[c] < g.nc[c] - 1) bound = fmin(bound, (g.lo[c] + (b[c] + 1) * g.cell) - xyz[c]);
+            }
+            bound -= 1e-9 * g.cell;   // margin for rounding in the cell assignment
+            double dk = __longlong_as_double((long long)key[k - 1]);
+            if (bound > 0.0 && dk < bound * bound) break;
+            ++R;
+        }
+        if (fail) {
+            if (lane == 0) atomicAdd((unsigned long long*)&flags[FLAG_KNN_CAP], 1ull);
+            for (int j = lane; j < k; j += 32) support[q * k + j] = 0;
+            __syncwarp();
+            continue;
+        }
+        // the k winners, ascending by node id
+        const int kp = next_pow2(k);
+        for (int j = k + lane; j < kp; j += 32) val[j] = 0x7FFFFFFF;
+        __syncwarp();
+        warp_bitonic_i32(val, kp);
+        for (int j = lane; j < k; j += 32) support[q * k + j] = val[j];
+        __syncwarp();
+    }
+}
+}  // namespace
+
+int rpim_stage_grid_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, int32_t* d_support, bool build_grid) {
+    cudaStream_t st = ctx->stream;
+    const int64_t N = ctx->N;
+    if (build_grid) {
+        int rc;
+        if ((rc = ws_alloc(ctx, &ctx->d_scratch, 8192))) return rc;
+        bbox_partial_kernel<<<256, 256, 0, st>>>(ctx->d_nodes, N, ctx->d_scratch);
+        KERNEL_CHECK(ctx);
+        bbox_final_kernel<<<1, 32, 0, st>>>(ctx->d_scratch, 256);
+        KERNEL_CHECK(ctx);
+        double bb[6];
+        CUDA_TRY(ctx, cudaMemcpyAsync(bb, ctx->d_scratch, sizeof(bb), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(ctx, cudaStreamSynchronize(st));
+        for (int c = 0; c < 6; ++c)
+            if (!std::isfinite(bb[c])) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "node coordinates are not finite");
+        double ext[3], emax = 0.0;
+        for (int c = 0; c < 3; ++c) { ext[c] = bb[3 + c] - bb[c]; emax = std::fmax(emax, ext[c]); }
+        if (!(emax > 0.0)) emax = 1.0;
+        double vol = 1.0;
+        for (int c = 0; c < 3; ++c) vol *= std::fmax(ext[c], 1e-9 * emax);
+        const double h_avg = std::cbrt(vol / (double)N);
+        const double r_k = std::cbrt(3.0 * k / (4.0 * 3.14159265358979323846)) * h_avg;
+        GridParams g;
+        g.cell = 1.08 * r_k / 2.0;   // two rings of cells cover the expected support radius
+        int64_t ncell;
+        while (true) {
+            ncell = 1;
+            for (int c = 0; c < 3; ++c) {
+                g.nc[c] = (int)std::fmin(2000.0, std::floor(ext[c] / g.cell) + 1.0);
+                ncell *= g.nc[c];
+            }
+            if (ncell <= 4 * N + 64) break;
+            g.cell *= 1.26;
+        }
+        g.inv_cell = 1.0 / g.cell;
+        for (int c = 0; c < 3; ++c) g.lo[c] = bb[c];
+        g.ncell = ncell;
+        ctx->grid = g;
+        if ((rc = ws_alloc(ctx, &ctx->d_cell_of, N))) return rc;
+        if ((rc = ws_alloc(ctx, &ctx->d_cell_start, ncell + 1))) return rc;
+        if ((rc = ws_alloc(ctx, &ctx->d_cell_cursor, ncell))) return rc;
+        if ((rc = ws_alloc(ctx, &ctx->d_node_order, N))) return rc;
+        if ((rc = ws_alloc(ctx, &ctx->d_sorted_xyz, 3 * N))) return rc;
+        CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_cell_cursor, 0, ncell * sizeof(int), st));
+        const unsigned nb = (unsigned)((N + 255) / 256);
+        cell_count_kernel<<<nb, 256, 0, st>>>(g, ctx->d_nodes, N, ctx->d_cell_of, ctx->d_cell_cursor);
+        KERNEL_CHECK(ctx);
+        if ((rc = rpim_scan_i32_to_i64(ctx, ctx->d_cell_cursor, ctx->d_cell_start, ncell))) return rc;
+        CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_cell_cursor, 0, ncell * sizeof(int), st));
+        cell_fill_kernel<<<nb, 256, 0, st>>>(ctx->d_nodes, N, ctx->d_cell_of, ctx->d_cell_start, ctx->d_cell_cursor,
+                                             ctx->d_node_order);
+        KERNEL_CHECK(ctx);
+        cell_sort_gather_kernel<<<(unsigned)((ncell + 127) / 128), 128, 0, st>>>(
+            ctx->d_nodes, ncell, ctx->d_cell_start, ctx->d_node_order, ctx->d_sorted_xyz, ctx->d_sorted_xyz + N,
+            ctx->d_sorted_xyz + 2 * N);
+        KERNEL_CHECK(ctx);
+    }
+    if (M == 0) return RPIM_OK;
+    const size_t smem = (size_t)KNN_WARPS * KNN_CAP * (sizeof(unsigned long long) + sizeof(int));
+    CUDA_TRY(ctx, cudaFuncSetAttribute(knn_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int64_t blocks = (M + KNN_WARPS - 1) / KNN_WARPS;
+    if (blocks > 148 * 64) blocks = 148 * 64;
+    knn_kernel<<<(unsigned)blocks, KNN_WARPS * 32, smem, st>>>(
+        ctx->grid, ctx->d_sorted_xyz, ctx->d_sorted_xyz + N, ctx->d_sorted_xyz + 2 * N, ctx->d_node_order,
+        ctx->d_cell_start, d_pts, M, k, 2, d_support, ctx->d_flags);
+    KERNEL_CHECK(ctx);
+    return RPIM_OK;
+}

@@ -1,0 +1,149 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI binding) against the CPU oracle on the same
+seeded inputs.  Bars (BASELINE.json north_star): supports and CSR pattern bit-exact; K and f within
+1e-10 relative, per entry, scaled by max|K_ii| (of the matrix compared).  Shape functions are
+compared BITWISE: DESIGN.md section 2 specifies the per-point stage at the operation level."""
+import numpy as np
+import pytest
+
+import workloads
+from gpu_harness import kmax_diag, run_cuda, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+def _compare(w, g, o, check_penalty=True):
+    assert np.array_equal(g["support"], o["support"])                     # a1 bit-exact
+    assert g["row_ptr"].dtype == (np.int32 if g["bits"] == 32 else np.int64)
+    assert np.array_equal(g["row_ptr"].astype(np.int64), o["row_ptr"])    # a2 bit-exact
+    assert np.array_equal(g["col_idx"].astype(np.int64), o["col_idx"])
+    assert g["nsing"] == o["nsing"]
+    assert np.array_equal(g["singular"], o["singular"])
+    assert np.array_equal(g["phi"], o["phi"])                             # a3+a4 bitwise
+    assert np.array_equal(g["dphi"], o["dphi"])
+    km = kmax_diag(o)
+    assert np.abs(g["vals0"] - o["vals0"]).max() <= TOL * km              # a5+a6
+    fs = max(np.abs(o["f_loaded"]).max(), 1e-300)
+    assert np.abs(g["f0"] - o["f0"]).max() <= TOL * max(np.abs(o["f0"]).max(), 1e-300)
+    assert np.abs(g["f_loaded"] - o["f_loaded"]).max() <= TOL * fs        # a5b
+    if check_penalty:                                                      # a7
+        assert abs(g["alpha"] - o["alpha"]) <= 1e-13 * o["alpha"]
+        km_pen = max(km, np.abs(o["vals"]).max())
+        assert np.abs(g["vals"] - o["vals"]).max() <= TOL * km_pen
+        changed = g["vals"] != g["vals0"]
+        ochanged = o["vals"] != o["vals0"]
+        assert np.array_equal(changed, ochanged)                           # exactly the constrained diagonals
+        assert np.allclose(g["vals"][changed] - g["vals0"][changed], g["alpha"], rtol=1e-12, atol=0)
+        assert np.abs(g["f"] - o["f"]).max() <= TOL * max(np.abs(o["f"]).max(), 1e-300)
+
+
+def test_config1_patch_full_parity():
+    w = workloads.config("patch")
+    _compare(w, run_cuda(w), run_oracle(w))
+
+
+def test_config2_cantilever_full_parity_with_traction_and_penalty():
+    w = workloads.config("cantilever")
+    g, o = run_cuda(w), run_oracle(w)
+    _compare(w, g, o)
+    assert abs(g["f_loaded"].reshape(-1, 3).sum(0)[2] + 1e6) < 1e-6       # total end shear = -1e6 N
+
+
+@pytest.mark.parametrize("k,dims,jit,gauss", [
+    (4, (5, 4, 4), 0.3, 1),        # smallest k: n = 8, only the four 2x2 pivots
+    (8, (6, 5, 5), 0.2, 1),
+    (27, (7, 7, 6), 0.25, 2),
+    (33, (8, 7, 7), 0.3, 2),       # k just over one warp
+    (40, (9, 8, 7), 0.3, 2),
+    (60, (10, 9, 8), 0.3, 2),
+    (64, (9, 9, 8), 0.3, 1),
+    (124, (9, 8, 8), 0.3, 1),      # maximum k: 128 x 128 moment systems
+])
+def test_jittered_blocks_span_tiles_and_ragged_tails(k, dims, jit, gauss):
+    # with k = 4 some boundary nodes belong to no support (no matrix row): use an empty BC list there,
+    # which also covers the m = 0 edge case of rpim_apply_penalty
+    w = workloads.make_block(f"j{k}", *dims, 1.0, gauss, k, 5e9, 0.3, jitter=jit, seed=100 + k,
+                             body=(10.0, -20.0, -2.5e4), bc="none" if k == 4 else "bottom+roller")
+    _compare(w, run_cuda(w), run_oracle(w))
+
+
+def test_nonunit_spacing_other_exponent_and_absolute_penalty():
+    w = workloads.make_block("q", 8, 7, 6, 0.37, 2, 30, 7e9, 0.33, jitter=0.25, seed=3, q=1.5, alpha_c=3.0,
+                             body=(0.0, 0.0, -1.0), bc="x0")
+    _compare(w, run_cuda(w), run_oracle(w))
+
+
+def test_run_to_run_bitwise_determinism_and_index_width():
+    w = workloads.make_block("det", 10, 9, 8, 1.0, 2, 40, 5e9, 0.3, jitter=0.3, seed=8,
+                             body=(0.0, 0.0, -2.5e4), bc="bottom")
+    a = run_cuda(w, index_bits=32)
+    b = run_cuda(w, index_bits=64)
+    c = run_cuda(w, index_bits=0)
+    assert a["bits"] == 32 and b["bits"] == 64 and c["bits"] == 32
+    assert a["row_ptr"].dtype == np.int32 and b["row_ptr"].dtype == np.int64
+    assert np.array_equal(a["row_ptr"], b["row_ptr"]) and np.array_equal(a["col_idx"], b["col_idx"])
+    for key in ("vals", "f", "vals0", "phi", "dphi"):
+        assert np.array_equal(a[key], b[key]) and np.array_equal(a[key], c[key])
+    assert a["launches"] > 0
+
+
+def test_planar_cloud_every_point_is_singular():
+    nodes = np.array([[i, j, 0.0] for j in range(6) for i in range(6)], dtype=np.float64)
+    w = workloads.make_block("flat", 6, 6, 2, 1.0, 1, 12, 1e9, 0.3)
+    w.nodes = nodes
+    w.qpts = np.ascontiguousarray(w.qpts[:25] * np.array([1.0, 1.0, 0.0]))
+    w.qw = np.ascontiguousarray(w.qw[:25])
+    w.bc_nodes = np.array([0, 1], dtype=np.int64)
+    w.bc_mask = np.array([7, 7], dtype=np.uint8)
+    w.bc_ubar = np.zeros((2, 3))
+    g, o = run_cuda(w, penalty=False), run_oracle(w, penalty=False)
+    assert g["nsing"] == o["nsing"] == 25
+    assert np.array_equal(g["support"], o["support"])
+    assert not g["vals"].any() and not g["phi"].any()
+
+
+def test_error_codes():
+    import torch
+    import paper_1802_04256_b200 as rp
+    w = workloads.make_block("e", 4, 4, 4, 1.0, 1, 8, 1e9, 0.3)
+    dev = torch.device("cuda:0")
+    dn, dq = torch.from_numpy(w.nodes).to(dev), torch.from_numpy(w.qpts).to(dev)
+    with rp.Context(0) as ctx:
+        with pytest.raises(rp.RpimError) as e:
+            ctx.build_pattern(dn, dq, 3)
+        assert e.value.code == -1
+        with pytest.raises(rp.RpimError) as e:
+            ctx.build_pattern(dn, dq, 65)          # k > N = 64
+        assert e.value.code == -1
+        with pytest.raises(rp.RpimError) as e:
+            ctx.assemble(torch.from_numpy(w.qw).to(dev), 1e9, 0.3, 4.0, 1.0, 1.03, (0, 0, 0),
+                         torch.empty(1, dtype=torch.float64, device=dev),
+                         torch.empty(1, dtype=torch.float64, device=dev))
+        assert e.value.code == -4                  # state: no pattern yet
+        nnz, bits = ctx.build_pattern(dn, dq, 8)
+        vals = torch.empty(nnz, dtype=torch.float64, device=dev)
+        f = torch.empty(3 * w.N, dtype=torch.float64, device=dev)
+        ctx.assemble(torch.from_numpy(w.qw).to(dev), 1e9, 0.3, 4.0, 1.0, 1.03, (0, 0, 0), vals, f)
+        bad = torch.tensor([1, 64], dtype=torch.int64, device=dev)
+        with pytest.raises(rp.RpimError) as e:
+            ctx.apply_penalty(bad, None, torch.zeros((2, 3), dtype=torch.float64, device=dev), 1.0, False, vals, f)
+        assert e.value.code == -5
+        assert ctx.workspace_bytes() > 0
+
+
+def test_host_buffer_entry_points_match_device_path():
+    import paper_1802_04256_b200 as rp
+    w = workloads.make_block("h", 9, 8, 7, 1.0, 2, 30, 5e9, 0.3, jitter=0.3, seed=21, body=(0.0, 0.0, -2.5e4),
+                             bc="bottom+roller")
+    g = run_cuda(w)
+    with rp.Context(0) as ctx:
+        nnz, bits = ctx.host_pattern(w.nodes, w.qpts, w.k, 0)
+        idt = np.int32 if bits == 32 else np.int64
+        rpa, cia = np.empty(3 * w.N + 1, idt), np.empty(nnz, idt)
+        vals, f = np.empty(nnz), np.empty(3 * w.N)
+        ns, alpha = ctx.host_assemble(w.qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, w.bc_nodes, w.bc_mask,
+                                      w.bc_ubar, w.penalty_alpha, True, rpa, cia, vals, f)
+    assert ns == 0 and alpha == g["alpha"]
+    assert np.array_equal(rpa, g["row_ptr"]) and np.array_equal(cia, g["col_idx"])
+    assert np.array_equal(vals, g["vals"]) and np.array_equal(f, g["f"])

@@ -1,0 +1,52 @@
+"""No-GPU checks of the boundary: librpim.so loads and exports every symbol include/rpim.h declares;
+the binding refuses to run without a CUDA device (no CPU fallback); product and oracle never import
+each other."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "rpim.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(rpim_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported_and_bound():
+    from paper_1802_04256_b200 import binding, build
+    path = build.build()
+    lib = ctypes.CDLL(path)
+    declared = _declared_symbols()
+    assert len(declared) >= 15
+    for sym in declared:
+        assert hasattr(lib, sym), f"{sym} declared in rpim.h but not exported"
+        assert hasattr(binding, sym), f"{sym} has no Python binding of the same name"
+    assert sorted(binding.EXPORTED_SYMBOLS) == declared
+
+
+def test_no_cpu_fallback_without_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    import paper_1802_04256_b200 as rp
+    with pytest.raises(rp.RpimError):
+        rp.rpim_create(0, 0)
+    with pytest.raises(RuntimeError):
+        rp.Context(0)
+
+
+def test_product_never_imports_oracle_and_vice_versa():
+    for sub, banned in (("paper_1802_04256_b200", "oracle"), ("oracle", "paper_1802_04256_b200")):
+        for dirpath, _, files in os.walk(os.path.join(ROOT, sub)):
+            for fn in files:
+                if fn.endswith(".py"):
+                    src = open(os.path.join(dirpath, fn)).read()
+                    assert not re.search(rf"^\s*(import|from)\s+\.*{banned}\b", src, flags=re.M), (fn, banned)
+                if fn.endswith((".cu", ".cuh", ".cpp", ".h")):
+                    src = open(os.path.join(dirpath, fn)).read()
+                    for inc in re.findall(r'#include\s+"([^"]+)"', src):
+                        assert banned not in inc and "oracle" not in inc.lower() or sub == "oracle", (fn, inc)

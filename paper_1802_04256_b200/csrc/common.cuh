@@ -158,6 +158,8 @@ int rpim_stage_block_pattern(rpim_ctx* ctx);
 int rpim_stage_emit_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx);
 int rpim_stage_shape(rpim_ctx* ctx, const double* d_pts, const int32_t* d_support, int64_t M, double* d_stage,
                      uint8_t* d_singular);
+int rpim_stage_shape_rows(rpim_ctx* ctx, const double* d_pts, const int32_t* d_support, int64_t M, double* d_stage,
+                          uint8_t* d_singular);   // 1 = no specialised kernel for ctx->k
 int rpim_stage_accumulate(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
                           double* d_vals, double* d_f);
 int rpim_stage_point_loads(rpim_ctx* ctx, const int32_t* d_support, const double* d_stage, const double* d_w,

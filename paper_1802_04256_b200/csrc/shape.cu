@@ -330,6 +330,10 @@ int rpim_stage_shape(rpim_ctx* ctx, const double* d_pts, const int32_t* d_suppor
                      uint8_t* d_singular) {
     if (M == 0) return RPIM_OK;
     const int k = ctx->k;
+    {   // register-resident kernels for the support sizes of the BASELINE.json configs (shape_rows.cu)
+        const int rc = rpim_stage_shape_rows(ctx, d_pts, d_support, M, d_stage, d_singular);
+        if (rc <= 0) return rc;
+    }
     const size_t per_warp = shape_smem_doubles_per_warp(k) * sizeof(double);
     int warps = 4;
     while (warps > 1 && per_warp * warps > 100 * 1024) warps >>= 1;

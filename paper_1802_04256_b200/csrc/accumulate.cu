@@ -1,15 +1,188 @@
 // Steps a5 + a6 (R8): w * B^T D B blocks and their deterministic reduction into the
 // CSR values, body-force load; step a5b (R9) point loads; step a7 (R10) penalty BCs.
 //
-// Reduction design: ROW OWNER.  Block row I (node I) is owned by one warp; it walks the node's
-// incidence list (points q whose support contains I, ascending q) and accumulates, for every
-// column J of supp(q), S_IJ += (w g_I) (x) g_J into an on-chip accumulator row.  Every CSR entry
-// is therefore summed in ascending q by exactly one warp: no floating-point atomics, bitwise
-// run-to-run reproducible, and K is written to HBM exactly once (never read).  The isotropic
-// closed form K_IJ = lambda S + mu S^T + mu tr(S) I is applied once per block at write-out.
+// Reduction design: ROW OWNER.  Block row I (node I) is owned by one group of warps; it walks the
+// node's incidence list (points q whose support contains I, ascending q) and accumulates, for
+// every column J of supp(q), S_IJ += (w g_I) (x) g_J.  Every CSR entry is therefore summed in
+// ascending q by exactly one thread: no floating-point atomics, bitwise run-to-run reproducible,
+// and K is written to HBM exactly once (never read).  The isotropic closed form
+// K_IJ = lambda S + mu S^T + mu tr(S) I is applied once per block at write-out.
+//
+// reduce_rows_kernel (rows of up to 1024 block columns): the accumulators live in REGISTERS.
+// Lane l of chunk c owns column slot 32 c + l of the row.  For a batch of incident points the
+// group first builds, per point, the bit mask of the row's slots that the point's support hits
+// (binary search of the sorted support in the sorted column list) with the running popcount per
+// 32-slot word; then every lane whose bit is set finds its node's position in the support as
+// prefix + popc(bits below), gathers that node's gradient (one 32-byte sector of the staged
+// [q][j][phi gx gy gz] array) and does nine fused multiply-adds.
+// accumulate_generic_kernel: fallback for longer rows, accumulators in shared memory.
 #include "common.cuh"
 
 namespace {
+
+constexpr unsigned FULLMASK = 0xffffffffu;
+
+template <int NWARP>
+__device__ __forceinline__ void group_sync(int rg) {
+    if constexpr (NWARP == 1) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(rg + 1), "r"(NWARP * 32) : "memory");
+}
+
+constexpr int ilog2_ce(int v) { return v <= 1 ? 0 : 1 + ilog2_ce(v >> 1); }
+
+constexpr int RED_NB = 32;   // incident points per batch
+
+template <int NWARP, int CPW>
+struct RedSmem {
+    static constexpr int NW = NWARP * CPW;
+    static constexpr int P2 = 1 << ilog2_ce(32 * NW - 1 + (32 * NW));   // power of two >= 32 NW
+    int cols[P2];                       // sorted block columns of the row, padded with INT_MAX
+    unsigned mask[RED_NB][NW];          // slots of the row hit by the support of point b
+    unsigned char pre[RED_NB][NW];      // support positions before word w
+    double a[RED_NB][3];                // w * grad phi_I at point b
+    const double* qbase[RED_NB];        // staged shape functions of point b
+    double fpart[NWARP];
+};
+
+// NWARP warps own one block row, each CPW chunks of 32 column slots (chunk c = cc * NWARP + wg);
+// a CTA holds ROWS such groups working on consecutive rows.
+template <int NWARP, int CPW, int ROWS>
+__global__ void __launch_bounds__(NWARP * ROWS * 32)
+reduce_rows_kernel(int64_t N, int k, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
+                   const uint8_t* __restrict__ inc_j, const int32_t* __restrict__ support,
+                   const double* __restrict__ stage, const double* __restrict__ qw,
+                   const int64_t* __restrict__ brow_ptr, const int32_t* __restrict__ bcol, double lambda, double mu,
+                   double bx, double by, double bz, double* __restrict__ vals, double* __restrict__ f) {
+    using S = RedSmem<NWARP, CPW>;
+    constexpr int NW = S::NW, P2 = S::P2;
+    extern __shared__ __align__(16) unsigned char red_smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int rg = warp / NWARP, wg = warp % NWARP;
+    S& sm = reinterpret_cast<S*>(red_smem_raw)[rg];
+    const unsigned lt = (1u << lane) - 1u;
+
+    for (int64_t I = (int64_t)blockIdx.x * ROWS + rg; I < N; I += (int64_t)gridDim.x * ROWS) {
+        const int64_t o = brow_ptr[I];
+        const int L = (int)(brow_ptr[I + 1] - o);
+        group_sync<NWARP>(rg);   // the previous row's shared data is dead
+        for (int s = wg * 32 + lane; s < P2; s += NWARP * 32) sm.cols[s] = (s < L) ? bcol[o + s] : 0x7FFFFFFF;
+        double acc[CPW][9];
+#pragma unroll
+        for (int cc = 0; cc < CPW; ++cc)
+#pragma unroll
+            for (int e = 0; e < 9; ++e) acc[cc][e] = 0.0;
+        double fsum = 0.0;
+        const int64_t pa = inc_ptr[I], pb = inc_ptr[I + 1];
+        for (int64_t p0 = pa; p0 < pb; p0 += RED_NB) {
+            const int nb = (int)min((int64_t)RED_NB, pb - p0);
+            group_sync<NWARP>(rg);   // cols visible; the previous batch has been consumed
+            // ---- phase 1: this warp prepares points b = wg, wg + NWARP, ... (lane t holds b = wg + NWARP t)
+            const int nmine = (nb - wg + NWARP - 1) / NWARP;
+            int qmine = 0;
+            {
+                const int bm = wg + NWARP * lane;
+                if (lane < nmine) {
+                    const int64_t p = p0 + bm;
+                    qmine = inc_q[p];
+                    const int i = inc_j[p];
+                    const double w = qw[qmine];
+                    const double* base = stage + (int64_t)qmine * k * 4;
+                    const double2 v01 = *reinterpret_cast<const double2*>(base + 4 * i);
+                    const double2 v23 = *reinterpret_cast<const double2*>(base + 4 * i + 2);
+                    fsum += w * v01.x;
+                    sm.a[bm][0] = w * v01.y; sm.a[bm][1] = w * v23.x; sm.a[bm][2] = w * v23.y;
+                    sm.qbase[bm] = base;
+                }
+            }
+            for (int t = 0; t < nmine; ++t) {
+                const int b = wg + NWARP * t;
+                const int q = __shfl_sync(FULLMASK, qmine, t);
+                const int32_t* sp = support + (int64_t)q * k;
+                unsigned mword = 0;   // lane w ends up with mask word w
+                for (int j0 = 0; j0 < k; j0 += 32) {
+                    const int j = j0 + lane;
+                    int slot = -1;
+                    if (j < k) {
+                        const int J = sp[j];
+                        int lo = 0;   // last index with cols[index] <= J; J is always present in the row
+#pragma unroll
+                        for (int step = P2 / 2; step > 0; step >>= 1)
+                            if (sm.cols[lo + step] <= J) lo += step;
+                        slot = lo;
+                    }
+                    const int wfirst = __shfl_sync(FULLMASK, slot, 0) >> 5;
+                    const int nact = min(32, k - j0);
+                    const int wlast = __shfl_sync(FULLMASK, slot, nact - 1) >> 5;
+                    const unsigned bit = (slot >= 0) ? (1u << (slot & 31)) : 0u;
+                    for (int w = wfirst; w <= wlast; ++w) {
+                        const unsigned m = __reduce_or_sync(FULLMASK, ((slot >> 5) == w) ? bit : 0u);
+                        if (lane == w) mword |= m;
+                    }
+                }
+                // exclusive prefix of the popcounts over the words (NW <= 32 words: one per lane)
+                const int cnt = __popc(mword);
+                int incl = cnt;
+#pragma unroll
+                for (int d = 1; d < NW; d <<= 1) {
+                    const int up = __shfl_up_sync(FULLMASK, incl, d);
+                    if (lane >= d) incl += up;
+                }
+                if (lane < NW) { sm.mask[b][lane] = mword; sm.pre[b][lane] = (unsigned char)(incl - cnt); }
+            }
+            group_sync<NWARP>(rg);
+            // ---- phase 2: every lane accumulates its slots over the points of the batch
+            for (int b = 0; b < nb; ++b) {
+                const double ax = sm.a[b][0], ay = sm.a[b][1], az = sm.a[b][2];
+                const double* base = sm.qbase[b];
+#pragma unroll
+                for (int cc = 0; cc < CPW; ++cc) {
+                    const int c = cc * NWARP + wg;
+                    const unsigned word = sm.mask[b][c];
+                    if (word == 0u) continue;
+                    if ((word >> lane) & 1u) {
+                        const int pos = sm.pre[b][c] + __popc(word & lt);
+                        const double* g = base + 4 * pos;
+                        const double gx = g[1];
+                        const double2 gyz = *reinterpret_cast<const double2*>(g + 2);
+                        acc[cc][0] = fma(ax, gx, acc[cc][0]); acc[cc][1] = fma(ax, gyz.x, acc[cc][1]); acc[cc][2] = fma(ax, gyz.y, acc[cc][2]);
+                        acc[cc][3] = fma(ay, gx, acc[cc][3]); acc[cc][4] = fma(ay, gyz.x, acc[cc][4]); acc[cc][5] = fma(ay, gyz.y, acc[cc][5]);
+                        acc[cc][6] = fma(az, gx, acc[cc][6]); acc[cc][7] = fma(az, gyz.x, acc[cc][7]); acc[cc][8] = fma(az, gyz.y, acc[cc][8]);
+                    }
+                }
+            }
+        }
+        // ---- K_IJ = lambda S + mu S^T + mu tr(S) I, three scalar rows per block row
+#pragma unroll
+        for (int cc = 0; cc < CPW; ++cc) {
+            const int s = 32 * (cc * NWARP + wg) + lane;
+            if (s < L) {
+                const double* a = acc[cc];
+                const double mtr = mu * ((a[0] + a[4]) + a[8]);
+#pragma unroll
+                for (int r = 0; r < 3; ++r) {
+                    double* dst = vals + 9 * o + (int64_t)r * 3 * L + 3 * s;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        double v = fma(lambda, a[3 * r + c], mu * a[3 * c + r]);
+                        if (r == c) v += mtr;
+                        dst[c] = v;
+                    }
+                }
+            }
+        }
+        // ---- body-force load: partial sums of the warps in a fixed order
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) fsum += __shfl_xor_sync(FULLMASK, fsum, d);
+        if constexpr (NWARP > 1) {
+            if (lane == 0) sm.fpart[wg] = fsum;
+            group_sync<NWARP>(rg);
+            fsum = 0.0;
+#pragma unroll
+            for (int w = 0; w < NWARP; ++w) fsum += sm.fpart[w];
+        }
+        if (wg == 0 && lane == 0) { f[3 * I] = fsum * bx; f[3 * I + 1] = fsum * by; f[3 * I + 2] = fsum * bz; }
+    }
+}
 
 __global__ void __launch_bounds__(256)
 accumulate_generic_kernel(int64_t N, int k, int Lcap, const int64_t* __restrict__ inc_ptr,
@@ -37,12 +210,12 @@ accumulate_generic_kernel(int64_t N, int k, int Lcap, const int64_t* __restrict_
             const int i = inc_j[p];
             const double w = qw[q];
             const double* st = stage + q * 4 * (int64_t)k;
-            const double wgx = w * st[k + i], wgy = w * st[2 * k + i], wgz = w * st[3 * k + i];
-            fI += w * st[i];
+            const double wgx = w * st[4 * i + 1], wgy = w * st[4 * i + 2], wgz = w * st[4 * i + 3];
+            fI += w * st[4 * i];
             const int32_t* sp = support + q * k;
             for (int j = lane; j < k; j += 32) {
                 const int J = sp[j];
-                const double gx = st[k + j], gy = st[2 * k + j], gz = st[3 * k + j];
+                const double gx = st[4 * j + 1], gy = st[4 * j + 2], gz = st[4 * j + 3];
                 int lo = 0, hi = L - 1;   // J is always present in the row
                 while (lo < hi) {
                     const int mid = (lo + hi) >> 1;
@@ -85,7 +258,7 @@ __global__ void point_loads_kernel(const int32_t* __restrict__ support, const do
         const double wp = w[p], tx = t[3 * p], ty = t[3 * p + 1], tz = t[3 * p + 2];
         for (int j = lane; j < k; j += 32) {
             const int64_t J = support[p * k + j];
-            const double wphi = wp * st[j];
+            const double wphi = wp * st[4 * j];
             f[3 * J] += wphi * tx;
             f[3 * J + 1] += wphi * ty;
             f[3 * J + 2] += wphi * tz;
@@ -155,7 +328,7 @@ __global__ void penalty_apply_kernel(int64_t N, const int64_t* __restrict__ bc_n
 
 }  // namespace
 
-int rpim_stage_accumulate(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
+static int accumulate_generic(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
                           double* d_vals, double* d_f) {
     const int Lcap = std::max(ctx->max_blen, 1);
     const size_t per_warp = ((size_t)Lcap * 9 + (Lcap + 1) / 2) * sizeof(double);
@@ -172,6 +345,42 @@ int rpim_stage_accumulate(rpim_ctx* ctx, const double* d_qw, double lambda, doub
         ctx->d_brow_ptr, ctx->d_bcol, lambda, mu, body[0], body[1], body[2], d_vals, d_f);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
+}
+
+namespace {
+template <int NWARP, int CPW, int ROWS>
+int launch_reduce_rows(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
+                       double* d_vals, double* d_f) {
+    auto kern = reduce_rows_kernel<NWARP, CPW, ROWS>;
+    const size_t smem = sizeof(RedSmem<NWARP, CPW>) * ROWS;
+    CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 1;
+    CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NWARP * ROWS * 32, smem));
+    if (per_sm < 1) per_sm = 1;
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
+    int64_t blocks = (ctx->N + ROWS - 1) / ROWS;
+    blocks = std::min<int64_t>(blocks, (int64_t)sms * per_sm * 8);   // several waves: boundary rows are cheaper
+    kern<<<(unsigned)blocks, NWARP * ROWS * 32, smem, ctx->stream>>>(
+        ctx->N, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_support, ctx->d_stage, d_qw,
+        ctx->d_brow_ptr, ctx->d_bcol, lambda, mu, body[0], body[1], body[2], d_vals, d_f);
+    KERNEL_CHECK(ctx);
+    return RPIM_OK;
+}
+}  // namespace
+
+int rpim_stage_accumulate(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
+                          double* d_vals, double* d_f) {
+    const int Lmax = std::max(ctx->max_blen, 1);
+    static_assert(sizeof(RedSmem<1, 4>) % 8 == 0 && sizeof(RedSmem<8, 4>) % 8 == 0, "group stride keeps 8-byte alignment");
+    if (Lmax <= 128) return launch_reduce_rows<1, 4, 8>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
+    if (Lmax <= 192) return launch_reduce_rows<2, 3, 4>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
+    if (Lmax <= 256) return launch_reduce_rows<2, 4, 4>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
+    if (Lmax <= 384) return launch_reduce_rows<4, 3, 2>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
+    if (Lmax <= 512) return launch_reduce_rows<4, 4, 2>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
+    if (Lmax <= 768) return launch_reduce_rows<8, 3, 1>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
+    if (Lmax <= 1024) return launch_reduce_rows<8, 4, 1>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
+    return accumulate_generic(ctx, d_qw, lambda, mu, body, d_vals, d_f);
 }
 
 int rpim_stage_point_loads(rpim_ctx* ctx, const int32_t* d_support, const double* d_stage, const double* d_w,

@@ -223,8 +223,9 @@ __global__ void split_stage_kernel(const double* __restrict__ stage, int64_t M, 
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
         const int64_t q = e / (4 * k);
         const int r = (int)(e % (4 * k));
-        if (r < k) { if (phi) phi[q * k + r] = stage[e]; }
-        else if (dphi) dphi[q * 3 * (int64_t)k + (r - k)] = stage[e];
+        const int j = r >> 2, c = r & 3;          // staged layout: [q][j][phi, d/dx, d/dy, d/dz]
+        if (c == 0) { if (phi) phi[q * k + j] = stage[e]; }
+        else if (dphi) dphi[(q * 3 + (c - 1)) * (int64_t)k + j] = stage[e];
     }
 }
 }  // namespace

@@ -13,7 +13,7 @@
 #define RPIM_WARP 32
 
 // device-side error / counter slots (ctx->d_flags, int64 each)
-enum { FLAG_KNN_CAP = 0, FLAG_PAT_CAP = 1, FLAG_BC_BAD = 2, FLAG_SINGULAR = 3, FLAG_INC_CAP = 4, NUM_FLAGS = 8 };
+enum { FLAG_KNN_CAP = 0, FLAG_PAT_CAP = 1, FLAG_BC_BAD = 2, FLAG_SINGULAR = 3, FLAG_INC_CAP = 4, FLAG_OVF_ROWS = 5, FLAG_OVF_Q = 6, NUM_FLAGS = 8 };
 
 struct GridParams {
     double lo[3];
@@ -76,7 +76,7 @@ struct rpim_ctx {
     int32_t* d_bcol = nullptr;       // nnzb
     int* d_bdiag = nullptr;          // N (slot of the diagonal block in its row)
 
-    // staged shape functions: Nq x 4 x k  (phi, dphi/dx, dphi/dy, dphi/dz)
+    // staged shape functions: Nq x k x 4  (phi, dphi/dx, dphi/dy, dphi/dz per support node: one 32-byte sector)
     double* d_stage = nullptr;
     uint8_t* d_singular = nullptr;   // Nq
     ShapeParams sp{};

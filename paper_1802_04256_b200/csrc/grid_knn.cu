@@ -213,26 +213,32 @@ __global__ void cell_sort_gather_kernel(const double* __restrict__ nodes, int64_
 }
 
 // ------------------------------------------------------------------ the search: one warp per query point
-constexpr int KNN_CAP = 2048;          // candidates held on chip per query
-constexpr int KNN_WARPS = 4;
+// CAP = candidates held on chip per query.  The first launch uses the smallest capacity that
+// fits the expected candidate count (more resident warps); queries that need more are appended
+// to an overflow list and redone by the KNN_CAP_MAX instantiation (LAST: overflow = failure).
+constexpr int KNN_CAP_MAX = 2048;
 
-__global__ void __launch_bounds__(KNN_WARPS * 32)
+template <int CAP, int WARPS, bool LAST>
+__global__ void __launch_bounds__(WARPS * 32)
 knn_kernel(GridParams g, const double* __restrict__ sx, const double* __restrict__ sy,
            const double* __restrict__ sz, const int* __restrict__ node_order,
            const int64_t* __restrict__ cell_start, const double* __restrict__ pts, int64_t M, int k, int R0,
-           int32_t* __restrict__ support, long long* __restrict__ flags) {
+           const int32_t* __restrict__ qlist, const long long* __restrict__ nq_ptr,
+           int32_t* __restrict__ ovf_list, int32_t* __restrict__ support, long long* __restrict__ flags) {
     extern __shared__ unsigned char smem_raw[];
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    unsigned long long* key = (unsigned long long*)smem_raw + (size_t)wid * KNN_CAP;
-    int* val = (int*)((unsigned long long*)smem_raw + (size_t)KNN_WARPS * KNN_CAP) + (size_t)wid * KNN_CAP;
+    unsigned long long* key = (unsigned long long*)smem_raw + (size_t)wid * CAP;
+    int* val = (int*)((unsigned long long*)smem_raw + (size_t)WARPS * CAP) + (size_t)wid * CAP;
+    const int64_t nq = qlist ? (int64_t)*nq_ptr : M;
 
-    for (int64_t q = (int64_t)blockIdx.x * KNN_WARPS + wid; q < M; q += (int64_t)gridDim.x * KNN_WARPS) {
+    for (int64_t qi = (int64_t)blockIdx.x * WARPS + wid; qi < nq; qi += (int64_t)gridDim.x * WARPS) {
+        const int64_t q = qlist ? qlist[qi] : qi;
         const double xq = pts[3 * q], yq = pts[3 * q + 1], zq = pts[3 * q + 2];
         int cq[3];
         cell_coords(g, xq, yq, zq, cq);
         int R = R0;
         int npad = 0;
-        bool fail = false;
+        bool fail = false, overflow = false;
         while (true) {
             int a[3], b[3];
             bool whole = true;
@@ -252,14 +258,13 @@ knn_kernel(GridParams g, const double* __restrict__ sx, const double* __restrict
                 int64_t c1 = c0 + (b[0] - a[0]);
                 cnt += (int)(cell_start[c1 + 1] - cell_start[c0]);
             }
-#pragma unroll
-            for (int d = 16; d > 0; d >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, d);
+            cnt = __reduce_add_sync(0xffffffffu, cnt);
             if (cnt < k) {
                 if (whole) { fail = true; break; }
                 ++R;
                 continue;
             }
-            if (cnt > KNN_CAP) { fail = true; break; }
+            if (cnt > CAP) { overflow = true; break; }
             // gather candidates with their squared distances (R1: no fma, fixed association)
             int base = 0;
             for (int r = 0; r < nrows; ++r) {
@@ -292,7 +297,15 @@ knn_kernel(GridParams g, const double* __restrict__ sx, const double* __restrict
             if (bound > 0.0 && dk < bound * bound) break;
             ++R;
         }
-        if (fail) {
+        if (overflow && !LAST) {
+            if (lane == 0) {
+                const unsigned long long slot = atomicAdd((unsigned long long*)&flags[FLAG_OVF_Q], 1ull);
+                ovf_list[slot] = (int32_t)q;
+            }
+            __syncwarp();
+            continue;
+        }
+        if (fail || overflow) {
             if (lane == 0) atomicAdd((unsigned long long*)&flags[FLAG_KNN_CAP], 1ull);
             for (int j = lane; j < k; j += 32) support[q * k + j] = 0;
             __syncwarp();
@@ -306,6 +319,21 @@ knn_kernel(GridParams g, const double* __restrict__ sx, const double* __restrict
         for (int j = lane; j < k; j += 32) support[q * k + j] = val[j];
         __syncwarp();
     }
+}
+
+template <int CAP, int WARPS, bool LAST>
+int launch_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, const int32_t* qlist, int32_t* ovf_list,
+               int32_t* d_support, int64_t blocks_cap) {
+    const int64_t N = ctx->N;
+    auto kern = knn_kernel<CAP, WARPS, LAST>;
+    const size_t smem = (size_t)WARPS * CAP * (sizeof(unsigned long long) + sizeof(int));
+    CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int64_t blocks = qlist ? blocks_cap : std::min<int64_t>((M + WARPS - 1) / WARPS, blocks_cap);
+    kern<<<(unsigned)blocks, WARPS * 32, smem, ctx->stream>>>(
+        ctx->grid, ctx->d_sorted_xyz, ctx->d_sorted_xyz + N, ctx->d_sorted_xyz + 2 * N, ctx->d_node_order,
+        ctx->d_cell_start, d_pts, M, k, 2, qlist, ctx->d_flags + FLAG_OVF_Q, ovf_list, d_support, ctx->d_flags);
+    KERNEL_CHECK(ctx);
+    return RPIM_OK;
 }
 }  // namespace
 
@@ -367,13 +395,22 @@ int rpim_stage_grid_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, in
         KERNEL_CHECK(ctx);
     }
     if (M == 0) return RPIM_OK;
-    const size_t smem = (size_t)KNN_WARPS * KNN_CAP * (sizeof(unsigned long long) + sizeof(int));
-    CUDA_TRY(ctx, cudaFuncSetAttribute(knn_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int64_t blocks = (M + KNN_WARPS - 1) / KNN_WARPS;
-    if (blocks > 148 * 64) blocks = 148 * 64;
-    knn_kernel<<<(unsigned)blocks, KNN_WARPS * 32, smem, st>>>(
-        ctx->grid, ctx->d_sorted_xyz, ctx->d_sorted_xyz + N, ctx->d_sorted_xyz + 2 * N, ctx->d_node_order,
-        ctx->d_cell_start, d_pts, M, k, 2, d_support, ctx->d_flags);
-    KERNEL_CHECK(ctx);
-    return RPIM_OK;
+    // expected candidates in the first (2 R0 + 1)^3 = 125 cells, with a margin for density fluctuations
+    const GridParams& g = ctx->grid;
+    const double per_cell = (double)N / (double)g.ncell;
+    const double expect = 125.0 * per_cell * 1.25;
+    const int cap = expect <= 256 ? 256 : expect <= 512 ? 512 : expect <= 1024 ? 1024 : KNN_CAP_MAX;
+    int rc = RPIM_OK;
+    if (cap == KNN_CAP_MAX) return launch_knn<KNN_CAP_MAX, 4, true>(ctx, d_pts, M, k, nullptr, nullptr, d_support, 148 * 64);
+    int32_t* d_ovf = nullptr;
+    if ((rc = ws_alloc(ctx, &d_ovf, M))) return rc;
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_OVF_Q, 0, sizeof(long long), st));
+    if (cap == 256) rc = launch_knn<256, 8, false>(ctx, d_pts, M, k, nullptr, d_ovf, d_support, 148 * 64);
+    else if (cap == 512) rc = launch_knn<512, 8, false>(ctx, d_pts, M, k, nullptr, d_ovf, d_support, 148 * 64);
+    else rc = launch_knn<1024, 4, false>(ctx, d_pts, M, k, nullptr, d_ovf, d_support, 148 * 64);
+    if (rc == RPIM_OK) rc = launch_knn<KNN_CAP_MAX, 4, true>(ctx, d_pts, M, k, d_ovf, nullptr, d_support, 148 * 2);
+    // the overflow list is read by the second launch: keep it until the stream has drained
+    if (rc == RPIM_OK) { cudaError_t e = cudaStreamSynchronize(st); if (e != cudaSuccess) rc = RPIM_ERR_CUDA; }
+    ws_free(ctx, &d_ovf);
+    return rc;
 }

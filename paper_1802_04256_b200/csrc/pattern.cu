@@ -56,60 +56,148 @@ inc_sort_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, int32_t* __restr
 }
 
 // ------------------------------------------------------------------ block rows: union of the supports of incident points
-constexpr int PAT_HASH = 4096;          // open-addressing table per warp (power of two)
+// Block row I = sorted union of supp(q) over the points q incident to node I.  A warp owns a row
+// and builds the union in an open-addressing table in shared memory.
+//
+// Fast path (brow_fast_kernel): a small table (HASH entries) and ONE pass -- the sorted row is
+// parked in a fixed-stride pool, lengths are scanned, rows are copied to their CSR place.  Rows
+// that do not fit (more than PSTRIDE columns) go to an overflow list and take the general
+// two-pass path (count, scan, fill) with the large table.
+constexpr int PAT_HASH = 4096;          // general path: open-addressing table per warp (power of two)
 constexpr int PAT_MAXROW = 2048;        // longest block row handled
 constexpr int PAT_WARPS = 4;
+constexpr int PAT_FAST_WARPS = 8;
 
-__device__ __forceinline__ unsigned pat_hash(int key) { return ((unsigned)key * 2654435761u) >> 20; }   // 12 bits
+template <int HASH>
+__device__ __forceinline__ unsigned pat_hash(int key) {
+    return (((unsigned)key * 2654435761u) >> 16) & (HASH - 1);
+}
 
-// returns the number of distinct columns of block row I (all lanes), leaving them in `table`;
-// PAT_MAXROW + 1 if the row does not fit
+// Number of distinct columns of block row I (same value in all lanes), leaving them in `table`
+// (HASH entries, -1 = empty); LIMIT + 1 when the row has more than LIMIT columns.  The total is
+// checked after every point, a point adds at most RPIM_MAX_K keys, so the table never holds more
+// than LIMIT + RPIM_MAX_K < HASH keys and probing always terminates.
+template <int HASH, int LIMIT>
 __device__ __forceinline__ int row_union(int* table, int64_t I, const int64_t* __restrict__ inc_ptr,
                                          const int32_t* __restrict__ inc_q, const int32_t* __restrict__ support,
                                          int k) {
+    static_assert(LIMIT + RPIM_MAX_K < HASH, "table too small");
     const int lane = lane_id();
-    for (int i = lane; i < PAT_HASH; i += 32) table[i] = -1;
+    for (int i = lane; i < HASH; i += 32) table[i] = -1;
     __syncwarp();
-    int fresh = 0;
-    bool overflow = false;
+    int total = 0;
     const int64_t a = inc_ptr[I], b = inc_ptr[I + 1];
-    for (int64_t p = a; p < b; ++p) {
-        const int32_t* s = support + (int64_t)inc_q[p] * k;
-        for (int j = lane; j < k; j += 32) {
-            int key = s[j];
-            unsigned h = pat_hash(key) & (PAT_HASH - 1);
-            for (int probes = 0;; ++probes) {
-                if (probes >= PAT_HASH) { overflow = true; break; }
-                int old = atomicCAS(&table[h], -1, key);
-                if (old == -1) { ++fresh; break; }
-                if (old == key) break;
-                h = (h + 1) & (PAT_HASH - 1);
+    for (int64_t p0 = a; p0 < b; p0 += 32) {
+        const int64_t pl = p0 + lane;
+        const int qmine = (pl < b) ? inc_q[pl] : 0;
+        const int np = (int)min((int64_t)32, b - p0);
+        for (int pp = 0; pp < np; ++pp) {
+            const int q = __shfl_sync(0xffffffffu, qmine, pp);
+            const int32_t* s = support + (int64_t)q * k;
+            int fresh = 0;
+            for (int j = lane; j < k; j += 32) {
+                const int key = s[j];
+                unsigned h = pat_hash<HASH>(key);
+                while (true) {
+                    const int old = atomicCAS(&table[h], -1, key);
+                    if (old == -1) { ++fresh; break; }
+                    if (old == key) break;
+                    h = (h + 1) & (HASH - 1);
+                }
             }
-        }
-        // every 8 points (<= 8 * RPIM_MAX_K new keys) stop if the row is already too long, so the
-        // table never fills up: 2048 + 992 < PAT_HASH
-        if (((p - a) & 7) == 7) {
-            int tot = fresh;
-#pragma unroll
-            for (int d = 16; d > 0; d >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, d);
-            if (tot > PAT_MAXROW || __any_sync(0xffffffffu, overflow)) return PAT_MAXROW + 1;
+            total += __reduce_add_sync(0xffffffffu, fresh);
+            if (total > LIMIT) return LIMIT + 1;
         }
     }
-    if (__any_sync(0xffffffffu, overflow)) return PAT_MAXROW + 1;
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) fresh += __shfl_xor_sync(0xffffffffu, fresh, d);
     __syncwarp();
-    return fresh;
+    return total;
 }
 
+// compact the table into `list`, pad to a power of two and sort ascending; returns nothing
+template <int HASH>
+__device__ __forceinline__ void table_to_sorted_list(const int* table, int* list, int L) {
+    const int lane = lane_id();
+    int base = 0;
+    for (int i0 = 0; i0 < HASH; i0 += 32) {
+        const int v = table[i0 + lane];
+        const unsigned m = __ballot_sync(0xffffffffu, v >= 0);
+        if (v >= 0) list[base + __popc(m & ((1u << lane) - 1))] = v;
+        base += __popc(m);
+    }
+    const int np = next_pow2(L);
+    for (int i = L + lane; i < np; i += 32) list[i] = 0x7FFFFFFF;
+    __syncwarp();
+    warp_bitonic_i32(list, np);
+}
+
+template <int HASH, int PSTRIDE>
+__global__ void __launch_bounds__(PAT_FAST_WARPS * 32)
+brow_fast_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
+                 const int32_t* __restrict__ support, int k, int* __restrict__ blen, int32_t* __restrict__ pool,
+                 int* __restrict__ bdiag, int32_t* __restrict__ ovf_rows, long long* __restrict__ flags) {
+    __shared__ int table_s[PAT_FAST_WARPS][HASH];
+    __shared__ int list_s[PAT_FAST_WARPS][PSTRIDE];
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int* table = table_s[wid];
+    int* list = list_s[wid];
+    for (int64_t I = (int64_t)blockIdx.x * PAT_FAST_WARPS + wid; I < N; I += (int64_t)gridDim.x * PAT_FAST_WARPS) {
+        const int L = row_union<HASH, PSTRIDE>(table, I, inc_ptr, inc_q, support, k);
+        if (L > PSTRIDE) {
+            if (lane == 0) {
+                blen[I] = 0;
+                const unsigned long long slot = atomicAdd((unsigned long long*)&flags[FLAG_OVF_ROWS], 1ull);
+                ovf_rows[slot] = (int32_t)I;
+            }
+            __syncwarp();
+            continue;
+        }
+        table_to_sorted_list<HASH>(table, list, L);
+        int32_t* dst = pool + I * PSTRIDE;
+        for (int i = lane; i < L; i += 32) {
+            const int c = list[i];
+            dst[i] = c;
+            if (c == (int)I) bdiag[I] = i;
+        }
+        if (lane == 0) blen[I] = L;
+        __syncwarp();
+    }
+}
+
+// rows parked in the pool -> their place in the block-CSR column array (overflow rows have a
+// negative pool marker: their length was set by the count pass, the fill pass writes them)
+template <int PSTRIDE>
+__global__ void __launch_bounds__(256)
+brow_copy_kernel(int64_t N, const int64_t* __restrict__ brow_ptr, const int32_t* __restrict__ pool,
+                 const uint8_t* __restrict__ is_ovf, int32_t* __restrict__ bcol) {
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int64_t I = (int64_t)blockIdx.x * 8 + wid; I < N; I += (int64_t)gridDim.x * 8) {
+        if (is_ovf[I]) continue;
+        const int64_t o = brow_ptr[I];
+        const int L = (int)(brow_ptr[I + 1] - o);
+        const int32_t* src = pool + I * PSTRIDE;
+        for (int i = lane; i < L; i += 32) bcol[o + i] = src[i];
+    }
+}
+
+__global__ void mark_rows_kernel(const int32_t* __restrict__ rows, const long long* __restrict__ nrows,
+                                 uint8_t* __restrict__ mark) {
+    const long long n = *nrows;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        mark[rows[i]] = 1;
+}
+
+// General path over a row list (rows == nullptr: all N rows).
 __global__ void __launch_bounds__(PAT_WARPS * 32)
-brow_count_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
+brow_count_kernel(int64_t N, const int32_t* __restrict__ rows, const long long* __restrict__ nrows,
+                  const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
                   const int32_t* __restrict__ support, int k, int* __restrict__ blen, long long* __restrict__ flags) {
     extern __shared__ int pat_smem[];
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int* table = pat_smem + (size_t)wid * PAT_HASH;
-    for (int64_t I = (int64_t)blockIdx.x * PAT_WARPS + wid; I < N; I += (int64_t)gridDim.x * PAT_WARPS) {
-        const int L = row_union(table, I, inc_ptr, inc_q, support, k);
+    const int64_t n = rows ? (int64_t)*nrows : N;
+    for (int64_t r = (int64_t)blockIdx.x * PAT_WARPS + wid; r < n; r += (int64_t)gridDim.x * PAT_WARPS) {
+        const int64_t I = rows ? rows[r] : r;
+        const int L = row_union<PAT_HASH, PAT_MAXROW>(table, I, inc_ptr, inc_q, support, k);
         if (L > PAT_MAXROW && lane == 0) atomicAdd((unsigned long long*)&flags[FLAG_PAT_CAP], 1ull);
         if (lane == 0) blen[I] = min(L, PAT_MAXROW);
         __syncwarp();
@@ -117,31 +205,23 @@ brow_count_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t*
 }
 
 __global__ void __launch_bounds__(PAT_WARPS * 32)
-brow_fill_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
+brow_fill_kernel(int64_t N, const int32_t* __restrict__ rows, const long long* __restrict__ nrows,
+                 const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
                  const int32_t* __restrict__ support, int k, const int64_t* __restrict__ brow_ptr,
                  int32_t* __restrict__ bcol, int* __restrict__ bdiag) {
     extern __shared__ int pat_smem[];
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int* table = pat_smem + (size_t)wid * PAT_HASH;
     int* list = pat_smem + (size_t)PAT_WARPS * PAT_HASH + (size_t)wid * PAT_MAXROW;
-    for (int64_t I = (int64_t)blockIdx.x * PAT_WARPS + wid; I < N; I += (int64_t)gridDim.x * PAT_WARPS) {
-        const int L = row_union(table, I, inc_ptr, inc_q, support, k);
+    const int64_t n = rows ? (int64_t)*nrows : N;
+    for (int64_t r = (int64_t)blockIdx.x * PAT_WARPS + wid; r < n; r += (int64_t)gridDim.x * PAT_WARPS) {
+        const int64_t I = rows ? rows[r] : r;
+        const int L = row_union<PAT_HASH, PAT_MAXROW>(table, I, inc_ptr, inc_q, support, k);
         if (L > PAT_MAXROW) continue;   // reported by the count pass
-        // compact the table into the list
-        int base = 0;
-        for (int i0 = 0; i0 < PAT_HASH; i0 += 32) {
-            int v = table[i0 + lane];
-            unsigned m = __ballot_sync(0xffffffffu, v >= 0);
-            if (v >= 0) list[base + __popc(m & ((1u << lane) - 1))] = v;
-            base += __popc(m);
-        }
-        const int np = next_pow2(L);
-        for (int i = L + lane; i < np; i += 32) list[i] = 0x7FFFFFFF;
-        __syncwarp();
-        warp_bitonic_i32(list, np);
+        table_to_sorted_list<PAT_HASH>(table, list, L);
         const int64_t o = brow_ptr[I];
         for (int i = lane; i < L; i += 32) {
-            int c = list[i];
+            const int c = list[i];
             bcol[o + i] = c;
             if (c == (int)I) bdiag[I] = i;
         }
@@ -217,6 +297,27 @@ int rpim_stage_incidence(rpim_ctx* ctx) {
     return RPIM_OK;
 }
 
+namespace {
+template <int HASH, int PSTRIDE>
+int launch_brow_fast(rpim_ctx* ctx, int32_t* d_pool, int32_t* d_ovf_rows) {
+    const int64_t N = ctx->N;
+    const unsigned nb = (unsigned)std::min<int64_t>((N + PAT_FAST_WARPS - 1) / PAT_FAST_WARPS, 148 * 16);
+    brow_fast_kernel<HASH, PSTRIDE><<<nb, PAT_FAST_WARPS * 32, 0, ctx->stream>>>(
+        N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->k, ctx->d_blen, d_pool, ctx->d_bdiag, d_ovf_rows,
+        ctx->d_flags);
+    KERNEL_CHECK(ctx);
+    return RPIM_OK;
+}
+template <int PSTRIDE>
+int launch_brow_copy(rpim_ctx* ctx, const int32_t* d_pool, const uint8_t* d_is_ovf) {
+    const int64_t N = ctx->N;
+    brow_copy_kernel<PSTRIDE><<<(unsigned)std::min<int64_t>((N + 7) / 8, 148 * 32), 256, 0, ctx->stream>>>(
+        N, ctx->d_brow_ptr, d_pool, d_is_ovf, ctx->d_bcol);
+    KERNEL_CHECK(ctx);
+    return RPIM_OK;
+}
+}  // namespace
+
 int rpim_stage_block_pattern(rpim_ctx* ctx) {
     cudaStream_t st = ctx->stream;
     const int64_t N = ctx->N;
@@ -224,15 +325,38 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
     if ((rc = ws_alloc(ctx, &ctx->d_blen, N))) return rc;
     if ((rc = ws_alloc(ctx, &ctx->d_brow_ptr, N + 1))) return rc;
     if ((rc = ws_alloc(ctx, &ctx->d_bdiag, N))) return rc;
+    // Fast path when the expected row length (about 5..8 supports' worth of columns) fits the
+    // pool stride; pstride = 0 selects the general two-pass path for every row.
+    const int pstride = (8 * ctx->k <= 256) ? 256 : (8 * ctx->k <= 512) ? 512 : 0;
+    int32_t *d_pool = nullptr, *d_ovf_rows = nullptr;
+    uint8_t* d_is_ovf = nullptr;
+    auto drop_tmp = [&]() { ws_free(ctx, &d_pool); ws_free(ctx, &d_ovf_rows); ws_free(ctx, &d_is_ovf); };
+    const long long* d_novf = ctx->d_flags + FLAG_OVF_ROWS;
     const unsigned nb = (unsigned)std::min<int64_t>((N + PAT_WARPS - 1) / PAT_WARPS, 148 * 16);
+    const unsigned nb_ovf = 148 * 2;   // the overflow list is normally empty: a small fixed grid
     const size_t smem_cnt = (size_t)PAT_WARPS * PAT_HASH * sizeof(int);
     const size_t smem_fill = smem_cnt + (size_t)PAT_WARPS * PAT_MAXROW * sizeof(int);
     CUDA_TRY(ctx, cudaFuncSetAttribute(brow_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cnt));
     CUDA_TRY(ctx, cudaFuncSetAttribute(brow_fill_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fill));
-    brow_count_kernel<<<nb, PAT_WARPS * 32, smem_cnt, st>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->k,
-                                                     ctx->d_blen, ctx->d_flags);
-    KERNEL_CHECK(ctx);
-    if ((rc = rpim_scan_i32_to_i64(ctx, ctx->d_blen, ctx->d_brow_ptr, N))) return rc;
+    if (pstride) {
+        if ((rc = ws_alloc(ctx, &d_pool, N * pstride)) || (rc = ws_alloc(ctx, &d_ovf_rows, N)) ||
+            (rc = ws_alloc(ctx, &d_is_ovf, N))) { drop_tmp(); return rc; }
+        CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_OVF_ROWS, 0, sizeof(long long), st));
+        CUDA_TRY(ctx, cudaMemsetAsync(d_is_ovf, 0, (size_t)N, st));
+        rc = (pstride == 256) ? launch_brow_fast<512, 256>(ctx, d_pool, d_ovf_rows)
+                              : launch_brow_fast<1024, 512>(ctx, d_pool, d_ovf_rows);
+        if (rc) { drop_tmp(); return rc; }
+        mark_rows_kernel<<<64, 256, 0, st>>>(d_ovf_rows, d_novf, d_is_ovf);
+        KERNEL_CHECK(ctx);
+        brow_count_kernel<<<nb_ovf, PAT_WARPS * 32, smem_cnt, st>>>(N, d_ovf_rows, d_novf, ctx->d_inc_ptr, ctx->d_inc_q,
+                                                                     ctx->d_support, ctx->k, ctx->d_blen, ctx->d_flags);
+        KERNEL_CHECK(ctx);
+    } else {
+        brow_count_kernel<<<nb, PAT_WARPS * 32, smem_cnt, st>>>(N, nullptr, nullptr, ctx->d_inc_ptr, ctx->d_inc_q,
+                                                                 ctx->d_support, ctx->k, ctx->d_blen, ctx->d_flags);
+        KERNEL_CHECK(ctx);
+    }
+    if ((rc = rpim_scan_i32_to_i64(ctx, ctx->d_blen, ctx->d_brow_ptr, N))) { drop_tmp(); return rc; }
     int* d_max = (int*)ctx->d_scratch;
     CUDA_TRY(ctx, cudaMemsetAsync(d_max, 0, sizeof(int), st));
     max_i32_kernel<<<(unsigned)std::min<int64_t>((N + 255) / 256, 1024), 256, 0, st>>>(ctx->d_blen, N, d_max);
@@ -242,19 +366,39 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
     CUDA_TRY(ctx, cudaMemcpyAsync(&ctx->max_blen, d_max, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaMemcpyAsync(h_flags, ctx->d_flags, sizeof(h_flags), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaStreamSynchronize(st));
-    if (h_flags[FLAG_KNN_CAP])
+    if (h_flags[FLAG_KNN_CAP]) {
+        drop_tmp();
         RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "kNN: %lld points need more than the on-chip candidate capacity (or k > N)",
                   h_flags[FLAG_KNN_CAP]);
-    if (h_flags[FLAG_INC_CAP])
+    }
+    if (h_flags[FLAG_INC_CAP]) {
+        drop_tmp();
         RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "incidence: %lld nodes belong to more than %d supports", h_flags[FLAG_INC_CAP],
                   INC_CAP);
-    if (h_flags[FLAG_PAT_CAP])
+    }
+    if (h_flags[FLAG_PAT_CAP]) {
+        drop_tmp();
         RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "pattern: %lld block rows are longer than %d", h_flags[FLAG_PAT_CAP],
                   PAT_MAXROW);
-    if ((rc = ws_alloc(ctx, &ctx->d_bcol, ctx->nnzb))) return rc;
-    brow_fill_kernel<<<nb, PAT_WARPS * 32, smem_fill, st>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->k,
-                                                    ctx->d_brow_ptr, ctx->d_bcol, ctx->d_bdiag);
-    KERNEL_CHECK(ctx);
+    }
+    if ((rc = ws_alloc(ctx, &ctx->d_bcol, ctx->nnzb))) { drop_tmp(); return rc; }
+    if (pstride) {
+        rc = (pstride == 256) ? launch_brow_copy<256>(ctx, d_pool, d_is_ovf) : launch_brow_copy<512>(ctx, d_pool, d_is_ovf);
+        if (rc) { drop_tmp(); return rc; }
+        if (h_flags[FLAG_OVF_ROWS] > 0) {
+            brow_fill_kernel<<<nb_ovf, PAT_WARPS * 32, smem_fill, st>>>(N, d_ovf_rows, d_novf, ctx->d_inc_ptr,
+                                                                        ctx->d_inc_q, ctx->d_support, ctx->k,
+                                                                        ctx->d_brow_ptr, ctx->d_bcol, ctx->d_bdiag);
+            KERNEL_CHECK(ctx);
+        }
+        CUDA_TRY(ctx, cudaStreamSynchronize(st));   // the pool is freed below
+        drop_tmp();
+    } else {
+        brow_fill_kernel<<<nb, PAT_WARPS * 32, smem_fill, st>>>(N, nullptr, nullptr, ctx->d_inc_ptr, ctx->d_inc_q,
+                                                                ctx->d_support, ctx->k, ctx->d_brow_ptr, ctx->d_bcol,
+                                                                ctx->d_bdiag);
+        KERNEL_CHECK(ctx);
+    }
     return RPIM_OK;
 }
 

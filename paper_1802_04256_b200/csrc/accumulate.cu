@@ -30,10 +30,18 @@ __device__ __forceinline__ void group_sync(int rg) {
 
 constexpr int ilog2_ce(int v) { return v <= 1 ? 0 : 1 + ilog2_ce(v >> 1); }
 
-constexpr int RED_NB = 32;   // incident points per batch
+constexpr int RED_NB = 32;   // incident points per batch (one per lane in the preparation phase)
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <int NWARP, int CPW>
-struct RedSmem {
+struct alignas(16) RedSmem {
     static constexpr int NW = NWARP * CPW;
     static constexpr int P2 = 1 << ilog2_ce(32 * NW - 1 + (32 * NW));   // power of two >= 32 NW
     int cols[P2];                       // sorted block columns of the row, padded with INT_MAX
@@ -44,28 +52,39 @@ struct RedSmem {
     double fpart[NWARP];
 };
 
+// Dynamic shared memory of one row group: RedSmem followed by the double-buffered gradient
+// staging area G[2][nbg][k][4] (copied with cp.async straight from the staged shape functions).
+__host__ __device__ inline size_t red_group_bytes(size_t head, int k, int nbg) {
+    return head + (size_t)2 * nbg * k * 4 * sizeof(double);
+}
+
 // NWARP warps own one block row, each CPW chunks of 32 column slots (chunk c = cc * NWARP + wg);
 // a CTA holds ROWS such groups working on consecutive rows.
 template <int NWARP, int CPW, int ROWS>
 __global__ void __launch_bounds__(NWARP * ROWS * 32)
-reduce_rows_kernel(int64_t N, int k, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
+reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
                    const uint8_t* __restrict__ inc_j, const int32_t* __restrict__ support,
                    const double* __restrict__ stage, const double* __restrict__ qw,
                    const int64_t* __restrict__ brow_ptr, const int32_t* __restrict__ bcol, double lambda, double mu,
                    double bx, double by, double bz, double* __restrict__ vals, double* __restrict__ f) {
     using S = RedSmem<NWARP, CPW>;
-    constexpr int NW = S::NW, P2 = S::P2;
+    constexpr int NW = S::NW, P2 = S::P2, GT = NWARP * 32;
     extern __shared__ __align__(16) unsigned char red_smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int rg = warp / NWARP, wg = warp % NWARP;
-    S& sm = reinterpret_cast<S*>(red_smem_raw)[rg];
+    const int rg = warp / NWARP, wg = warp % NWARP, tg = wg * 32 + lane;
+    unsigned char* gbase = red_smem_raw + (size_t)rg * red_group_bytes(sizeof(S), k, nbg);
+    S& sm = *reinterpret_cast<S*>(gbase);
+    double* G = reinterpret_cast<double*>(gbase + sizeof(S));
+    const int gstride = nbg * k * 4;   // doubles per staging buffer
+    const int row2 = 2 * k;            // 16-byte chunks per point
     const unsigned lt = (1u << lane) - 1u;
+    const int npass = (k + 31) >> 5;
 
     for (int64_t I = (int64_t)blockIdx.x * ROWS + rg; I < N; I += (int64_t)gridDim.x * ROWS) {
         const int64_t o = brow_ptr[I];
         const int L = (int)(brow_ptr[I + 1] - o);
         group_sync<NWARP>(rg);   // the previous row's shared data is dead
-        for (int s = wg * 32 + lane; s < P2; s += NWARP * 32) sm.cols[s] = (s < L) ? bcol[o + s] : 0x7FFFFFFF;
+        for (int s = tg; s < P2; s += GT) sm.cols[s] = (s < L) ? bcol[o + s] : 0x7FFFFFFF;
         double acc[CPW][9];
 #pragma unroll
         for (int cc = 0; cc < CPW; ++cc)
@@ -75,8 +94,8 @@ reduce_rows_kernel(int64_t N, int k, const int64_t* __restrict__ inc_ptr, const 
         const int64_t pa = inc_ptr[I], pb = inc_ptr[I + 1];
         for (int64_t p0 = pa; p0 < pb; p0 += RED_NB) {
             const int nb = (int)min((int64_t)RED_NB, pb - p0);
-            group_sync<NWARP>(rg);   // cols visible; the previous batch has been consumed
-            // ---- phase 1: this warp prepares points b = wg, wg + NWARP, ... (lane t holds b = wg + NWARP t)
+            const int nsub = (nb + nbg - 1) / nbg;
+            // ---- phase 1a: this warp prepares points b = wg, wg + NWARP, ... (lane t holds b = wg + NWARP t)
             const int nmine = (nb - wg + NWARP - 1) / NWARP;
             int qmine = 0;
             {
@@ -94,61 +113,91 @@ reduce_rows_kernel(int64_t N, int k, const int64_t* __restrict__ inc_ptr, const 
                     sm.qbase[bm] = base;
                 }
             }
-            for (int t = 0; t < nmine; ++t) {
-                const int b = wg + NWARP * t;
-                const int q = __shfl_sync(FULLMASK, qmine, t);
-                const int32_t* sp = support + (int64_t)q * k;
+            group_sync<NWARP>(rg);   // cols and qbase visible
+            // gradient rows of sub-batch sb -> staging buffer sb & 1 (asynchronous)
+            auto issue = [&](int sb) {
+                const int b0 = sb * nbg, cnt = min(nbg, nb - b0);
+                double* dstb = G + (sb & 1) * gstride;
+                for (int e = tg; e < cnt * row2; e += GT) {
+                    const int bb = e / row2, ch = e - bb * row2;
+                    cp_async16(dstb + (bb * k) * 4 + 2 * ch, sm.qbase[b0 + bb] + 2 * ch);
+                }
+                cp_async_commit();
+            };
+            issue(0);
+            // ---- phase 1b: slot masks of this warp's points (overlaps the copies in flight)
+            {
+                const int nitems = nmine * npass;
+                auto loadJ = [&](int item) {
+                    const int t = item / npass, j = (item - t * npass) * 32 + lane;
+                    const int q = __shfl_sync(FULLMASK, qmine, t);
+                    return (j < k) ? support[(int64_t)q * k + j] : -1;
+                };
+                int Jnext = (nitems > 0) ? loadJ(0) : -1;
                 unsigned mword = 0;   // lane w ends up with mask word w
-                for (int j0 = 0; j0 < k; j0 += 32) {
-                    const int j = j0 + lane;
+                for (int item = 0; item < nitems; ++item) {
+                    const int J = Jnext;
+                    if (item + 1 < nitems) Jnext = loadJ(item + 1);
+                    const int t = item / npass, ps = item - t * npass;
+                    if (ps == 0) mword = 0;
                     int slot = -1;
-                    if (j < k) {
-                        const int J = sp[j];
+                    if (J >= 0) {
                         int lo = 0;   // last index with cols[index] <= J; J is always present in the row
 #pragma unroll
                         for (int step = P2 / 2; step > 0; step >>= 1)
                             if (sm.cols[lo + step] <= J) lo += step;
                         slot = lo;
                     }
+                    const int nact = min(32, k - ps * 32);
                     const int wfirst = __shfl_sync(FULLMASK, slot, 0) >> 5;
-                    const int nact = min(32, k - j0);
                     const int wlast = __shfl_sync(FULLMASK, slot, nact - 1) >> 5;
                     const unsigned bit = (slot >= 0) ? (1u << (slot & 31)) : 0u;
                     for (int w = wfirst; w <= wlast; ++w) {
                         const unsigned m = __reduce_or_sync(FULLMASK, ((slot >> 5) == w) ? bit : 0u);
                         if (lane == w) mword |= m;
                     }
-                }
-                // exclusive prefix of the popcounts over the words (NW <= 32 words: one per lane)
-                const int cnt = __popc(mword);
-                int incl = cnt;
+                    if (ps == npass - 1) {
+                        // exclusive prefix of the popcounts over the words (NW <= 32 words: one per lane)
+                        const int cnt = __popc(mword);
+                        int incl = cnt;
 #pragma unroll
-                for (int d = 1; d < NW; d <<= 1) {
-                    const int up = __shfl_up_sync(FULLMASK, incl, d);
-                    if (lane >= d) incl += up;
-                }
-                if (lane < NW) { sm.mask[b][lane] = mword; sm.pre[b][lane] = (unsigned char)(incl - cnt); }
-            }
-            group_sync<NWARP>(rg);
-            // ---- phase 2: every lane accumulates its slots over the points of the batch
-            for (int b = 0; b < nb; ++b) {
-                const double ax = sm.a[b][0], ay = sm.a[b][1], az = sm.a[b][2];
-                const double* base = sm.qbase[b];
-#pragma unroll
-                for (int cc = 0; cc < CPW; ++cc) {
-                    const int c = cc * NWARP + wg;
-                    const unsigned word = sm.mask[b][c];
-                    if (word == 0u) continue;
-                    if ((word >> lane) & 1u) {
-                        const int pos = sm.pre[b][c] + __popc(word & lt);
-                        const double* g = base + 4 * pos;
-                        const double gx = g[1];
-                        const double2 gyz = *reinterpret_cast<const double2*>(g + 2);
-                        acc[cc][0] = fma(ax, gx, acc[cc][0]); acc[cc][1] = fma(ax, gyz.x, acc[cc][1]); acc[cc][2] = fma(ax, gyz.y, acc[cc][2]);
-                        acc[cc][3] = fma(ay, gx, acc[cc][3]); acc[cc][4] = fma(ay, gyz.x, acc[cc][4]); acc[cc][5] = fma(ay, gyz.y, acc[cc][5]);
-                        acc[cc][6] = fma(az, gx, acc[cc][6]); acc[cc][7] = fma(az, gyz.x, acc[cc][7]); acc[cc][8] = fma(az, gyz.y, acc[cc][8]);
+                        for (int d = 1; d < NW; d <<= 1) {
+                            const int up = __shfl_up_sync(FULLMASK, incl, d);
+                            if (lane >= d) incl += up;
+                        }
+                        const int b = wg + NWARP * t;
+                        if (lane < NW) { sm.mask[b][lane] = mword; sm.pre[b][lane] = (unsigned char)(incl - cnt); }
                     }
                 }
+            }
+            // ---- phase 2: every lane accumulates its slots over the points, sub-batch by sub-batch
+            for (int sb = 0; sb < nsub; ++sb) {
+                if (sb + 1 < nsub) { issue(sb + 1); cp_async_wait<1>(); }
+                else cp_async_wait<0>();
+                group_sync<NWARP>(rg);   // sub-batch sb has landed for every thread (and the masks are visible)
+                const int b0 = sb * nbg, cnt = min(nbg, nb - b0);
+                const double* Gb = G + (sb & 1) * gstride;
+                for (int bb = 0; bb < cnt; ++bb) {
+                    const int b = b0 + bb;
+                    const double ax = sm.a[b][0], ay = sm.a[b][1], az = sm.a[b][2];
+                    const double* base = Gb + bb * k * 4;
+#pragma unroll
+                    for (int cc = 0; cc < CPW; ++cc) {
+                        const int c = cc * NWARP + wg;
+                        const unsigned word = sm.mask[b][c];
+                        if (word == 0u) continue;
+                        if ((word >> lane) & 1u) {
+                            const int pos = sm.pre[b][c] + __popc(word & lt);
+                            const double2 g01 = *reinterpret_cast<const double2*>(base + 4 * pos);
+                            const double2 gyz = *reinterpret_cast<const double2*>(base + 4 * pos + 2);
+                            const double gx = g01.y;
+                            acc[cc][0] = fma(ax, gx, acc[cc][0]); acc[cc][1] = fma(ax, gyz.x, acc[cc][1]); acc[cc][2] = fma(ax, gyz.y, acc[cc][2]);
+                            acc[cc][3] = fma(ay, gx, acc[cc][3]); acc[cc][4] = fma(ay, gyz.x, acc[cc][4]); acc[cc][5] = fma(ay, gyz.y, acc[cc][5]);
+                            acc[cc][6] = fma(az, gx, acc[cc][6]); acc[cc][7] = fma(az, gyz.x, acc[cc][7]); acc[cc][8] = fma(az, gyz.y, acc[cc][8]);
+                        }
+                    }
+                }
+                group_sync<NWARP>(rg);   // buffer sb & 1 may be refilled
             }
         }
         // ---- K_IJ = lambda S + mu S^T + mu tr(S) I, three scalar rows per block row
@@ -352,7 +401,9 @@ template <int NWARP, int CPW, int ROWS>
 int launch_reduce_rows(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
                        double* d_vals, double* d_f) {
     auto kern = reduce_rows_kernel<NWARP, CPW, ROWS>;
-    const size_t smem = sizeof(RedSmem<NWARP, CPW>) * ROWS;
+    // gradient staging: two buffers of nbg points each, about 16 KB per row group
+    const int nbg = std::max(2, std::min(8, 8192 / (ctx->k * 32)));
+    const size_t smem = red_group_bytes(sizeof(RedSmem<NWARP, CPW>), ctx->k, nbg) * ROWS;
     CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 1;
     CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NWARP * ROWS * 32, smem));
@@ -362,7 +413,7 @@ int launch_reduce_rows(rpim_ctx* ctx, const double* d_qw, double lambda, double 
     int64_t blocks = (ctx->N + ROWS - 1) / ROWS;
     blocks = std::min<int64_t>(blocks, (int64_t)sms * per_sm * 8);   // several waves: boundary rows are cheaper
     kern<<<(unsigned)blocks, NWARP * ROWS * 32, smem, ctx->stream>>>(
-        ctx->N, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_support, ctx->d_stage, d_qw,
+        ctx->N, ctx->k, nbg, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_support, ctx->d_stage, d_qw,
         ctx->d_brow_ptr, ctx->d_bcol, lambda, mu, body[0], body[1], body[2], d_vals, d_f);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
@@ -372,7 +423,7 @@ int launch_reduce_rows(rpim_ctx* ctx, const double* d_qw, double lambda, double 
 int rpim_stage_accumulate(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
                           double* d_vals, double* d_f) {
     const int Lmax = std::max(ctx->max_blen, 1);
-    static_assert(sizeof(RedSmem<1, 4>) % 8 == 0 && sizeof(RedSmem<8, 4>) % 8 == 0, "group stride keeps 8-byte alignment");
+    static_assert(sizeof(RedSmem<1, 4>) % 16 == 0 && sizeof(RedSmem<8, 4>) % 16 == 0, "group stride keeps 16-byte alignment");
     if (Lmax <= 128) return launch_reduce_rows<1, 4, 8>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
     if (Lmax <= 192) return launch_reduce_rows<2, 3, 4>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
     if (Lmax <= 256) return launch_reduce_rows<2, 4, 4>(ctx, d_qw, lambda, mu, body, d_vals, d_f);

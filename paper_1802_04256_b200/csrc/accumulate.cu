@@ -9,12 +9,13 @@
 // K_IJ = lambda S + mu S^T + mu tr(S) I is applied once per block at write-out.
 //
 // reduce_rows_kernel (rows of up to 1024 block columns): the accumulators live in REGISTERS.
-// Lane l of chunk c owns column slot 32 c + l of the row.  For a batch of incident points the
-// group first builds, per point, the bit mask of the row's slots that the point's support hits
-// (binary search of the sorted support in the sorted column list) with the running popcount per
-// 32-slot word; then every lane whose bit is set finds its node's position in the support as
-// prefix + popc(bits below), gathers that node's gradient (one 32-byte sector of the staged
-// [q][j][phi gx gy gz] array) and does nine fused multiply-adds.
+// Lane l of chunk c owns column slot 32 c + l of the row.  Per row the group builds an
+// open-addressing table column node -> slot in shared memory.  For a batch of incident points
+// it then fills a byte table pos[point][slot] = position of the slot's node in the point's
+// support (one table probe per support node), while one thread bulk-copies (cp.async.bulk + mbarrier)
+// the points' staged [k][phi gx gy gz] rows into a double-buffered staging area.  In the
+// accumulation phase every lane reads its byte, and if the point hits its slot gathers that
+// node's gradient (one 32-byte sector) from the staging area and does nine fused multiply-adds.
 // accumulate_generic_kernel: fallback for longer rows, accumulators in shared memory.
 #include "common.cuh"
 
@@ -30,30 +31,47 @@ __device__ __forceinline__ void group_sync(int rg) {
 
 constexpr int ilog2_ce(int v) { return v <= 1 ? 0 : 1 + ilog2_ce(v >> 1); }
 
-constexpr int RED_NB = 32;   // incident points per batch (one per lane in the preparation phase)
+constexpr int RED_NB = 32;   // incident points per batch
 
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+// ---- mbarrier / bulk-copy (TMA, non-tensor) helpers: one elected thread moves a whole point's
+// staged [k][phi gx gy gz] row (k * 32 bytes, contiguous) into shared memory with one instruction.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    unsigned ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
 
 template <int NWARP, int CPW>
 struct alignas(16) RedSmem {
-    static constexpr int NW = NWARP * CPW;
-    static constexpr int P2 = 1 << ilog2_ce(32 * NW - 1 + (32 * NW));   // power of two >= 32 NW
-    int cols[P2];                       // sorted block columns of the row, padded with INT_MAX
-    unsigned mask[RED_NB][NW];          // slots of the row hit by the support of point b
-    unsigned char pre[RED_NB][NW];      // support positions before word w
-    double a[RED_NB][3];                // w * grad phi_I at point b
+    static constexpr int NW = NWARP * CPW;                 // 32-slot chunks of the row
+    static constexpr int NS = 32 * NW;                     // column slots
+    static constexpr int HLOG = ilog2_ce(4 * NS - 1);
+    static constexpr int HSZ = 1 << HLOG;                  // open-addressing table: 2..4 x the row length
+    unsigned long long hent[HSZ];       // (column node id << 32) | slot, ~0 = empty
+    unsigned char pos[RED_NB][NS];      // position of slot's node in the support of point b, 0xFF = absent
+    double a[RED_NB][4];                // w * grad phi_I at point b (+ pad)
     const double* qbase[RED_NB];        // staged shape functions of point b
+    unsigned cmask[RED_NB];             // chunks of the row hit by point b
+    unsigned long long full[2];         // mbarriers of the two staging buffers
     double fpart[NWARP];
 };
 
 // Dynamic shared memory of one row group: RedSmem followed by the double-buffered gradient
-// staging area G[2][nbg][k][4] (copied with cp.async straight from the staged shape functions).
+// staging area G[2][nbg][k][4] (bulk-copied straight from the staged shape functions).
 __host__ __device__ inline size_t red_group_bytes(size_t head, int k, int nbg) {
     return head + (size_t)2 * nbg * k * 4 * sizeof(double);
 }
@@ -68,23 +86,34 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                    const int64_t* __restrict__ brow_ptr, const int32_t* __restrict__ bcol, double lambda, double mu,
                    double bx, double by, double bz, double* __restrict__ vals, double* __restrict__ f) {
     using S = RedSmem<NWARP, CPW>;
-    constexpr int NW = S::NW, P2 = S::P2, GT = NWARP * 32;
+    constexpr int NS = S::NS, HSZ = S::HSZ, GT = NWARP * 32;
+    constexpr int HSHIFT = 32 - S::HLOG;
     extern __shared__ __align__(16) unsigned char red_smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int rg = warp / NWARP, wg = warp % NWARP, tg = wg * 32 + lane;
     unsigned char* gbase = red_smem_raw + (size_t)rg * red_group_bytes(sizeof(S), k, nbg);
     S& sm = *reinterpret_cast<S*>(gbase);
     double* G = reinterpret_cast<double*>(gbase + sizeof(S));
-    const int gstride = nbg * k * 4;   // doubles per staging buffer
-    const int row2 = 2 * k;            // 16-byte chunks per point
-    const unsigned lt = (1u << lane) - 1u;
+    const int gstride = nbg * k * 4;            // doubles per staging buffer
+    const unsigned pbytes = (unsigned)k * 32u;  // bytes of one point's staged row
     const int npass = (k + 31) >> 5;
+    if (tg == 0) { mbar_init(&sm.full[0], 1); mbar_init(&sm.full[1], 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    unsigned ph0 = 0, ph1 = 0;   // parity of the next completion of each staging buffer
+    __syncthreads();
 
     for (int64_t I = (int64_t)blockIdx.x * ROWS + rg; I < N; I += (int64_t)gridDim.x * ROWS) {
         const int64_t o = brow_ptr[I];
         const int L = (int)(brow_ptr[I + 1] - o);
         group_sync<NWARP>(rg);   // the previous row's shared data is dead
-        for (int s = tg; s < P2; s += GT) sm.cols[s] = (s < L) ? bcol[o + s] : 0x7FFFFFFF;
+        for (int s = tg; s < HSZ; s += GT) sm.hent[s] = ~0ull;
+        group_sync<NWARP>(rg);
+        for (int s = tg; s < L; s += GT) {
+            const unsigned J = (unsigned)bcol[o + s];
+            unsigned h = (J * 2654435761u) >> HSHIFT;
+            const unsigned long long ent = ((unsigned long long)J << 32) | (unsigned)s;
+            while (atomicCAS(&sm.hent[h], ~0ull, ent) != ~0ull) h = (h + 1) & (HSZ - 1);
+        }
         double acc[CPW][9];
 #pragma unroll
         for (int cc = 0; cc < CPW; ++cc)
@@ -95,101 +124,77 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
         for (int64_t p0 = pa; p0 < pb; p0 += RED_NB) {
             const int nb = (int)min((int64_t)RED_NB, pb - p0);
             const int nsub = (nb + nbg - 1) / nbg;
-            // ---- phase 1a: this warp prepares points b = wg, wg + NWARP, ... (lane t holds b = wg + NWARP t)
-            const int nmine = (nb - wg + NWARP - 1) / NWARP;
-            int qmine = 0;
-            {
-                const int bm = wg + NWARP * lane;
-                if (lane < nmine) {
-                    const int64_t p = p0 + bm;
-                    qmine = inc_q[p];
-                    const int i = inc_j[p];
-                    const double w = qw[qmine];
-                    const double* base = stage + (int64_t)qmine * k * 4;
-                    const double2 v01 = *reinterpret_cast<const double2*>(base + 4 * i);
-                    const double2 v23 = *reinterpret_cast<const double2*>(base + 4 * i + 2);
-                    fsum += w * v01.x;
-                    sm.a[bm][0] = w * v01.y; sm.a[bm][1] = w * v23.x; sm.a[bm][2] = w * v23.y;
-                    sm.qbase[bm] = base;
-                }
+            group_sync<NWARP>(rg);   // previous batch fully consumed (pos, a, staging buffers); hash table complete
+            // ---- phase 1a: per-point scalars (thread b of the group) and a clean position table
+            if (tg < nb) {
+                const int64_t p = p0 + tg;
+                const int q = inc_q[p];
+                const int i = inc_j[p];
+                const double w = qw[q];
+                const double* base = stage + (int64_t)q * k * 4;
+                const double2 v01 = *reinterpret_cast<const double2*>(base + 4 * i);
+                const double2 v23 = *reinterpret_cast<const double2*>(base + 4 * i + 2);
+                fsum += w * v01.x;
+                sm.a[tg][0] = w * v01.y; sm.a[tg][1] = w * v23.x; sm.a[tg][2] = w * v23.y;
+                sm.qbase[tg] = base;
             }
-            group_sync<NWARP>(rg);   // cols and qbase visible
-            // gradient rows of sub-batch sb -> staging buffer sb & 1 (asynchronous)
+            {
+                uint4* pz = reinterpret_cast<uint4*>(&sm.pos[0][0]);
+                const uint4 ff = make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu);
+                for (int e = tg; e < nb * (NS / 16); e += GT) pz[e] = ff;
+            }
+            group_sync<NWARP>(rg);   // qbase visible, table clean
+            // gradient rows of sub-batch sb -> staging buffer sb & 1 (bulk copies issued by one thread)
             auto issue = [&](int sb) {
                 const int b0 = sb * nbg, cnt = min(nbg, nb - b0);
+                unsigned long long* bar = &sm.full[sb & 1];
+                mbar_expect_tx(bar, (unsigned)cnt * pbytes);
                 double* dstb = G + (sb & 1) * gstride;
-                for (int e = tg; e < cnt * row2; e += GT) {
-                    const int bb = e / row2, ch = e - bb * row2;
-                    cp_async16(dstb + (bb * k) * 4 + 2 * ch, sm.qbase[b0 + bb] + 2 * ch);
-                }
-                cp_async_commit();
+                for (int bb = 0; bb < cnt; ++bb) bulk_g2s(dstb + bb * k * 4, sm.qbase[b0 + bb], pbytes, bar);
             };
-            issue(0);
-            // ---- phase 1b: slot masks of this warp's points (overlaps the copies in flight)
-            {
-                const int nitems = nmine * npass;
-                auto loadJ = [&](int item) {
-                    const int t = item / npass, j = (item - t * npass) * 32 + lane;
-                    const int q = __shfl_sync(FULLMASK, qmine, t);
-                    return (j < k) ? support[(int64_t)q * k + j] : -1;
-                };
-                int Jnext = (nitems > 0) ? loadJ(0) : -1;
-                unsigned mword = 0;   // lane w ends up with mask word w
-                for (int item = 0; item < nitems; ++item) {
-                    const int J = Jnext;
-                    if (item + 1 < nitems) Jnext = loadJ(item + 1);
-                    const int t = item / npass, ps = item - t * npass;
-                    if (ps == 0) mword = 0;
-                    int slot = -1;
-                    if (J >= 0) {
-                        int lo = 0;   // last index with cols[index] <= J; J is always present in the row
-#pragma unroll
-                        for (int step = P2 / 2; step > 0; step >>= 1)
-                            if (sm.cols[lo + step] <= J) lo += step;
-                        slot = lo;
+            if (tg == 0) { issue(0); if (nsub > 1) issue(1); }
+            // ---- phase 1b: positions of this warp's points b = wg, wg + NWARP, ... (overlaps the copies)
+            for (int b = wg; b < nb; b += NWARP) {
+                const int32_t* sp = support + (sm.qbase[b] - stage) / 4;   // = support + q * k
+                unsigned cm = 0;
+                for (int ps = 0; ps < npass; ++ps) {
+                    const int j = ps * 32 + lane;
+                    unsigned wbit = 0;
+                    if (j < k) {
+                        const unsigned J = (unsigned)sp[j];
+                        unsigned h = (J * 2654435761u) >> HSHIFT;
+                        unsigned long long ent = sm.hent[h];
+                        while ((unsigned)(ent >> 32) != J) { h = (h + 1) & (HSZ - 1); ent = sm.hent[h]; }
+                        const unsigned slot = (unsigned)ent;
+                        sm.pos[b][slot] = (unsigned char)j;
+                        wbit = 1u << (slot >> 5);
                     }
-                    const int nact = min(32, k - ps * 32);
-                    const int wfirst = __shfl_sync(FULLMASK, slot, 0) >> 5;
-                    const int wlast = __shfl_sync(FULLMASK, slot, nact - 1) >> 5;
-                    const unsigned bit = (slot >= 0) ? (1u << (slot & 31)) : 0u;
-                    for (int w = wfirst; w <= wlast; ++w) {
-                        const unsigned m = __reduce_or_sync(FULLMASK, ((slot >> 5) == w) ? bit : 0u);
-                        if (lane == w) mword |= m;
-                    }
-                    if (ps == npass - 1) {
-                        // exclusive prefix of the popcounts over the words (NW <= 32 words: one per lane)
-                        const int cnt = __popc(mword);
-                        int incl = cnt;
-#pragma unroll
-                        for (int d = 1; d < NW; d <<= 1) {
-                            const int up = __shfl_up_sync(FULLMASK, incl, d);
-                            if (lane >= d) incl += up;
-                        }
-                        const int b = wg + NWARP * t;
-                        if (lane < NW) { sm.mask[b][lane] = mword; sm.pre[b][lane] = (unsigned char)(incl - cnt); }
-                    }
+                    cm |= __reduce_or_sync(FULLMASK, wbit);
                 }
+                if (lane == 0) sm.cmask[b] = cm;
             }
             // ---- phase 2: every lane accumulates its slots over the points, sub-batch by sub-batch
             for (int sb = 0; sb < nsub; ++sb) {
-                if (sb + 1 < nsub) { issue(sb + 1); cp_async_wait<1>(); }
-                else cp_async_wait<0>();
-                group_sync<NWARP>(rg);   // sub-batch sb has landed for every thread (and the masks are visible)
+                group_sync<NWARP>(rg);   // positions visible (sb = 0); buffer (sb + 1) & 1 fully consumed (sb > 0)
+                if (sb > 0 && sb + 1 < nsub && tg == 0) issue(sb + 1);
+                if (sb & 1) { mbar_wait(&sm.full[1], ph1); ph1 ^= 1u; }
+                else { mbar_wait(&sm.full[0], ph0); ph0 ^= 1u; }
                 const int b0 = sb * nbg, cnt = min(nbg, nb - b0);
                 const double* Gb = G + (sb & 1) * gstride;
                 for (int bb = 0; bb < cnt; ++bb) {
                     const int b = b0 + bb;
+                    const unsigned cm = sm.cmask[b];
                     const double ax = sm.a[b][0], ay = sm.a[b][1], az = sm.a[b][2];
                     const double* base = Gb + bb * k * 4;
+                    const unsigned char* prow = &sm.pos[b][lane];
 #pragma unroll
                     for (int cc = 0; cc < CPW; ++cc) {
                         const int c = cc * NWARP + wg;
-                        const unsigned word = sm.mask[b][c];
-                        if (word == 0u) continue;
-                        if ((word >> lane) & 1u) {
-                            const int pos = sm.pre[b][c] + __popc(word & lt);
-                            const double2 g01 = *reinterpret_cast<const double2*>(base + 4 * pos);
-                            const double2 gyz = *reinterpret_cast<const double2*>(base + 4 * pos + 2);
+                        if (!((cm >> c) & 1u)) continue;
+                        const unsigned j = prow[32 * c];
+                        if (j != 0xFFu) {
+                            const double2 g01 = *reinterpret_cast<const double2*>(base + 4 * j);
+                            const double2 gyz = *reinterpret_cast<const double2*>(base + 4 * j + 2);
                             const double gx = g01.y;
                             acc[cc][0] = fma(ax, gx, acc[cc][0]); acc[cc][1] = fma(ax, gyz.x, acc[cc][1]); acc[cc][2] = fma(ax, gyz.y, acc[cc][2]);
                             acc[cc][3] = fma(ay, gx, acc[cc][3]); acc[cc][4] = fma(ay, gyz.x, acc[cc][4]); acc[cc][5] = fma(ay, gyz.y, acc[cc][5]);
@@ -197,7 +202,6 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                         }
                     }
                 }
-                group_sync<NWARP>(rg);   // buffer sb & 1 may be refilled
             }
         }
         // ---- K_IJ = lambda S + mu S^T + mu tr(S) I, three scalar rows per block row

@@ -32,6 +32,7 @@ void free_all(rpim_ctx* c) {
     ws_free(c, &c->d_stage); ws_free(c, &c->d_singular); ws_free(c, &c->d_scratch);
     ws_free(c, &c->h2d_nodes); ws_free(c, &c->h2d_qpts);
     { int64_t* t = (int64_t*)c->d_scan_tmp; ws_free(c, &t); c->d_scan_tmp = nullptr; c->scan_tmp_elems = 0; }
+    ws_release_cache(c);
     c->have_pattern = c->have_shape = false;
 }
 

@@ -42,7 +42,8 @@ struct rpim_ctx {
     std::string err;
     int64_t launches = 0;
     int64_t ws_bytes = 0;
-    std::unordered_map<void*, int64_t> ws_sizes;
+    std::unordered_map<void*, int64_t> ws_sizes;          // live blocks -> capacity in bytes
+    std::vector<std::pair<void*, int64_t>> ws_cache;      // parked blocks (freed, reusable)
 
     // problem
     const double* d_nodes = nullptr;
@@ -125,28 +126,62 @@ struct rpim_ctx {
                       cudaGetErrorString(_e), __FILE__, __LINE__);                              \
     } while (0)
 
+// Workspace allocator with a per-context cache: a freed block is parked and handed out again to
+// the next request it fits (capacity within 2x of the request), so that repeated
+// rpim_build_pattern / rpim_assemble calls on same-sized problems never reach cudaMalloc/cudaFree
+// (both synchronise the device).  ws_release_cache really frees the parked blocks.
+inline void ws_release_cache(rpim_ctx* ctx) {
+    for (auto& b : ctx->ws_cache) { cudaFree(b.first); ctx->ws_bytes -= b.second; }
+    ctx->ws_cache.clear();
+}
 template <typename T>
 void ws_free(rpim_ctx* ctx, T** p) {
     if (*p) {
         auto it = ctx->ws_sizes.find((void*)*p);
-        if (it != ctx->ws_sizes.end()) { ctx->ws_bytes -= it->second; ctx->ws_sizes.erase(it); }
-        cudaFree(*p);
+        if (it != ctx->ws_sizes.end()) {
+            ctx->ws_cache.emplace_back((void*)*p, it->second);
+            ctx->ws_sizes.erase(it);
+        } else {
+            cudaFree(*p);
+        }
     }
     *p = nullptr;
 }
 template <typename T>
 int ws_alloc(rpim_ctx* ctx, T** p, int64_t count) {
-    ws_free(ctx, p);
     if (count <= 0) count = 1;
-    cudaError_t e = cudaMalloc((void**)p, (size_t)count * sizeof(T));
+    const int64_t need = count * (int64_t)sizeof(T);
+    if (*p) {   // already large enough (and not wastefully so): keep it
+        auto it = ctx->ws_sizes.find((void*)*p);
+        if (it != ctx->ws_sizes.end() && it->second >= need && it->second <= 2 * need + 4096) return RPIM_OK;
+    }
+    ws_free(ctx, p);
+    int best = -1;
+    for (int i = 0; i < (int)ctx->ws_cache.size(); ++i) {
+        const int64_t cap = ctx->ws_cache[i].second;
+        if (cap >= need && cap <= 2 * need + 4096 && (best < 0 || cap < ctx->ws_cache[best].second)) best = i;
+    }
+    if (best >= 0) {
+        *p = (T*)ctx->ws_cache[best].first;
+        ctx->ws_sizes[(void*)*p] = ctx->ws_cache[best].second;
+        ctx->ws_cache.erase(ctx->ws_cache.begin() + best);
+        return RPIM_OK;
+    }
+    cudaError_t e = cudaMalloc((void**)p, (size_t)need);
+    if (e != cudaSuccess) {   // give the parked blocks back to the driver and retry once
+        cudaGetLastError();
+        cudaStreamSynchronize(ctx->stream);
+        ws_release_cache(ctx);
+        e = cudaMalloc((void**)p, (size_t)need);
+    }
     if (e != cudaSuccess) {
         *p = nullptr;
         cudaGetLastError();
-        RPIM_FAIL(ctx, RPIM_ERR_ALLOC, "device allocation of %lld bytes failed: %s",
-                  (long long)(count * (int64_t)sizeof(T)), cudaGetErrorString(e));
+        RPIM_FAIL(ctx, RPIM_ERR_ALLOC, "device allocation of %lld bytes failed: %s", (long long)need,
+                  cudaGetErrorString(e));
     }
-    ctx->ws_sizes[(void*)*p] = count * (int64_t)sizeof(T);
-    ctx->ws_bytes += count * (int64_t)sizeof(T);
+    ctx->ws_sizes[(void*)*p] = need;
+    ctx->ws_bytes += need;
     return RPIM_OK;
 }
 

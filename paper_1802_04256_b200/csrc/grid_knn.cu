@@ -409,8 +409,6 @@ int rpim_stage_grid_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, in
     else if (cap == 512) rc = launch_knn<512, 8, false>(ctx, d_pts, M, k, nullptr, d_ovf, d_support, 148 * 64);
     else rc = launch_knn<1024, 4, false>(ctx, d_pts, M, k, nullptr, d_ovf, d_support, 148 * 64);
     if (rc == RPIM_OK) rc = launch_knn<KNN_CAP_MAX, 4, true>(ctx, d_pts, M, k, d_ovf, nullptr, d_support, 148 * 2);
-    // the overflow list is read by the second launch: keep it until the stream has drained
-    if (rc == RPIM_OK) { cudaError_t e = cudaStreamSynchronize(st); if (e != cudaSuccess) rc = RPIM_ERR_CUDA; }
-    ws_free(ctx, &d_ovf);
+    ws_free(ctx, &d_ovf);   // parked in the workspace cache (later reuse is ordered by the stream)
     return rc;
 }

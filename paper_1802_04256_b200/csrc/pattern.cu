@@ -25,20 +25,25 @@ __global__ void inc_fill_kernel(const int32_t* __restrict__ support, int64_t tot
 
 constexpr int INC_CAP = 4096;   // longest incidence list sorted on chip
 constexpr int INC_WARPS = 4;
+constexpr int INC_FAST_CAP = 128;   // lists up to this length take the high-occupancy launch
+constexpr int INC_FAST_WARPS = 8;
 
-// one warp per node: sort its list ascending by point id (the position byte rides along)
-__global__ void __launch_bounds__(INC_WARPS * 32)
+// one warp per node: sort its list ascending by point id (the position byte rides along).
+// Launched twice: CAP = INC_FAST_CAP handles the usual short lists with 1 KB of shared memory per
+// warp (full occupancy), CAP = INC_CAP picks up the longer ones (LO = INC_FAST_CAP).
+template <int CAP, int LO, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32)
 inc_sort_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, int32_t* __restrict__ inc_q,
                 uint8_t* __restrict__ inc_j, long long* __restrict__ flags) {
     extern __shared__ unsigned char smem_raw[];
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    unsigned long long* key = (unsigned long long*)smem_raw + (size_t)wid * INC_CAP;
-    for (int64_t I = (int64_t)blockIdx.x * INC_WARPS + wid; I < N; I += (int64_t)gridDim.x * INC_WARPS) {
+    unsigned long long* key = (unsigned long long*)smem_raw + (size_t)wid * CAP;
+    for (int64_t I = (int64_t)blockIdx.x * WARPS + wid; I < N; I += (int64_t)gridDim.x * WARPS) {
         const int64_t a = inc_ptr[I];
         const int len = (int)(inc_ptr[I + 1] - a);
-        if (len <= 1) continue;
-        if (len > INC_CAP) {
-            if (lane == 0) atomicAdd((unsigned long long*)&flags[FLAG_INC_CAP], 1ull);
+        if (len <= 1 || len <= LO) continue;
+        if (len > CAP) {
+            if (CAP == INC_CAP && lane == 0) atomicAdd((unsigned long long*)&flags[FLAG_INC_CAP], 1ull);
             continue;
         }
         const int np = next_pow2(len);
@@ -288,11 +293,19 @@ int rpim_stage_incidence(rpim_ctx* ctx) {
     inc_fill_kernel<<<nb, 256, 0, st>>>(ctx->d_support, total, ctx->k, ctx->d_inc_ptr, ctx->d_inc_count,
                                         ctx->d_inc_q, ctx->d_inc_j);
     KERNEL_CHECK(ctx);
-    const size_t smem = (size_t)INC_WARPS * INC_CAP * sizeof(unsigned long long);
-    CUDA_TRY(ctx, cudaFuncSetAttribute(inc_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    inc_sort_kernel<<<(unsigned)std::min<int64_t>((N + INC_WARPS - 1) / INC_WARPS, 148 * 16), INC_WARPS * 32, smem,
-                      st>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_flags);
-    KERNEL_CHECK(ctx);
+    {
+        auto fast = inc_sort_kernel<INC_FAST_CAP, 0, INC_FAST_WARPS>;
+        const size_t smem_f = (size_t)INC_FAST_WARPS * INC_FAST_CAP * sizeof(unsigned long long);
+        fast<<<(unsigned)std::min<int64_t>((N + INC_FAST_WARPS - 1) / INC_FAST_WARPS, 148 * 64), INC_FAST_WARPS * 32,
+               smem_f, st>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_flags);
+        KERNEL_CHECK(ctx);
+        auto slow = inc_sort_kernel<INC_CAP, INC_FAST_CAP, INC_WARPS>;
+        const size_t smem = (size_t)INC_WARPS * INC_CAP * sizeof(unsigned long long);
+        CUDA_TRY(ctx, cudaFuncSetAttribute(slow, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        slow<<<(unsigned)std::min<int64_t>((N + INC_WARPS - 1) / INC_WARPS, 148), INC_WARPS * 32, smem, st>>>(
+            N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_flags);
+        KERNEL_CHECK(ctx);
+    }
     CUDA_TRY(ctx, cudaMemcpyAsync(&ctx->max_inc, d_max, sizeof(int), cudaMemcpyDeviceToHost, st));
     return RPIM_OK;
 }
@@ -391,8 +404,7 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
                                                                         ctx->d_brow_ptr, ctx->d_bcol, ctx->d_bdiag);
             KERNEL_CHECK(ctx);
         }
-        CUDA_TRY(ctx, cudaStreamSynchronize(st));   // the pool is freed below
-        drop_tmp();
+        drop_tmp();   // parked in the workspace cache: reused in stream order, no synchronisation needed
     } else {
         brow_fill_kernel<<<nb, PAT_WARPS * 32, smem_fill, st>>>(N, nullptr, nullptr, ctx->d_inc_ptr, ctx->d_inc_q,
                                                                 ctx->d_support, ctx->k, ctx->d_brow_ptr, ctx->d_bcol,

@@ -17,6 +17,7 @@
 // accumulation phase every lane reads its byte, and if the point hits its slot gathers that
 // node's gradient (one 32-byte sector) from the staging area and does nine fused multiply-adds.
 // accumulate_generic_kernel: fallback for longer rows, accumulators in shared memory.
+#include "bulk_copy.cuh"
 #include "common.cuh"
 
 namespace {
@@ -32,28 +33,6 @@ __device__ __forceinline__ void group_sync(int rg) {
 constexpr int ilog2_ce(int v) { return v <= 1 ? 0 : 1 + ilog2_ce(v >> 1); }
 
 constexpr int RED_NB = 32;   // incident points per batch
-
-// ---- mbarrier / bulk-copy (TMA, non-tensor) helpers: one elected thread moves a whole point's
-// staged [k][phi gx gy gz] row (k * 32 bytes, contiguous) into shared memory with one instruction.
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
-    unsigned ok;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
 
 template <int NWARP, int CPW>
 struct alignas(16) RedSmem {

@@ -321,6 +321,229 @@ knn_kernel(GridParams g, const double* __restrict__ sx, const double* __restrict
     }
 }
 
+// ------------------------------------------------------------------ the search, fast form: candidates in registers
+// One warp per query, at most 32 * EPL candidates (EPL per lane) from at most 32 x-rows of cells.
+// Instead of sorting the candidates the warp SELECTS the k smallest under the order (d^2, node id):
+// bisection on the bit pattern of d^2 (monotone for d^2 >= 0) with a warp-wide count per step,
+// stopping as soon as exactly k candidates lie at or below the trial value; exact ties at the k-th
+// distance (regular grids, R1) are resolved by a second bisection on the node id.  Only the
+// k winners are sorted (ascending node id).  Queries that need more cells or candidates go to the
+// overflow list and are redone by knn_kernel<KNN_CAP_MAX>.  Same result, bit for bit.
+template <int EPL, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32)
+knn_select_kernel(GridParams g, const double* __restrict__ sx, const double* __restrict__ sy,
+                  const double* __restrict__ sz, const int* __restrict__ node_order,
+                  const int64_t* __restrict__ cell_start, const double* __restrict__ pts, int64_t M, int k, int R0,
+                  int32_t* __restrict__ ovf_list, int32_t* __restrict__ support, long long* __restrict__ flags) {
+    constexpr unsigned FULLW = 0xffffffffu;
+    constexpr unsigned long long KINF = 0xFFFFFFFFFFFFFFFFull;
+    __shared__ int win_s[WARPS][128];
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int* win = win_s[wid];
+    const unsigned lt = (1u << lane) - 1u;
+
+    for (int64_t q = (int64_t)blockIdx.x * WARPS + wid; q < M; q += (int64_t)gridDim.x * WARPS) {
+        const double xq = pts[3 * q], yq = pts[3 * q + 1], zq = pts[3 * q + 2];
+        int cq[3];
+        cell_coords(g, xq, yq, zq, cq);
+        int R = R0;
+        bool fail = false, overflow = false;
+        unsigned long long key[EPL];
+        int id[EPL];
+        unsigned sel = 0;   // bit e: candidate e of this lane is one of the k winners
+        while (true) {
+            int a[3], b[3];
+            bool whole = true;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                a[c] = max(cq[c] - R, 0);
+                b[c] = min(cq[c] + R, g.nc[c] - 1);
+                if (a[c] > 0 || b[c] < g.nc[c] - 1) whole = false;
+            }
+            const int ny = b[1] - a[1] + 1, nz = b[2] - a[2] + 1;
+            const int nrows = ny * nz;
+            if (nrows > 32) { overflow = true; break; }
+            // lane r: x-row r of cells (contiguous in cell order) -> first sorted node and length
+            int s0 = 0, len = 0;
+            if (lane < nrows) {
+                const int y = a[1] + lane % ny, z = a[2] + lane / ny;
+                const int64_t c0 = a[0] + (int64_t)g.nc[0] * (y + (int64_t)g.nc[1] * z);
+                const int64_t st = cell_start[c0];
+                s0 = (int)st;
+                len = (int)(cell_start[c0 + (b[0] - a[0]) + 1] - st);
+            }
+            int incl = len;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int up = __shfl_up_sync(FULLW, incl, d);
+                if (lane >= d) incl += up;
+            }
+            const int cnt = __shfl_sync(FULLW, incl, 31);
+            if (cnt < k) {
+                if (whole) { fail = true; break; }
+                ++R;
+                continue;
+            }
+            if (cnt > 32 * EPL) { overflow = true; break; }
+            const int off = incl - len;
+            // non-empty rows compacted to lanes 0..: lane c holds (first node - offset) of the c-th non-empty row
+            const unsigned nonempty = __ballot_sync(FULLW, len > 0);
+            const int src = __fns(nonempty, 0, lane + 1);
+            const int bs = __shfl_sync(FULLW, s0 - off, src & 31);
+            // candidate c = 32 e + lane: row = number of row starts at or before c, minus one
+            int pre = 0;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e) {
+                const unsigned word = __reduce_or_sync(FULLW, (len > 0 && (off >> 5) == e) ? (1u << (off & 31)) : 0u);
+                const int c = 32 * e + lane;
+                const int crow = pre + __popc(word & (lt | (1u << lane))) - 1;
+                const int p = __shfl_sync(FULLW, bs, crow & 31) + c;
+                pre += __popc(word);
+                if (c < cnt) {
+                    // R1: no fma, fixed association
+                    const double dx = __dsub_rn(sx[p], xq), dy = __dsub_rn(sy[p], yq), dz = __dsub_rn(sz[p], zq);
+                    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+                    key[e] = (unsigned long long)__double_as_longlong(d2);
+                    id[e] = node_order[p];
+                } else {
+                    key[e] = KINF;
+                    id[e] = 0x7FFFFFFF;
+                }
+            }
+            // ---- select: smallest T with count(key <= T) >= k
+            unsigned long long kmax = 0;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e)
+                if (key[e] != KINF && key[e] > kmax) kmax = key[e];
+            {
+                unsigned hi32 = __reduce_max_sync(FULLW, (unsigned)(kmax >> 32));
+                unsigned lo32 = __reduce_max_sync(FULLW, ((unsigned)(kmax >> 32) == hi32) ? (unsigned)kmax : 0u);
+                kmax = ((unsigned long long)hi32 << 32) | lo32;
+            }
+            unsigned long long lo = 0, hi = kmax, T = 0;
+            int c_le = 0;
+            bool found = false;
+            for (int it = 0; it < 24 && !found; ++it) {
+                const unsigned long long mid = lo + ((hi - lo) >> 1);
+                int c = 0;
+#pragma unroll
+                for (int e = 0; e < EPL; ++e) c += (key[e] <= mid) ? 1 : 0;
+                c = __reduce_add_sync(FULLW, c);
+                if (c == k) { T = mid; c_le = c; found = true; }
+                else if (c > k) hi = mid;
+                else lo = mid + 1;
+                if (!found && lo == hi) {
+                    T = lo; found = true;
+                    int cc = 0;
+#pragma unroll
+                    for (int e = 0; e < EPL; ++e) cc += (key[e] <= T) ? 1 : 0;
+                    c_le = __reduce_add_sync(FULLW, cc);
+                }
+            }
+            while (!found) {   // step through the distinct values left in [lo, hi]
+                unsigned long long v = KINF;
+#pragma unroll
+                for (int e = 0; e < EPL; ++e)
+                    if (key[e] >= lo && key[e] < v) v = key[e];
+                const unsigned vh = __reduce_min_sync(FULLW, (unsigned)(v >> 32));
+                const unsigned vl = __reduce_min_sync(FULLW, ((unsigned)(v >> 32) == vh) ? (unsigned)v : 0xffffffffu);
+                v = ((unsigned long long)vh << 32) | vl;
+                int c = 0;
+#pragma unroll
+                for (int e = 0; e < EPL; ++e) c += (key[e] <= v) ? 1 : 0;
+                c = __reduce_add_sync(FULLW, c);
+                if (c >= k) { T = v; c_le = c; found = true; }
+                else lo = v + 1;
+            }
+            sel = 0;
+            if (c_le == k) {
+#pragma unroll
+                for (int e = 0; e < EPL; ++e) sel |= (key[e] <= T) ? (1u << e) : 0u;
+            } else {
+                // exact ties at the k-th distance: all of key < T, and of key == T the `need` smallest ids
+                int c = 0;
+#pragma unroll
+                for (int e = 0; e < EPL; ++e) c += (key[e] < T) ? 1 : 0;
+                const int need = k - __reduce_add_sync(FULLW, c);
+                unsigned ilo = 0, ihi = 0x7FFFFFFEu, IT = 0;
+                while (true) {   // node ids are distinct: some trial value separates exactly `need` of them
+                    const unsigned mid = ilo + ((ihi - ilo) >> 1);
+                    int ci = 0;
+#pragma unroll
+                    for (int e = 0; e < EPL; ++e) ci += (key[e] == T && (unsigned)id[e] <= mid) ? 1 : 0;
+                    ci = __reduce_add_sync(FULLW, ci);
+                    if (ci == need) { IT = mid; break; }
+                    if (ci > need) ihi = mid; else ilo = mid + 1;
+                }
+#pragma unroll
+                for (int e = 0; e < EPL; ++e)
+                    sel |= (key[e] < T || (key[e] == T && (unsigned)id[e] <= IT)) ? (1u << e) : 0u;
+            }
+            if (whole) break;
+            // distance from the query to the part of space not covered by the scanned cells
+            double bound = DBL_MAX;
+            const double xyz[3] = {xq, yq, zq};
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                if (a[c] > 0) bound = fmin(bound, xyz[c] - (g.lo[c] + a[c] * g.cell));
+                if (b[c] < g.nc[c] - 1) bound = fmin(bound, (g.lo[c] + (b[c] + 1) * g.cell) - xyz[c]);
+            }
+            bound -= 1e-9 * g.cell;   // margin for rounding in the cell assignment
+            // the k-th distance = largest selected key
+            unsigned long long km = 0;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e)
+                if (((sel >> e) & 1u) && key[e] > km) km = key[e];
+            const unsigned kh = __reduce_max_sync(FULLW, (unsigned)(km >> 32));
+            const unsigned kl = __reduce_max_sync(FULLW, ((unsigned)(km >> 32) == kh) ? (unsigned)km : 0u);
+            const double dk = __longlong_as_double((long long)(((unsigned long long)kh << 32) | kl));
+            if (bound > 0.0 && dk < bound * bound) break;
+            ++R;
+        }
+        if (overflow) {
+            if (lane == 0) {
+                const unsigned long long slot = atomicAdd((unsigned long long*)&flags[FLAG_OVF_Q], 1ull);
+                ovf_list[slot] = (int32_t)q;
+            }
+            __syncwarp();
+            continue;
+        }
+        if (fail) {
+            if (lane == 0) atomicAdd((unsigned long long*)&flags[FLAG_KNN_CAP], 1ull);
+            for (int j = lane; j < k; j += 32) support[q * k + j] = 0;
+            __syncwarp();
+            continue;
+        }
+        // the k winners -> shared memory (any order), then ascending by node id
+        int base = 0;
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) {
+            const bool s = (sel >> e) & 1u;
+            const unsigned m = __ballot_sync(FULLW, s);
+            if (s) win[base + __popc(m & lt)] = id[e];
+            base += __popc(m);
+        }
+        const int kp = next_pow2(k);
+        for (int j = k + lane; j < kp; j += 32) win[j] = 0x7FFFFFFF;
+        __syncwarp();
+        warp_bitonic_i32(win, kp);
+        for (int j = lane; j < k; j += 32) support[q * k + j] = win[j];
+        __syncwarp();
+    }
+}
+
+template <int EPL, int WARPS>
+int launch_knn_select(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, int32_t* ovf_list, int32_t* d_support,
+                      int64_t blocks_cap) {
+    const int64_t N = ctx->N;
+    const int64_t blocks = std::min<int64_t>((M + WARPS - 1) / WARPS, blocks_cap);
+    knn_select_kernel<EPL, WARPS><<<(unsigned)blocks, WARPS * 32, 0, ctx->stream>>>(
+        ctx->grid, ctx->d_sorted_xyz, ctx->d_sorted_xyz + N, ctx->d_sorted_xyz + 2 * N, ctx->d_node_order,
+        ctx->d_cell_start, d_pts, M, k, 2, ovf_list, d_support, ctx->d_flags);
+    KERNEL_CHECK(ctx);
+    return RPIM_OK;
+}
+
 template <int CAP, int WARPS, bool LAST>
 int launch_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, const int32_t* qlist, int32_t* ovf_list,
                int32_t* d_support, int64_t blocks_cap) {
@@ -405,8 +628,8 @@ int rpim_stage_grid_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, in
     int32_t* d_ovf = nullptr;
     if ((rc = ws_alloc(ctx, &d_ovf, M))) return rc;
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_OVF_Q, 0, sizeof(long long), st));
-    if (cap == 256) rc = launch_knn<256, 8, false>(ctx, d_pts, M, k, nullptr, d_ovf, d_support, 148 * 64);
-    else if (cap == 512) rc = launch_knn<512, 8, false>(ctx, d_pts, M, k, nullptr, d_ovf, d_support, 148 * 64);
+    if (cap == 256) rc = launch_knn_select<8, 8>(ctx, d_pts, M, k, d_ovf, d_support, 148 * 64);
+    else if (cap == 512) rc = launch_knn_select<16, 8>(ctx, d_pts, M, k, d_ovf, d_support, 148 * 64);
     else rc = launch_knn<1024, 4, false>(ctx, d_pts, M, k, nullptr, d_ovf, d_support, 148 * 64);
     if (rc == RPIM_OK) rc = launch_knn<KNN_CAP_MAX, 4, true>(ctx, d_pts, M, k, d_ovf, nullptr, d_support, 148 * 2);
     ws_free(ctx, &d_ovf);   // parked in the workspace cache (later reuse is ordered by the stream)

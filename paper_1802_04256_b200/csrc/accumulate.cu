@@ -34,14 +34,17 @@ constexpr int ilog2_ce(int v) { return v <= 1 ? 0 : 1 + ilog2_ce(v >> 1); }
 
 constexpr int RED_NB = 32;   // incident points per batch
 
-template <int NWARP, int CPW>
+// MASKED = false: slot lookup on the fly (hash table + byte table).  MASKED = true: the slot masks
+// precomputed by rpim_stage_slot_masks (pattern.cu) are used instead.
+template <int NWARP, int CPW, bool MASKED>
 struct alignas(16) RedSmem {
     static constexpr int NW = NWARP * CPW;                 // 32-slot chunks of the row
     static constexpr int NS = 32 * NW;                     // column slots
     static constexpr int HLOG = ilog2_ce(4 * NS - 1);
     static constexpr int HSZ = 1 << HLOG;                  // open-addressing table: 2..4 x the row length
-    unsigned long long hent[HSZ];       // (column node id << 32) | slot, ~0 = empty
-    unsigned char pos[RED_NB][NS];      // position of slot's node in the support of point b, 0xFF = absent
+    unsigned long long hent[MASKED ? 2 : HSZ];             // (column node id << 32) | slot, ~0 = empty
+    unsigned char pos[MASKED ? 1 : RED_NB][NS];            // position of slot's node in the support of point b, 0xFF = absent
+    unsigned long long mp[MASKED ? RED_NB : 1][NW];        // (support positions before chunk c << 32) | slot mask of chunk c
     double a[RED_NB][4];                // w * grad phi_I at point b (+ pad)
     const double* qbase[RED_NB];        // staged shape functions of point b
     unsigned cmask[RED_NB];             // chunks of the row hit by point b
@@ -57,14 +60,15 @@ __host__ __device__ inline size_t red_group_bytes(size_t head, int k, int nbg) {
 
 // NWARP warps own one block row, each CPW chunks of 32 column slots (chunk c = cc * NWARP + wg);
 // a CTA holds ROWS such groups working on consecutive rows.
-template <int NWARP, int CPW, int ROWS>
+template <int NWARP, int CPW, int ROWS, bool MASKED>
 __global__ void __launch_bounds__(NWARP * ROWS * 32)
 reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
                    const uint8_t* __restrict__ inc_j, const int32_t* __restrict__ support,
                    const double* __restrict__ stage, const double* __restrict__ qw,
-                   const int64_t* __restrict__ brow_ptr, const int32_t* __restrict__ bcol, double lambda, double mu,
+                   const int64_t* __restrict__ brow_ptr, const int32_t* __restrict__ bcol,
+                   const int64_t* __restrict__ mask_ptr, const unsigned* __restrict__ masks, double lambda, double mu,
                    double bx, double by, double bz, double* __restrict__ vals, double* __restrict__ f) {
-    using S = RedSmem<NWARP, CPW>;
+    using S = RedSmem<NWARP, CPW, MASKED>;
     constexpr int NS = S::NS, HSZ = S::HSZ, GT = NWARP * 32;
     constexpr int HSHIFT = 32 - S::HLOG;
     extern __shared__ __align__(16) unsigned char red_smem_raw[];
@@ -76,6 +80,7 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
     const int gstride = nbg * k * 4;            // doubles per staging buffer
     const unsigned pbytes = (unsigned)k * 32u;  // bytes of one point's staged row
     const int npass = (k + 31) >> 5;
+    const unsigned lt = (1u << lane) - 1u;
     if (tg == 0) { mbar_init(&sm.full[0], 1); mbar_init(&sm.full[1], 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     unsigned ph0 = 0, ph1 = 0;   // parity of the next completion of each staging buffer
@@ -85,14 +90,18 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
         const int64_t o = brow_ptr[I];
         const int L = (int)(brow_ptr[I + 1] - o);
         group_sync<NWARP>(rg);   // the previous row's shared data is dead
-        for (int s = tg; s < HSZ; s += GT) sm.hent[s] = ~0ull;
-        group_sync<NWARP>(rg);
-        for (int s = tg; s < L; s += GT) {
-            const unsigned J = (unsigned)bcol[o + s];
-            unsigned h = (J * 2654435761u) >> HSHIFT;
-            const unsigned long long ent = ((unsigned long long)J << 32) | (unsigned)s;
-            while (atomicCAS(&sm.hent[h], ~0ull, ent) != ~0ull) h = (h + 1) & (HSZ - 1);
+        if constexpr (!MASKED) {
+            for (int s = tg; s < HSZ; s += GT) sm.hent[s] = ~0ull;
+            group_sync<NWARP>(rg);
+            for (int s = tg; s < L; s += GT) {
+                const unsigned J = (unsigned)bcol[o + s];
+                unsigned h = (J * 2654435761u) >> HSHIFT;
+                const unsigned long long ent = ((unsigned long long)J << 32) | (unsigned)s;
+                while (atomicCAS(&sm.hent[h], ~0ull, ent) != ~0ull) h = (h + 1) & (HSZ - 1);
+            }
         }
+        const int NWc = (L + 31) >> 5;   // mask words per incident point of this row
+        const unsigned* mrow = MASKED ? masks + mask_ptr[I] : nullptr;
         double acc[CPW][9];
 #pragma unroll
         for (int cc = 0; cc < CPW; ++cc)
@@ -116,8 +125,19 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                 fsum += w * v01.x;
                 sm.a[tg][0] = w * v01.y; sm.a[tg][1] = w * v23.x; sm.a[tg][2] = w * v23.y;
                 sm.qbase[tg] = base;
+                if constexpr (MASKED) {
+                    const unsigned* mw = mrow + (p - pa) * NWc;
+                    unsigned pre = 0, cm = 0;
+                    for (int w = 0; w < NWc; ++w) {
+                        const unsigned word = mw[w];
+                        sm.mp[tg][w] = ((unsigned long long)pre << 32) | word;
+                        pre += __popc(word);
+                        cm |= (word != 0u ? 1u : 0u) << w;
+                    }
+                    sm.cmask[tg] = cm;
+                }
             }
-            {
+            if constexpr (!MASKED) {
                 uint4* pz = reinterpret_cast<uint4*>(&sm.pos[0][0]);
                 const uint4 ff = make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu);
                 for (int e = tg; e < nb * (NS / 16); e += GT) pz[e] = ff;
@@ -133,7 +153,7 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
             };
             if (tg == 0) { issue(0); if (nsub > 1) issue(1); }
             // ---- phase 1b: positions of this warp's points b = wg, wg + NWARP, ... (overlaps the copies)
-            for (int b = wg; b < nb; b += NWARP) {
+            for (int b = wg; !MASKED && b < nb; b += NWARP) {
                 const int32_t* sp = support + (sm.qbase[b] - stage) / 4;   // = support + q * k
                 unsigned cm = 0;
                 for (int ps = 0; ps < npass; ++ps) {
@@ -170,7 +190,14 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                     for (int cc = 0; cc < CPW; ++cc) {
                         const int c = cc * NWARP + wg;
                         if (!((cm >> c) & 1u)) continue;
-                        const unsigned j = prow[32 * c];
+                        unsigned j;
+                        if constexpr (MASKED) {
+                            const unsigned long long mpv = sm.mp[b][c];
+                            const unsigned word = (unsigned)mpv;
+                            j = ((word >> lane) & 1u) ? (unsigned)(mpv >> 32) + __popc(word & lt) : 0xFFu;
+                        } else {
+                            j = prow[32 * c];
+                        }
                         if (j != 0xFFu) {
                             const double2 g01 = *reinterpret_cast<const double2*>(base + 4 * j);
                             const double2 gyz = *reinterpret_cast<const double2*>(base + 4 * j + 2);
@@ -380,13 +407,13 @@ static int accumulate_generic(rpim_ctx* ctx, const double* d_qw, double lambda, 
 }
 
 namespace {
-template <int NWARP, int CPW, int ROWS>
-int launch_reduce_rows(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
-                       double* d_vals, double* d_f) {
-    auto kern = reduce_rows_kernel<NWARP, CPW, ROWS>;
+template <int NWARP, int CPW, int ROWS, bool MASKED>
+int launch_reduce_rows_m(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
+                         double* d_vals, double* d_f) {
+    auto kern = reduce_rows_kernel<NWARP, CPW, ROWS, MASKED>;
     // gradient staging: two buffers of nbg points each, about 16 KB per row group
     const int nbg = std::max(2, std::min(8, 8192 / (ctx->k * 32)));
-    const size_t smem = red_group_bytes(sizeof(RedSmem<NWARP, CPW>), ctx->k, nbg) * ROWS;
+    const size_t smem = red_group_bytes(sizeof(RedSmem<NWARP, CPW, MASKED>), ctx->k, nbg) * ROWS;
     CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 1;
     CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NWARP * ROWS * 32, smem));
@@ -397,16 +424,23 @@ int launch_reduce_rows(rpim_ctx* ctx, const double* d_qw, double lambda, double 
     blocks = std::min<int64_t>(blocks, (int64_t)sms * per_sm * 8);   // several waves: boundary rows are cheaper
     kern<<<(unsigned)blocks, NWARP * ROWS * 32, smem, ctx->stream>>>(
         ctx->N, ctx->k, nbg, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_support, ctx->d_stage, d_qw,
-        ctx->d_brow_ptr, ctx->d_bcol, lambda, mu, body[0], body[1], body[2], d_vals, d_f);
+        ctx->d_brow_ptr, ctx->d_bcol, ctx->d_mask_ptr, ctx->d_masks, lambda, mu, body[0], body[1], body[2], d_vals, d_f);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
+}
+// precomputed slot masks when the pattern stage could afford them (pattern.cu), else on-the-fly lookup
+template <int NWARP, int CPW, int ROWS>
+int launch_reduce_rows(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
+                       double* d_vals, double* d_f) {
+    return ctx->have_masks ? launch_reduce_rows_m<NWARP, CPW, ROWS, true>(ctx, d_qw, lambda, mu, body, d_vals, d_f)
+                           : launch_reduce_rows_m<NWARP, CPW, ROWS, false>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
 }
 }  // namespace
 
 int rpim_stage_accumulate(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
                           double* d_vals, double* d_f) {
     const int Lmax = std::max(ctx->max_blen, 1);
-    static_assert(sizeof(RedSmem<1, 4>) % 16 == 0 && sizeof(RedSmem<8, 4>) % 16 == 0, "group stride keeps 16-byte alignment");
+    static_assert(sizeof(RedSmem<1, 4, false>) % 16 == 0 && sizeof(RedSmem<8, 4, true>) % 16 == 0 && sizeof(RedSmem<2, 3, true>) % 16 == 0, "group stride keeps 16-byte alignment");
     if (Lmax <= 128) return launch_reduce_rows<1, 4, 8>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
     if (Lmax <= 192) return launch_reduce_rows<2, 3, 4>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
     if (Lmax <= 256) return launch_reduce_rows<2, 4, 4>(ctx, d_qw, lambda, mu, body, d_vals, d_f);

@@ -30,6 +30,8 @@ void free_all(rpim_ctx* c) {
     ws_free(c, &c->d_inc_count); ws_free(c, &c->d_inc_ptr); ws_free(c, &c->d_inc_q); ws_free(c, &c->d_inc_j);
     ws_free(c, &c->d_blen); ws_free(c, &c->d_brow_ptr); ws_free(c, &c->d_bcol); ws_free(c, &c->d_bdiag);
     ws_free(c, &c->d_stage); ws_free(c, &c->d_singular); ws_free(c, &c->d_scratch);
+    ws_free(c, &c->d_mask_ptr); ws_free(c, &c->d_masks);
+    c->have_masks = false;
     ws_free(c, &c->h2d_nodes); ws_free(c, &c->h2d_qpts);
     { int64_t* t = (int64_t*)c->d_scan_tmp; ws_free(c, &t); c->d_scan_tmp = nullptr; c->scan_tmp_elems = 0; }
     ws_release_cache(c);
@@ -85,7 +87,7 @@ int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const do
     if (N > 700000000 || Nq * (int64_t)k > 0x7fffffff00LL || Nq > 0x7fffffff) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "problem too large for 32-bit node / point ids");
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
-    ctx->have_pattern = ctx->have_shape = false;
+    ctx->have_pattern = ctx->have_shape = ctx->have_masks = false;
     ws_free(ctx, &ctx->d_stage);
     ws_free(ctx, &ctx->d_singular);
     ctx->d_nodes = d_nodes; ctx->d_qpts = d_qpts; ctx->N = N; ctx->Nq = Nq; ctx->k = k;
@@ -98,6 +100,7 @@ int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const do
     if ((rc = rpim_stage_incidence(ctx))) return rc;
     cudaEventRecord(ctx->ev[2], st);
     if ((rc = rpim_stage_block_pattern(ctx))) return rc;
+    if ((rc = rpim_stage_slot_masks(ctx))) return rc;
     cudaEventRecord(ctx->ev[3], st);
     CUDA_TRY(ctx, cudaStreamSynchronize(st));
     for (int i = 0; i < 3; ++i) {

@@ -77,6 +77,13 @@ struct rpim_ctx {
     int32_t* d_bcol = nullptr;       // nnzb
     int* d_bdiag = nullptr;          // N (slot of the diagonal block in its row)
 
+    // precomputed slot maps of the reduction (optional: skipped when they would not fit):
+    // for incident point p of block row I, ceil(L_I / 32) words; bit s = column slot s of the row
+    // is a support node of the point
+    bool have_masks = false;
+    int64_t* d_mask_ptr = nullptr;   // N + 1 (word offset of row I)
+    unsigned* d_masks = nullptr;
+
     // staged shape functions: Nq x k x 4  (phi, dphi/dx, dphi/dy, dphi/dz per support node: one 32-byte sector)
     double* d_stage = nullptr;
     uint8_t* d_singular = nullptr;   // Nq
@@ -190,6 +197,7 @@ int rpim_scan_i32_to_i64(rpim_ctx* ctx, const int* d_in, int64_t* d_out, int64_t
 int rpim_stage_grid_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, int32_t* d_support, bool build_grid);
 int rpim_stage_incidence(rpim_ctx* ctx);
 int rpim_stage_block_pattern(rpim_ctx* ctx);
+int rpim_stage_slot_masks(rpim_ctx* ctx);
 int rpim_stage_emit_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx);
 int rpim_stage_shape(rpim_ctx* ctx, const double* d_pts, const int32_t* d_support, int64_t M, double* d_stage,
                      uint8_t* d_singular);

@@ -414,6 +414,129 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
     return RPIM_OK;
 }
 
+// ------------------------------------------------------------------ precomputed slot maps of the reduction (step a6)
+// For incident point p of block row I: ceil(L_I / 32) words, bit s set iff column slot s of the row
+// is a support node of the point.  With the supports and the rows both ascending, the position of
+// slot s's node in the support is the number of set bits below s, so the masks are all the
+// reduction needs to route gradients to CSR slots (accumulate.cu, MASKED kernels).
+namespace {
+__global__ void mask_count_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int64_t* __restrict__ brow_ptr,
+                                  int* __restrict__ count) {
+    const int64_t I = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (I >= N) return;
+    const int64_t len = inc_ptr[I + 1] - inc_ptr[I];
+    const int64_t nw = (brow_ptr[I + 1] - brow_ptr[I] + 31) >> 5;
+    count[I] = (int)(len * nw);
+}
+
+template <int HLOG, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32)
+slot_mask_kernel(int64_t N, int k, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
+                 const int32_t* __restrict__ support, const int64_t* __restrict__ brow_ptr,
+                 const int32_t* __restrict__ bcol, const int64_t* __restrict__ mask_ptr, unsigned* __restrict__ masks) {
+    constexpr int HSZ = 1 << HLOG;
+    __shared__ unsigned long long hent_s[WARPS][HSZ];
+    __shared__ unsigned words_s[WARPS][32];
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned long long* hent = hent_s[wid];
+    unsigned* words = words_s[wid];
+    const int npass = (k + 31) >> 5;
+    for (int64_t I = (int64_t)blockIdx.x * WARPS + wid; I < N; I += (int64_t)gridDim.x * WARPS) {
+        const int64_t o = brow_ptr[I];
+        const int L = (int)(brow_ptr[I + 1] - o);
+        const int NWc = (L + 31) >> 5;
+        const int64_t pa = inc_ptr[I], pb = inc_ptr[I + 1];
+        if (pa == pb) continue;
+        __syncwarp();
+        for (int s = lane; s < HSZ; s += 32) hent[s] = ~0ull;
+        __syncwarp();
+        for (int s = lane; s < L; s += 32) {
+            const unsigned J = (unsigned)bcol[o + s];
+            unsigned h = (J * 2654435761u) >> (32 - HLOG);
+            const unsigned long long ent = ((unsigned long long)J << 32) | (unsigned)s;
+            while (atomicCAS(&hent[h], ~0ull, ent) != ~0ull) h = (h + 1) & (HSZ - 1);
+        }
+        __syncwarp();
+        unsigned* dst = masks + mask_ptr[I];
+        const int64_t nitems = (pb - pa) * npass;
+        auto loadJ = [&](int64_t item) {
+            const int64_t t = item / npass;
+            const int j = (int)(item - t * npass) * 32 + lane;
+            return (j < k) ? support[(int64_t)inc_q[pa + t] * k + j] : -1;
+        };
+        int Jnext = loadJ(0);
+        for (int64_t item = 0; item < nitems; ++item) {
+            const int J = Jnext;
+            if (item + 1 < nitems) Jnext = loadJ(item + 1);
+            const int64_t t = item / npass;
+            const int ps = (int)(item - t * npass);
+            if (ps == 0) {
+                if (lane < NWc) words[lane] = 0u;
+                __syncwarp();
+            }
+            if (J >= 0) {
+                unsigned h = ((unsigned)J * 2654435761u) >> (32 - HLOG);
+                unsigned long long ent = hent[h];
+                while ((unsigned)(ent >> 32) != (unsigned)J) { h = (h + 1) & (HSZ - 1); ent = hent[h]; }
+                const unsigned slot = (unsigned)ent;
+                atomicOr(&words[slot >> 5], 1u << (slot & 31));
+            }
+            if (ps == npass - 1) {
+                __syncwarp();
+                if (lane < NWc) dst[t * NWc + lane] = words[lane];
+                __syncwarp();
+            }
+        }
+    }
+}
+}  // namespace
+
+int rpim_stage_slot_masks(rpim_ctx* ctx) {
+    cudaStream_t st = ctx->stream;
+    const int64_t N = ctx->N;
+    ctx->have_masks = false;
+    if (ctx->max_blen > 1024 || ctx->max_blen < 1) return RPIM_OK;   // such rows take the generic reduction
+    int rc;
+    int* d_cnt = nullptr;
+    if ((rc = ws_alloc(ctx, &d_cnt, N))) return rc;
+    if ((rc = ws_alloc(ctx, &ctx->d_mask_ptr, N + 1))) { ws_free(ctx, &d_cnt); return rc; }
+    mask_count_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, ctx->d_inc_ptr, ctx->d_brow_ptr, d_cnt);
+    KERNEL_CHECK(ctx);
+    rc = rpim_scan_i32_to_i64(ctx, d_cnt, ctx->d_mask_ptr, N);
+    ws_free(ctx, &d_cnt);
+    if (rc) return rc;
+    int64_t nwords = 0;
+    CUDA_TRY(ctx, cudaMemcpyAsync(&nwords, ctx->d_mask_ptr + N, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    // budget: the maps are an accelerator, not a requirement -- skip them when they would take
+    // more than a quarter of the free device memory (config 5: ~55 GB) or the allocation fails
+    size_t free_b = 0, total_b = 0;
+    CUDA_TRY(ctx, cudaMemGetInfo(&free_b, &total_b));
+    const int64_t bytes = nwords * (int64_t)sizeof(unsigned);
+    bool reuse = false;   // a parked block of the right size does not count against the budget
+    for (auto& b : ctx->ws_cache) reuse = reuse || (b.second >= bytes && b.second <= 2 * bytes + 4096);
+    if (ctx->d_masks) { auto it = ctx->ws_sizes.find((void*)ctx->d_masks); reuse = reuse || (it != ctx->ws_sizes.end() && it->second >= bytes && it->second <= 2 * bytes + 4096); }
+    if (!reuse && (uint64_t)bytes > free_b / 4) { ws_free(ctx, &ctx->d_masks); return RPIM_OK; }
+    if (ws_alloc(ctx, &ctx->d_masks, nwords) != RPIM_OK) { ctx->err.clear(); return RPIM_OK; }
+    const int Lmax = ctx->max_blen;
+    constexpr int W = 8;
+    const unsigned nb = (unsigned)std::min<int64_t>((N + W - 1) / W, 148 * 32);
+    if (Lmax <= 256)
+        slot_mask_kernel<9, W><<<nb, W * 32, 0, st>>>(N, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support,
+                                                      ctx->d_brow_ptr, ctx->d_bcol, ctx->d_mask_ptr, ctx->d_masks);
+    else if (Lmax <= 512)
+        slot_mask_kernel<10, 4><<<(unsigned)std::min<int64_t>((N + 3) / 4, 148 * 32), 128, 0, st>>>(
+            N, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->d_brow_ptr, ctx->d_bcol, ctx->d_mask_ptr,
+            ctx->d_masks);
+    else
+        slot_mask_kernel<11, 2><<<(unsigned)std::min<int64_t>((N + 1) / 2, 148 * 32), 64, 0, st>>>(
+            N, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->d_brow_ptr, ctx->d_bcol, ctx->d_mask_ptr,
+            ctx->d_masks);
+    KERNEL_CHECK(ctx);
+    ctx->have_masks = true;
+    return RPIM_OK;
+}
+
 int rpim_stage_emit_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx) {
     cudaStream_t st = ctx->stream;
     const int64_t N = ctx->N;

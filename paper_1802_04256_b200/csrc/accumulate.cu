@@ -80,7 +80,7 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
     const int gstride = nbg * k * 4;            // doubles per staging buffer
     const unsigned pbytes = (unsigned)k * 32u;  // bytes of one point's staged row
     const int npass = (k + 31) >> 5;
-    const unsigned lt = (1u << lane) - 1u;
+    const unsigned lbit = 1u << lane, lt = lbit - 1u;
     if (tg == 0) { mbar_init(&sm.full[0], 1); mbar_init(&sm.full[1], 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     unsigned ph0 = 0, ph1 = 0;   // parity of the next completion of each staging buffer
@@ -127,14 +127,13 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                 sm.qbase[tg] = base;
                 if constexpr (MASKED) {
                     const unsigned* mw = mrow + (p - pa) * NWc;
-                    unsigned pre = 0, cm = 0;
+                    unsigned pre = 0;
                     for (int w = 0; w < NWc; ++w) {
                         const unsigned word = mw[w];
                         sm.mp[tg][w] = ((unsigned long long)pre << 32) | word;
                         pre += __popc(word);
-                        cm |= (word != 0u ? 1u : 0u) << w;
                     }
-                    sm.cmask[tg] = cm;
+                    for (int w = NWc; w < S::NW; ++w) sm.mp[tg][w] = 0ull;
                 }
             }
             if constexpr (!MASKED) {
@@ -182,29 +181,43 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                 const double* Gb = G + (sb & 1) * gstride;
                 for (int bb = 0; bb < cnt; ++bb) {
                     const int b = b0 + bb;
-                    const unsigned cm = sm.cmask[b];
                     const double ax = sm.a[b][0], ay = sm.a[b][1], az = sm.a[b][2];
                     const double* base = Gb + bb * k * 4;
-                    const unsigned char* prow = &sm.pos[b][lane];
+                    if constexpr (MASKED) {
+                        // all chunk words first (independent loads), then the hits; an empty chunk
+                        // (word = 0, also every chunk beyond the row's length) is skipped by the whole warp
+                        unsigned long long mpv[CPW];
 #pragma unroll
-                    for (int cc = 0; cc < CPW; ++cc) {
-                        const int c = cc * NWARP + wg;
-                        if (!((cm >> c) & 1u)) continue;
-                        unsigned j;
-                        if constexpr (MASKED) {
-                            const unsigned long long mpv = sm.mp[b][c];
-                            const unsigned word = (unsigned)mpv;
-                            j = ((word >> lane) & 1u) ? (unsigned)(mpv >> 32) + __popc(word & lt) : 0xFFu;
-                        } else {
-                            j = prow[32 * c];
+                        for (int cc = 0; cc < CPW; ++cc) mpv[cc] = sm.mp[b][cc * NWARP + wg];
+#pragma unroll
+                        for (int cc = 0; cc < CPW; ++cc) {
+                            const unsigned word = (unsigned)mpv[cc];
+                            if (word & lbit) {
+                                const unsigned j = (unsigned)(mpv[cc] >> 32) + __popc(word & lt);
+                                const double2 g01 = *reinterpret_cast<const double2*>(base + 4 * j);
+                                const double2 gyz = *reinterpret_cast<const double2*>(base + 4 * j + 2);
+                                const double gx = g01.y;
+                                acc[cc][0] = fma(ax, gx, acc[cc][0]); acc[cc][1] = fma(ax, gyz.x, acc[cc][1]); acc[cc][2] = fma(ax, gyz.y, acc[cc][2]);
+                                acc[cc][3] = fma(ay, gx, acc[cc][3]); acc[cc][4] = fma(ay, gyz.x, acc[cc][4]); acc[cc][5] = fma(ay, gyz.y, acc[cc][5]);
+                                acc[cc][6] = fma(az, gx, acc[cc][6]); acc[cc][7] = fma(az, gyz.x, acc[cc][7]); acc[cc][8] = fma(az, gyz.y, acc[cc][8]);
+                            }
                         }
-                        if (j != 0xFFu) {
-                            const double2 g01 = *reinterpret_cast<const double2*>(base + 4 * j);
-                            const double2 gyz = *reinterpret_cast<const double2*>(base + 4 * j + 2);
-                            const double gx = g01.y;
-                            acc[cc][0] = fma(ax, gx, acc[cc][0]); acc[cc][1] = fma(ax, gyz.x, acc[cc][1]); acc[cc][2] = fma(ax, gyz.y, acc[cc][2]);
-                            acc[cc][3] = fma(ay, gx, acc[cc][3]); acc[cc][4] = fma(ay, gyz.x, acc[cc][4]); acc[cc][5] = fma(ay, gyz.y, acc[cc][5]);
-                            acc[cc][6] = fma(az, gx, acc[cc][6]); acc[cc][7] = fma(az, gyz.x, acc[cc][7]); acc[cc][8] = fma(az, gyz.y, acc[cc][8]);
+                    } else {
+                        const unsigned cm = sm.cmask[b];
+                        const unsigned char* prow = &sm.pos[b][lane];
+#pragma unroll
+                        for (int cc = 0; cc < CPW; ++cc) {
+                            const int c = cc * NWARP + wg;
+                            if (!((cm >> c) & 1u)) continue;
+                            const unsigned j = prow[32 * c];
+                            if (j != 0xFFu) {
+                                const double2 g01 = *reinterpret_cast<const double2*>(base + 4 * j);
+                                const double2 gyz = *reinterpret_cast<const double2*>(base + 4 * j + 2);
+                                const double gx = g01.y;
+                                acc[cc][0] = fma(ax, gx, acc[cc][0]); acc[cc][1] = fma(ax, gyz.x, acc[cc][1]); acc[cc][2] = fma(ax, gyz.y, acc[cc][2]);
+                                acc[cc][3] = fma(ay, gx, acc[cc][3]); acc[cc][4] = fma(ay, gyz.x, acc[cc][4]); acc[cc][5] = fma(ay, gyz.y, acc[cc][5]);
+                                acc[cc][6] = fma(az, gx, acc[cc][6]); acc[cc][7] = fma(az, gyz.x, acc[cc][7]); acc[cc][8] = fma(az, gyz.y, acc[cc][8]);
+                            }
                         }
                     }
                 }

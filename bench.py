@@ -50,6 +50,15 @@ def read_peaks():
     return 6650.0, 1965.0, "fallback"
 
 
+def read_traffic(config_name: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the two hot kernels, from the committed
+    `ncu --set full` summaries (profiles/traffic.json, keyed by config); {} when there is none."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        return json.load(open(p)).get(config_name, {})
+    return {}
+
+
 def flops_per_point(k: int):
     """Algorithmic fp64 flops per quadrature point of THIS implementation,
     fma = 2.  Returns (shape_flops, reduce_flops)."""
@@ -284,28 +293,43 @@ def main():
     ms_asm = e0.elapsed_time(e1) / args.steps
 
     # ------------------------------------------------ roofline of the dominant kernel (live CUDA events)
+    # the reduction into CSR is bound by HBM (K is written once: 8 nnz bytes, plus
+    # one read of the staged shape functions and of the incidence lists); the shape-function kernel is
+    # bound by the plain FP64 pipe (no tensor-core form exists for the operation-level contract).
     n_asm = max(1, calls[1])
     shape_ms, reduce_ms = phase_ms[3] / n_asm, phase_ms[4] / n_asm
     fl_shape, fl_reduce = flops_per_point(w.k)
     peak_tflops = N_SM * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
-    if shape_ms >= reduce_ms:
-        dom, dom_ms, dom_fl = "shape_functions", shape_ms, fl_shape * w.Nq
+    reduce_bytes = 8 * nnz + 32 * w.Nq * w.k + 5 * w.Nq * w.k + 24 * w.N
+    traffic = read_traffic(w.name)
+    if reduce_ms >= shape_ms:
+        achieved = reduce_bytes / (reduce_ms * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": "reduce_rows_kernel (reduce_into_csr)", "achieved": achieved,
+                    "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
+                    "traffic": traffic.get("reduce_rows_kernel"),
+                    "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
+                    "algorithmic_bytes_per_launch": reduce_bytes}
     else:
-        dom, dom_ms, dom_fl = "reduce_into_csr", reduce_ms, fl_reduce * w.Nq
-    achieved = dom_fl / (dom_ms * 1e-3) / 1e12
-    roofline = {
-        "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-        "frac": achieved / peak_tflops, "traffic": None,
-        "peak_source": f"derived: {N_SM} SM x {FP64_LANES_PER_SM} DFMA/clk x 2 x {sm_max_mhz:.0f} MHz (DESIGN.md section 5)",
+        achieved = fl_shape * w.Nq / (shape_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "shape_rows_kernel (shape_functions)", "achieved": achieved,
+                    "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+                    "traffic": traffic.get("shape_rows_kernel"),
+                    "peak_source": f"derived: {N_SM} SM x {FP64_LANES_PER_SM} DFMA/clk x 2 x {sm_max_mhz:.0f} MHz "
+                                   "(DESIGN.md section 5)",
+                    "algorithmic_flops_per_launch": fl_shape * w.Nq}
+    hbm_min = nnz * 8 + w.Nq * w.k * 4 + w.Nq * 32 + w.N * 24 + 3 * w.N * 8
+    roofline.update({
         "kernel_ms": {"shape_functions": shape_ms, "reduce_into_csr": reduce_ms,
                       "knn": phase_ms[0] / max(1, calls[0]), "incidence": phase_ms[1] / max(1, calls[0]),
                       "block_pattern": phase_ms[2] / max(1, calls[0])},
+        "shape_fp64_frac": fl_shape * w.Nq / (shape_ms * 1e-3) / 1e12 / peak_tflops,
+        "reduce_hbm_frac": reduce_bytes / (reduce_ms * 1e-3) / 1e9 / hbm_gbs,
         "assemble_flops_per_point": fl_shape + fl_reduce,
         "assemble_fp64_frac": (fl_shape + fl_reduce) * w.Nq / (ms_asm * 1e-3) / 1e12 / peak_tflops,
-        "assemble_hbm_min_bytes": nnz * 8 + w.Nq * w.k * 4 + w.Nq * 32 + w.N * 24 + 3 * w.N * 8,
-        "assemble_hbm_frac": (nnz * 8 + w.Nq * w.k * 4 + w.Nq * 32 + w.N * 24 + 3 * w.N * 8) / (ms_asm * 1e-3) / 1e9 / hbm_gbs,
-        "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": peak_src,
-    }
+        "assemble_hbm_min_bytes": hbm_min,
+        "assemble_hbm_frac": hbm_min / (ms_asm * 1e-3) / 1e9 / hbm_gbs,
+        "fp64_peak_tflops": peak_tflops, "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": peak_src,
+    })
 
     # ------------------------------------------------ end to end through the host-buffer C ABI calls
     e2e = None

@@ -52,11 +52,15 @@ def read_peaks():
 
 def read_traffic(config_name: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the two hot kernels, from the committed
-    `ncu --set full` summaries (profiles/traffic.json, keyed by config); {} when there is none."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    `ncu --set full` summaries (profiles/traffic.csv, see profiles/traffic.md); {} when there is none."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    out = {}
     if os.path.exists(p):
-        return json.load(open(p)).get(config_name, {})
-    return {}
+        for line in open(p).read().splitlines()[1:]:
+            parts = line.split(",")
+            if len(parts) == 3 and parts[0] == config_name:
+                out[parts[1]] = float(parts[2])
+    return out
 
 
 def flops_per_point(k: int):

@@ -38,12 +38,14 @@ inc_sort_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, int32_t* __restr
     extern __shared__ unsigned char smem_raw[];
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned long long* key = (unsigned long long*)smem_raw + (size_t)wid * CAP;
+    if (LO > 0 && flags[FLAG_INC_LONG] == 0) return;   // second launch: the first one met no longer list
     for (int64_t I = (int64_t)blockIdx.x * WARPS + wid; I < N; I += (int64_t)gridDim.x * WARPS) {
         const int64_t a = inc_ptr[I];
         const int len = (int)(inc_ptr[I + 1] - a);
         if (len <= 1 || len <= LO) continue;
         if (len > CAP) {
             if (CAP == INC_CAP && lane == 0) atomicAdd((unsigned long long*)&flags[FLAG_INC_CAP], 1ull);
+            if (CAP != INC_CAP && lane == 0) flags[FLAG_INC_LONG] = 1;
             continue;
         }
         const int np = next_pow2(len);

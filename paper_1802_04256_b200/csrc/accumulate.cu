@@ -66,8 +66,8 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                    const uint8_t* __restrict__ inc_j, const int32_t* __restrict__ support,
                    const double* __restrict__ stage, const double* __restrict__ qw,
                    const int64_t* __restrict__ brow_ptr, const int32_t* __restrict__ bcol,
-                   const int64_t* __restrict__ mask_ptr, const unsigned* __restrict__ masks, double lambda, double mu,
-                   double bx, double by, double bz, double* __restrict__ vals, double* __restrict__ f) {
+                   const int64_t* __restrict__ mask_ptr, const unsigned* __restrict__ masks, int mask_stride, double lambda,
+                   double mu, double bx, double by, double bz, double* __restrict__ vals, double* __restrict__ f) {
     using S = RedSmem<NWARP, CPW, MASKED>;
     constexpr int NS = S::NS, HSZ = S::HSZ, GT = NWARP * 32;
     constexpr int HSHIFT = 32 - S::HLOG;
@@ -101,7 +101,8 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
             }
         }
         const int NWc = (L + 31) >> 5;   // mask words per incident point of this row
-        const unsigned* mrow = MASKED ? masks + mask_ptr[I] : nullptr;
+        const int mstep = mask_stride > 0 ? mask_stride : NWc;   // words from one incident point to the next
+        const unsigned* mrow = !MASKED ? nullptr : (mask_stride > 0 ? masks + inc_ptr[I] * mask_stride : masks + mask_ptr[I]);
         double acc[CPW][9];
 #pragma unroll
         for (int cc = 0; cc < CPW; ++cc)
@@ -126,7 +127,7 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                 sm.a[tg][0] = w * v01.y; sm.a[tg][1] = w * v23.x; sm.a[tg][2] = w * v23.y;
                 sm.qbase[tg] = base;
                 if constexpr (MASKED) {
-                    const unsigned* mw = mrow + (p - pa) * NWc;
+                    const unsigned* mw = mrow + (p - pa) * mstep;
                     unsigned pre = 0;
                     for (int w = 0; w < NWc; ++w) {
                         const unsigned word = mw[w];
@@ -437,7 +438,7 @@ int launch_reduce_rows_m(rpim_ctx* ctx, const double* d_qw, double lambda, doubl
     blocks = std::min<int64_t>(blocks, (int64_t)sms * per_sm * 8);   // several waves: boundary rows are cheaper
     kern<<<(unsigned)blocks, NWARP * ROWS * 32, smem, ctx->stream>>>(
         ctx->N, ctx->k, nbg, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_support, ctx->d_stage, d_qw,
-        ctx->d_brow_ptr, ctx->d_bcol, ctx->d_mask_ptr, ctx->d_masks, lambda, mu, body[0], body[1], body[2], d_vals, d_f);
+        ctx->d_brow_ptr, ctx->d_bcol, ctx->d_mask_ptr, ctx->d_masks, ctx->mask_stride, lambda, mu, body[0], body[1], body[2], d_vals, d_f);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
 }

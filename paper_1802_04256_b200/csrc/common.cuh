@@ -81,6 +81,7 @@ struct rpim_ctx {
     // for incident point p of block row I, ceil(L_I / 32) words; bit s = column slot s of the row
     // is a support node of the point
     bool have_masks = false;
+    int mask_stride = 0;             // > 0: words per incident point, row I at inc_ptr[I] * stride; 0: d_mask_ptr, ceil(L_I/32)
     int64_t* d_mask_ptr = nullptr;   // N + 1 (word offset of row I)
     unsigned* d_masks = nullptr;
 

@@ -66,10 +66,8 @@ inc_sort_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, int32_t* __restr
 // Block row I = sorted union of supp(q) over the points q incident to node I.  A warp owns a row
 // and builds the union in an open-addressing table in shared memory.
 //
-// Fast path (brow_fast_kernel): a small table (HASH entries) and ONE pass -- the sorted row is
-// parked in a fixed-stride pool, lengths are scanned, rows are copied to their CSR place.  Rows
-// that do not fit (more than PSTRIDE columns) go to an overflow list and take the general
-// two-pass path (count, scan, fill) with the large table.
+// Rows that do not fit the fast path below (more than PSTRIDE columns) go to an overflow list and
+// take the general two-pass path (count, scan, fill) with the large table.
 constexpr int PAT_HASH = 4096;          // general path: open-addressing table per warp (power of two)
 constexpr int PAT_MAXROW = 2048;        // longest block row handled
 constexpr int PAT_WARPS = 4;
@@ -137,19 +135,109 @@ __device__ __forceinline__ void table_to_sorted_list(const int* table, int* list
     warp_bitonic_i32(list, np);
 }
 
+// Fast path (brow_fast_kernel): a small table (HASH entries) and ONE pass.  While the union is
+// built the table position found for every (incident point, support node) is remembered; the
+// compacted keys are sorted in REGISTERS (bitonic network, PSTRIDE / 32 keys per lane, shuffles
+// for the cross-lane strides); every table entry then learns its slot, and the slot masks of the
+// reduction (step a6) follow from the remembered positions without a second round of probing.
+// The sorted row is parked in a fixed-stride pool, lengths are scanned, rows are copied to their
+// CSR place.  Rows that do not fit go to an overflow list and take the general two-pass path.
+constexpr int HP_CAP = 2560;   // remembered table positions per row (incident points x k); beyond: re-probe
+
+// ascending bitonic sort of 32 * NPL keys, key e = lane * NPL + r held in v[r]
+template <int NPL>
+__device__ __forceinline__ void warp_sort_regs(int (&v)[NPL]) {
+    const int lane = lane_id();
+#pragma unroll
+    for (int size = 2; size <= 32 * NPL; size <<= 1) {
+#pragma unroll
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            if (stride >= NPL) {
+                const int ls = stride / NPL;
+                const bool lower = (lane & ls) == 0;
+#pragma unroll
+                for (int r = 0; r < NPL; ++r) {
+                    const bool up = ((lane * NPL + r) & size) == 0;
+                    const int other = __shfl_xor_sync(0xffffffffu, v[r], ls);
+                    v[r] = (lower == up) ? min(v[r], other) : max(v[r], other);
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < NPL; ++r) {
+                    if (r & stride) continue;
+                    const bool up = ((lane * NPL + r) & size) == 0;
+                    const int a = v[r], b = v[r + stride];
+                    const int mn = min(a, b), mx = max(a, b);
+                    v[r] = up ? mn : mx;
+                    v[r + stride] = up ? mx : mn;
+                }
+            }
+        }
+    }
+}
+
 template <int HASH, int PSTRIDE>
 __global__ void __launch_bounds__(PAT_FAST_WARPS * 32)
 brow_fast_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
                  const int32_t* __restrict__ support, int k, int* __restrict__ blen, int32_t* __restrict__ pool,
-                 int* __restrict__ bdiag, int32_t* __restrict__ ovf_rows, long long* __restrict__ flags) {
-    __shared__ int table_s[PAT_FAST_WARPS][HASH];
-    __shared__ int list_s[PAT_FAST_WARPS][PSTRIDE];
+                 int* __restrict__ bdiag, int32_t* __restrict__ ovf_rows, unsigned* __restrict__ masks,
+                 long long* __restrict__ flags) {
+    constexpr int NPL = PSTRIDE / 32;   // keys per lane in the sort = mask words per incident point
+    extern __shared__ int bf_smem[];
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    int* table = table_s[wid];
-    int* list = list_s[wid];
+    // per warp: table[HASH] | list[PSTRIDE] | tslot[HASH] (u16) | hp[HP_CAP] (u16) | mw[32]
+    constexpr int PER_WARP = HASH + PSTRIDE + HASH / 2 + HP_CAP / 2 + 32;
+    int* table = bf_smem + (size_t)wid * PER_WARP;
+    int* list = table + HASH;
+    unsigned short* tslot = reinterpret_cast<unsigned short*>(list + PSTRIDE);
+    unsigned short* hp = reinterpret_cast<unsigned short*>(list + PSTRIDE + HASH / 2);
+    unsigned* mw = reinterpret_cast<unsigned*>(list + PSTRIDE + HASH / 2 + HP_CAP / 2);
+    const int npass = (k + 31) >> 5;
+    const int kpad = npass * 32;
     for (int64_t I = (int64_t)blockIdx.x * PAT_FAST_WARPS + wid; I < N; I += (int64_t)gridDim.x * PAT_FAST_WARPS) {
-        const int L = row_union<HASH, PSTRIDE>(table, I, inc_ptr, inc_q, support, k);
-        if (L > PSTRIDE) {
+        const int64_t pa = inc_ptr[I], pb = inc_ptr[I + 1];
+        const int np = (int)(pb - pa);
+        __syncwarp();
+        for (int i = lane; i < HASH; i += 32) table[i] = -1;
+        __syncwarp();
+        // ---- union of the supports; remember where every (point, position) landed
+        int L = 0;
+        bool ovf = false;
+        {
+            auto loadJ = [&](int t, int ps) {
+                const int j = ps * 32 + lane;
+                return (t < np && j < k) ? support[(int64_t)inc_q[pa + t] * k + j] : -1;
+            };
+            int Jnext = loadJ(0, 0);
+            int fresh = 0, item = 0;
+            for (int t = 0; t < np && !ovf; ++t) {
+                for (int ps = 0; ps < npass; ++ps, ++item) {
+                    const int key = Jnext;
+                    Jnext = (ps + 1 < npass) ? loadJ(t, ps + 1) : loadJ(t + 1, 0);
+                    if (key >= 0) {
+                        unsigned h = pat_hash<HASH>(key);
+                        while (true) {
+                            const int old = atomicCAS(&table[h], -1, key);
+                            if (old == -1) { ++fresh; break; }
+                            if (old == key) break;
+                            h = (h + 1) & (HASH - 1);
+                        }
+                        const int idx = item * 32 + lane;   // = t * kpad + j
+                        if (idx < HP_CAP) hp[idx] = (unsigned short)h;
+                    }
+                    // every fourth item: at most 128 keys since the last check, so the table never
+                    // holds more than PSTRIDE + 128 < HASH keys and probing always terminates
+                    if ((item & 3) == 3) {
+                        L += __reduce_add_sync(0xffffffffu, fresh);
+                        fresh = 0;
+                        if (L > PSTRIDE) { ovf = true; break; }
+                    }
+                }
+            }
+            L += __reduce_add_sync(0xffffffffu, fresh);
+            if (L > PSTRIDE) ovf = true;
+        }
+        if (ovf) {
             if (lane == 0) {
                 blen[I] = 0;
                 const unsigned long long slot = atomicAdd((unsigned long long*)&flags[FLAG_OVF_ROWS], 1ull);
@@ -158,15 +246,66 @@ brow_fast_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t* 
             __syncwarp();
             continue;
         }
-        table_to_sorted_list<HASH>(table, list, L);
+        __syncwarp();
+        // ---- compact, sort in registers, park the row
+        {
+            int base = 0;
+            for (int i0 = 0; i0 < HASH; i0 += 32) {
+                const int v = table[i0 + lane];
+                const unsigned m = __ballot_sync(0xffffffffu, v >= 0);
+                if (v >= 0) list[base + __popc(m & ((1u << lane) - 1))] = v;
+                base += __popc(m);
+            }
+            for (int i = L + lane; i < PSTRIDE; i += 32) list[i] = 0x7FFFFFFF;
+            __syncwarp();
+            int v[NPL];
+#pragma unroll
+            for (int r = 0; r < NPL; ++r) v[r] = list[lane * NPL + r];
+            warp_sort_regs<NPL>(v);
+            __syncwarp();
+#pragma unroll
+            for (int r = 0; r < NPL; ++r) list[lane * NPL + r] = v[r];
+            __syncwarp();
+        }
         int32_t* dst = pool + I * PSTRIDE;
-        for (int i = lane; i < L; i += 32) {
-            const int c = list[i];
-            dst[i] = c;
-            if (c == (int)I) bdiag[I] = i;
+        for (int s = lane; s < L; s += 32) {
+            const int c = list[s];
+            dst[s] = c;
+            if (c == (int)I) bdiag[I] = s;
+            if (masks) {   // the table entry of this key learns its slot
+                unsigned h = pat_hash<HASH>(c);
+                while (table[h] != c) h = (h + 1) & (HASH - 1);
+                tslot[h] = (unsigned short)s;
+            }
         }
         if (lane == 0) blen[I] = L;
+        if (!masks) continue;
         __syncwarp();
+        // ---- slot masks: bit (slot of node J) for every support node J of every incident point
+        unsigned* mdst = masks + pa * NPL;
+        for (int t = 0; t < np; ++t) {
+            if (lane < NPL) mw[lane] = 0u;
+            __syncwarp();
+            for (int ps = 0; ps < npass; ++ps) {
+                const int j = ps * 32 + lane;
+                if (j < k) {
+                    const int idx = t * kpad + j;
+                    unsigned h;
+                    if (idx < HP_CAP) {
+                        h = hp[idx];
+                    } else {
+                        const int key = support[(int64_t)inc_q[pa + t] * k + j];
+                        h = pat_hash<HASH>(key);
+                        while (table[h] != key) h = (h + 1) & (HASH - 1);
+                    }
+                    const unsigned slot = tslot[h];
+                    atomicOr(&mw[slot >> 5], 1u << (slot & 31));
+                }
+            }
+            __syncwarp();
+            if (lane < NPL) mdst[(int64_t)t * NPL + lane] = mw[lane];
+            __syncwarp();
+        }
     }
 }
 
@@ -314,12 +453,15 @@ int rpim_stage_incidence(rpim_ctx* ctx) {
 
 namespace {
 template <int HASH, int PSTRIDE>
-int launch_brow_fast(rpim_ctx* ctx, int32_t* d_pool, int32_t* d_ovf_rows) {
+int launch_brow_fast(rpim_ctx* ctx, int32_t* d_pool, int32_t* d_ovf_rows, unsigned* d_masks) {
     const int64_t N = ctx->N;
+    auto kern = brow_fast_kernel<HASH, PSTRIDE>;
+    const size_t smem = (size_t)PAT_FAST_WARPS * (HASH + PSTRIDE + HASH / 2 + HP_CAP / 2 + 32) * sizeof(int);
+    CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const unsigned nb = (unsigned)std::min<int64_t>((N + PAT_FAST_WARPS - 1) / PAT_FAST_WARPS, 148 * 16);
-    brow_fast_kernel<HASH, PSTRIDE><<<nb, PAT_FAST_WARPS * 32, 0, ctx->stream>>>(
-        N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->k, ctx->d_blen, d_pool, ctx->d_bdiag, d_ovf_rows,
-        ctx->d_flags);
+    kern<<<nb, PAT_FAST_WARPS * 32, smem, ctx->stream>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->k,
+                                                         ctx->d_blen, d_pool, ctx->d_bdiag, d_ovf_rows, d_masks,
+                                                         ctx->d_flags);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
 }
@@ -343,6 +485,7 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
     // Fast path when the expected row length (about 5..8 supports' worth of columns) fits the
     // pool stride; pstride = 0 selects the general two-pass path for every row.
     const int pstride = (8 * ctx->k <= 256) ? 256 : (8 * ctx->k <= 512) ? 512 : 0;
+    int masks_stride = 0;
     int32_t *d_pool = nullptr, *d_ovf_rows = nullptr;
     uint8_t* d_is_ovf = nullptr;
     auto drop_tmp = [&]() { ws_free(ctx, &d_pool); ws_free(ctx, &d_ovf_rows); ws_free(ctx, &d_is_ovf); };
@@ -358,8 +501,29 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
             (rc = ws_alloc(ctx, &d_is_ovf, N))) { drop_tmp(); return rc; }
         CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_OVF_ROWS, 0, sizeof(long long), st));
         CUDA_TRY(ctx, cudaMemsetAsync(d_is_ovf, 0, (size_t)N, st));
-        rc = (pstride == 256) ? launch_brow_fast<512, 256>(ctx, d_pool, d_ovf_rows)
-                              : launch_brow_fast<1024, 512>(ctx, d_pool, d_ovf_rows);
+        // slot masks of the reduction ride along (fixed stride of pstride / 32 words per incident
+        // point); they are an accelerator: skipped when they would take more than a quarter of the
+        // free device memory
+        unsigned* d_masks = nullptr;
+        {
+            const int64_t words = ctx->Nq * (int64_t)ctx->k * (pstride / 32);
+            const int64_t bytes = words * (int64_t)sizeof(unsigned);
+            size_t free_b = 0, total_b = 0;
+            CUDA_TRY(ctx, cudaMemGetInfo(&free_b, &total_b));
+            bool reuse = false;   // a block we already own does not count against the budget
+            for (auto& b : ctx->ws_cache) reuse = reuse || (b.second >= bytes && b.second <= 2 * bytes + 4096);
+            if (ctx->d_masks) {
+                auto it = ctx->ws_sizes.find((void*)ctx->d_masks);
+                reuse = reuse || (it != ctx->ws_sizes.end() && it->second >= bytes && it->second <= 2 * bytes + 4096);
+            }
+            if (reuse || (uint64_t)bytes <= free_b / 4) {
+                if (ws_alloc(ctx, &ctx->d_masks, words) == RPIM_OK) d_masks = ctx->d_masks;
+                else ctx->err.clear();
+            }
+        }
+        rc = (pstride == 256) ? launch_brow_fast<512, 256>(ctx, d_pool, d_ovf_rows, d_masks)
+                              : launch_brow_fast<1024, 512>(ctx, d_pool, d_ovf_rows, d_masks);
+        masks_stride = d_masks ? pstride / 32 : 0;
         if (rc) { drop_tmp(); return rc; }
         mark_rows_kernel<<<64, 256, 0, st>>>(d_ovf_rows, d_novf, d_is_ovf);
         KERNEL_CHECK(ctx);
@@ -396,6 +560,9 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
         RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "pattern: %lld block rows are longer than %d", h_flags[FLAG_PAT_CAP],
                   PAT_MAXROW);
     }
+    // the ride-along masks are complete only if no row took the general path
+    ctx->have_masks = masks_stride > 0 && h_flags[FLAG_OVF_ROWS] == 0;
+    ctx->mask_stride = ctx->have_masks ? masks_stride : 0;
     if ((rc = ws_alloc(ctx, &ctx->d_bcol, ctx->nnzb))) { drop_tmp(); return rc; }
     if (pstride) {
         rc = (pstride == 256) ? launch_brow_copy<256>(ctx, d_pool, d_is_ovf) : launch_brow_copy<512>(ctx, d_pool, d_is_ovf);
@@ -496,7 +663,8 @@ slot_mask_kernel(int64_t N, int k, const int64_t* __restrict__ inc_ptr, const in
 int rpim_stage_slot_masks(rpim_ctx* ctx) {
     cudaStream_t st = ctx->stream;
     const int64_t N = ctx->N;
-    ctx->have_masks = false;
+    if (ctx->have_masks) return RPIM_OK;   // built together with the block rows (fixed stride)
+    ctx->mask_stride = 0;
     if (ctx->max_blen > 1024 || ctx->max_blen < 1) return RPIM_OK;   // such rows take the generic reduction
     int rc;
     int* d_cnt = nullptr;

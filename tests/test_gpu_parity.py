@@ -88,6 +88,25 @@ def test_run_to_run_bitwise_determinism_and_index_width():
     assert a["launches"] > 0
 
 
+def test_shuffled_node_numbering():
+    # 69,120 nodes numbered at random (no spatial coherence of the ids: hash tables, incidence lists and
+    # the cell grid must not rely on it; also the largest parity case the oracle finishes in seconds).
+    # Same bars as everywhere else.
+    w = workloads.make_block("shuf", 48, 40, 36, 1.0, 1, 8, 5e9, 0.3, jitter=0.3, seed=77,
+                             body=(0.0, 0.0, -2.5e4), bc="bottom")
+    rng = np.random.default_rng(5)
+    perm = rng.permutation(w.N)                 # new id i holds old node perm[i]
+    inv = np.empty_like(perm)
+    inv[perm] = np.arange(w.N)
+    w.nodes = np.ascontiguousarray(w.nodes[perm])
+    nb = inv[w.bc_nodes]
+    order = np.argsort(nb)
+    w.bc_nodes = np.ascontiguousarray(nb[order]).astype(np.int64)
+    w.bc_mask = np.ascontiguousarray(w.bc_mask[order])
+    w.bc_ubar = np.ascontiguousarray(w.bc_ubar[order])
+    _compare(w, run_cuda(w), run_oracle(w))
+
+
 def test_planar_cloud_every_point_is_singular():
     nodes = np.array([[i, j, 0.0] for j in range(6) for i in range(6)], dtype=np.float64)
     w = workloads.make_block("flat", 6, 6, 2, 1.0, 1, 12, 1e9, 0.3)

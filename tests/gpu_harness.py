@@ -77,3 +77,83 @@ def kmax_diag(o):
     rp_, ci, v = o["row_ptr"], o["col_idx"], o["vals0"]
     rows = np.repeat(np.arange(len(rp_) - 1), np.diff(rp_))
     return np.abs(v[rows == ci]).max()
+
+
+def run_cuda_rows(w, slabs, *, want_shape=True):
+    """Full-size run of the CUDA path in the launch configuration bench.py times; brings back only
+    what the sampled checks need: for every node slab [lo, hi) the CSR rows, values (before and after
+    the penalty) and load entries, plus the ids, supports and shape functions of the quadrature points
+    incident to the slab."""
+    import torch
+    import paper_1802_04256_b200 as rp
+
+    dev = torch.device("cuda:0")
+    out = {"slabs": []}
+    with rp.Context(0) as ctx:
+        d_nodes = torch.from_numpy(w.nodes).to(dev)
+        d_qpts = torch.from_numpy(w.qpts).to(dev)
+        d_qw = torch.from_numpy(w.qw).to(dev)
+        nnz, bits = ctx.build_pattern(d_nodes, d_qpts, w.k, w.index_bits)
+        idt = torch.int32 if bits == 32 else torch.int64
+        d_rp = torch.empty(3 * w.N + 1, dtype=idt, device=dev)
+        d_ci = torch.empty(nnz, dtype=idt, device=dev)
+        d_sup = torch.empty((w.Nq, w.k), dtype=torch.int32, device=dev)
+        ctx.get_pattern(d_rp, d_ci, d_sup)
+        d_vals = torch.full((nnz,), float("nan"), dtype=torch.float64, device=dev)
+        d_f = torch.full((3 * w.N,), float("nan"), dtype=torch.float64, device=dev)
+        nsing = ctx.assemble(d_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f)
+        out.update(nnz=nnz, bits=bits, nsing=nsing)
+        # pattern-wide properties that hold at any size (cheap on the device)
+        rp64 = d_rp.to(torch.int64)
+        out["row_ptr_monotone"] = bool((rp64[1:] >= rp64[:-1]).all().item()) and int(rp64[0]) == 0 and int(rp64[-1]) == nnz
+        out["support_sorted"] = bool((d_sup[:, 1:] > d_sup[:, :-1]).all().item())
+        del rp64
+        pts_of = []
+        for lo, hi in slabs:
+            parts = []   # in chunks of points: the temporaries stay small next to a 170 GB problem
+            for c0 in range(0, w.Nq, 1 << 20):
+                blk = d_sup[c0:c0 + (1 << 20)]
+                parts.append(torch.nonzero(((blk >= lo) & (blk < hi)).any(dim=1)).flatten() + c0)
+            ids = torch.cat(parts)
+            pts_of.append(ids)
+            a, b = int(d_rp[3 * lo]), int(d_rp[3 * hi])
+            out["slabs"].append(dict(lo=lo, hi=hi, q=ids.cpu().numpy(), support=d_sup[ids].cpu().numpy(),
+                                     row_ptr=(d_rp[3 * lo:3 * hi + 1].to(torch.int64) - a).cpu().numpy(),
+                                     col_idx=d_ci[a:b].to(torch.int64).cpu().numpy(),
+                                     vals0=d_vals[a:b].cpu().numpy(), f0=d_f[3 * lo:3 * hi].cpu().numpy(), a=a, b=b))
+        if want_shape:
+            d_phi = torch.empty((w.Nq, w.k), dtype=torch.float64, device=dev)
+            d_dphi = torch.empty((w.Nq, 3, w.k), dtype=torch.float64, device=dev)
+            ctx.get_shape(d_phi, d_dphi, None)
+            for s, ids in zip(out["slabs"], pts_of):
+                s["phi"] = d_phi[ids].cpu().numpy()
+                s["dphi"] = d_dphi[ids].cpu().numpy()
+            del d_phi, d_dphi
+        out["alpha"] = ctx.apply_penalty(torch.from_numpy(w.bc_nodes).to(dev), torch.from_numpy(w.bc_mask).to(dev),
+                                         torch.from_numpy(w.bc_ubar).to(dev), w.penalty_alpha, True, d_vals, d_f)
+        for s in out["slabs"]:
+            s["vals"] = d_vals[s["a"]:s["b"]].cpu().numpy()
+            s["f"] = d_f[3 * s["lo"]:3 * s["hi"]].cpu().numpy()
+        out["launches"] = ctx.launch_count()
+        del d_vals, d_ci, d_rp, d_sup, d_f
+    torch.cuda.empty_cache()
+    return out
+
+
+def oracle_rows(w, slab):
+    """The oracle on the same slab: supports of the incident points (its own grid search over ALL nodes),
+    the CSR rows of the slab's nodes, their values and load entries (row-slab mode of the oracle)."""
+    import oracle
+
+    lo, hi = slab["lo"], slab["hi"]
+    q = slab["q"]
+    pts, qw = np.ascontiguousarray(w.qpts[q]), np.ascontiguousarray(w.qw[q])
+    s = oracle.knn(w.nodes, pts, w.k, "grid")
+    rp_, ci = oracle.pattern(s, w.N)               # complete for the slab's rows: every incident point is in q
+    a, b = rp_[3 * lo], rp_[3 * hi]
+    rows_rp = rp_[3 * lo:3 * hi + 1] - a
+    rows_ci = ci[a:b]
+    phi, dphi, sing = oracle.shape(w.nodes, pts, s, w.alpha_c, w.d_c, w.q)
+    vals, f, ns = oracle.assemble(w.nodes, pts, qw, s, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, rows_rp, rows_ci,
+                                  node_lo=lo, node_hi=hi)
+    return dict(support=s, row_ptr=rows_rp, col_idx=rows_ci, phi=phi, dphi=dphi, vals0=vals, f0=f, nsing=ns)

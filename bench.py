@@ -162,6 +162,35 @@ def oracle_sample_rate(w, budget_s: float = 15.0):
     return S / t, S, t
 
 
+def rank_workload(config_name: str, rank: int, world: int):
+    """The partition rank `rank` assembles.  The path shards by spatial partition (quadrature points are
+    independent; K is row-partitionable) with no data-path collective: under weak scaling every
+    rank gets a block of the config's size with its own jitter stream (seed + 1000 * rank)."""
+    w = workloads.config(config_name)
+    if world > 1 and w.meta.get("jitter", 0.0) > 0:
+        nx, ny, nz = w.grid
+        w = workloads.make_block(w.name, nx, ny, nz, w.h, w.meta["gauss"], w.k, w.E, w.nu, jitter=w.meta["jitter"],
+                                 seed=int(w.meta.get("seed", 0)) + 1000 * rank, body=tuple(w.body), bc=w.meta["bc"],
+                                 index_bits=w.index_bits)
+    return w
+
+
+def max_over_ranks(ms_local: float, world: int, device=None) -> float:
+    """Device-timed milliseconds of this rank -> the job's time (the slowest rank's)."""
+    if world <= 1:
+        return float(ms_local)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(points_per_rank: int, world: int, ms_step: float) -> float:
+    """Whole-job throughput: the quadrature points all ranks processed per second."""
+    return world * points_per_rank / (ms_step * 1e-3)
+
+
 def run_reference(args, w):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -206,14 +235,7 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
 
-    w = workloads.config(args.config)
-    if world > 1:
-        # weak scaling: every rank assembles its own partition (same size, its own jitter stream)
-        seed = int(w.meta.get("seed", 0)) + 1000 * rank
-        if w.meta.get("jitter", 0.0) > 0:
-            nx, ny, nz = w.grid
-            w = workloads.make_block(w.name, nx, ny, nz, w.h, w.meta["gauss"], w.k, w.E, w.nu, jitter=w.meta["jitter"],
-                                     seed=seed, body=tuple(w.body), bc=w.meta["bc"], index_bits=w.index_bits)
+    w = rank_workload(args.config, rank, world)
 
     if args.impl == "reference":
         run_reference(args, w)
@@ -279,12 +301,9 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     launches = ctx.launch_count() - launches0
     phase_ms, calls = ctx.phase_totals(reset=True)
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, world, dev)
     ms_step = ms_total / args.steps
-    value = world * w.Nq / (ms_step * 1e-3)
+    value = job_value(w.Nq, world, ms_step)
 
     # assemble + penalty only (paper stages 1 + 2), same timing discipline
     barrier()
@@ -364,10 +383,7 @@ def main():
             e1.record(stream)
             barrier()
             ms_e2e = e0.elapsed_time(e1) / n_e2e
-            if world > 1:
-                t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                ms_e2e = float(t.item())
+            ms_e2e = max_over_ranks(ms_e2e, world, dev)
             h2d = h_nodes.nbytes + h_qpts.nbytes + h_qw.nbytes + h_bcn.nbytes + h_bcm.nbytes + h_bcu.nbytes
             d2h = h_rp.nbytes + h_ci.nbytes + h_vals.nbytes + h_f.nbytes
             e2e = {"value": world * w.Nq / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),

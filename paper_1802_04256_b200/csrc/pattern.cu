@@ -71,7 +71,6 @@ inc_sort_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, int32_t* __restr
 constexpr int PAT_HASH = 4096;          // general path: open-addressing table per warp (power of two)
 constexpr int PAT_MAXROW = 2048;        // longest block row handled
 constexpr int PAT_WARPS = 4;
-constexpr int PAT_FAST_WARPS = 8;
 
 template <int HASH>
 __device__ __forceinline__ unsigned pat_hash(int key) {
@@ -135,107 +134,146 @@ __device__ __forceinline__ void table_to_sorted_list(const int* table, int* list
     warp_bitonic_i32(list, np);
 }
 
-// Fast path (brow_fast_kernel): a small table (HASH entries) and ONE pass.  While the union is
-// built the table position found for every (incident point, support node) is remembered; the
-// compacted keys are sorted in REGISTERS (bitonic network, PSTRIDE / 32 keys per lane, shuffles
-// for the cross-lane strides); every table entry then learns its slot, and the slot masks of the
-// reduction (step a6) follow from the remembered positions without a second round of probing.
-// The sorted row is parked in a fixed-stride pool, lengths are scanned, rows are copied to their
-// CSR place.  Rows that do not fit go to an overflow list and take the general two-pass path.
-constexpr int HP_CAP = 2560;   // remembered table positions per row (incident points x k); beyond: re-probe
+// Fast path (brow_bitmap_kernel): the union of a row as a TWO-LEVEL BITMAP over the window of node
+// ids its supports span -- no hashing, no probing, no sort.  Level 1 has one bit per block of 64
+// consecutive ids (which blocks are touched), level 2 one 64-bit word per TOUCHED block, stored
+// compactly in block order (rank = set level-1 bits below).  Three sweeps over the (incident point,
+// support node) pairs: mark blocks, mark ids, and -- once prefix popcounts are known -- turn every
+// support node into its column slot (set bits below it), which gives the slot masks of the
+// reduction (step a6) in the same pass.  The sorted row is the set bits in order.  With a
+// spatially coherent numbering the window is a few z-planes of ids; rows whose window, number of
+// touched blocks or length does not fit go to the overflow list and take the general path.
+constexpr int B1W = 320;      // level-1 words per warp: windows of up to 320 * 32 * 32 = 327,680 node ids
+constexpr int B2CAP = 512;    // touched 32-id blocks per row
+constexpr int BM_WARPS = 8;
+constexpr int BM_PER_WARP = B1W + B1W / 2 + B2CAP + B2CAP / 2 + 32;   // 32-bit words of shared memory
 
-// ascending bitonic sort of 32 * NPL keys, key e = lane * NPL + r held in v[r]
-template <int NPL>
-__device__ __forceinline__ void warp_sort_regs(int (&v)[NPL]) {
-    const int lane = lane_id();
-#pragma unroll
-    for (int size = 2; size <= 32 * NPL; size <<= 1) {
-#pragma unroll
-        for (int stride = size >> 1; stride > 0; stride >>= 1) {
-            if (stride >= NPL) {
-                const int ls = stride / NPL;
-                const bool lower = (lane & ls) == 0;
-#pragma unroll
-                for (int r = 0; r < NPL; ++r) {
-                    const bool up = ((lane * NPL + r) & size) == 0;
-                    const int other = __shfl_xor_sync(0xffffffffu, v[r], ls);
-                    v[r] = (lower == up) ? min(v[r], other) : max(v[r], other);
-                }
-            } else {
-#pragma unroll
-                for (int r = 0; r < NPL; ++r) {
-                    if (r & stride) continue;
-                    const bool up = ((lane * NPL + r) & size) == 0;
-                    const int a = v[r], b = v[r + stride];
-                    const int mn = min(a, b), mx = max(a, b);
-                    v[r] = up ? mn : mx;
-                    v[r + stride] = up ? mx : mn;
-                }
-            }
-        }
-    }
-}
-
-template <int HASH, int PSTRIDE>
-__global__ void __launch_bounds__(PAT_FAST_WARPS * 32)
-brow_fast_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
-                 const int32_t* __restrict__ support, int k, int* __restrict__ blen, int32_t* __restrict__ pool,
-                 int* __restrict__ bdiag, int32_t* __restrict__ ovf_rows, unsigned* __restrict__ masks,
-                 long long* __restrict__ flags) {
-    constexpr int NPL = PSTRIDE / 32;   // keys per lane in the sort = mask words per incident point
-    extern __shared__ int bf_smem[];
+template <int PSTRIDE>
+__global__ void __launch_bounds__(BM_WARPS * 32)
+brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
+                   const int32_t* __restrict__ support, int k, int* __restrict__ blen, int32_t* __restrict__ pool,
+                   int* __restrict__ bdiag, int32_t* __restrict__ ovf_rows, unsigned* __restrict__ masks,
+                   long long* __restrict__ flags) {
+    constexpr int NWS = PSTRIDE / 32;   // mask words per (row, incident point)
+    constexpr int NPASS = PSTRIDE / 256; // passes of 32 lanes over a support (8 k <= PSTRIDE)
+    constexpr unsigned FULLW = 0xffffffffu;
+    extern __shared__ unsigned bm_smem[];
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    // per warp: table[HASH] | list[PSTRIDE] | tslot[HASH] (u16) | hp[HP_CAP] (u16) | mw[32]
-    constexpr int PER_WARP = HASH + PSTRIDE + HASH / 2 + HP_CAP / 2 + 32;
-    int* table = bf_smem + (size_t)wid * PER_WARP;
-    int* list = table + HASH;
-    unsigned short* tslot = reinterpret_cast<unsigned short*>(list + PSTRIDE);
-    unsigned short* hp = reinterpret_cast<unsigned short*>(list + PSTRIDE + HASH / 2);
-    unsigned* mw = reinterpret_cast<unsigned*>(list + PSTRIDE + HASH / 2 + HP_CAP / 2);
-    const int npass = (k + 31) >> 5;
-    const int kpad = npass * 32;
-    for (int64_t I = (int64_t)blockIdx.x * PAT_FAST_WARPS + wid; I < N; I += (int64_t)gridDim.x * PAT_FAST_WARPS) {
+    unsigned* ws = bm_smem + (size_t)wid * BM_PER_WARP;
+    unsigned* l2 = ws;                                                                // [B2CAP] ids of a touched block
+    unsigned* l1 = ws + B2CAP;                                                    // [B1W] touched blocks
+    unsigned short* p1 = reinterpret_cast<unsigned short*>(l1 + B1W);                 // [B1W] touched blocks before word
+    unsigned short* p2 = reinterpret_cast<unsigned short*>(l1 + B1W + B1W / 2);       // [B2CAP] columns before block
+    unsigned* mw = l1 + B1W + B1W / 2 + B2CAP / 2;                                    // [32] mask words of one point
+    for (int64_t I = (int64_t)blockIdx.x * BM_WARPS + wid; I < N; I += (int64_t)gridDim.x * BM_WARPS) {
         const int64_t pa = inc_ptr[I], pb = inc_ptr[I + 1];
         const int np = (int)(pb - pa);
-        __syncwarp();
-        for (int i = lane; i < HASH; i += 32) table[i] = -1;
-        __syncwarp();
-        // ---- union of the supports; remember where every (point, position) landed
-        int L = 0;
-        bool ovf = false;
-        {
-            auto loadJ = [&](int t, int ps) {
-                const int j = ps * 32 + lane;
-                return (t < np && j < k) ? support[(int64_t)inc_q[pa + t] * k + j] : -1;
+        if (np == 0) {
+            if (lane == 0) blen[I] = 0;
+            continue;
+        }
+        // window of node ids: supports are ascending, so first and last entries bound each of them
+        int lo = 0x7FFFFFFF, hi = -1;
+        for (int p = lane; p < np; p += 32) {
+            const int32_t* sp = support + (int64_t)inc_q[pa + p] * k;
+            lo = min(lo, sp[0]);
+            hi = max(hi, sp[k - 1]);
+        }
+        lo = __reduce_min_sync(FULLW, lo);
+        hi = __reduce_max_sync(FULLW, hi);
+        const int base = lo & ~31;
+        const int nblk = ((hi - base) >> 5) + 1;
+        const int n1 = (nblk + 31) >> 5;
+        bool ovf = n1 > B1W;
+        int L = 0, nb2 = 0;
+        // sweep over the (incident point, support node) pairs: lane j of pass ps holds node sp[32 ps + j]
+        auto sweep = [&](auto&& body_point_begin, auto&& body, auto&& body_point_end) {
+            // software pipeline: the point id two points ahead, the support nodes one point ahead
+            // (PSTRIDE = 256 serves k <= 32: one pass of 32 lanes; PSTRIDE = 512 serves k <= 64: two)
+            auto fetch = [&](int q, bool valid, int (&J)[NPASS]) {
+#pragma unroll
+                for (int ps = 0; ps < NPASS; ++ps) {
+                    const int j = ps * 32 + lane;
+                    J[ps] = (valid && j < k) ? support[(int64_t)q * k + j] : -1;
+                }
             };
-            int Jnext = loadJ(0, 0);
-            int fresh = 0, item = 0;
-            for (int t = 0; t < np && !ovf; ++t) {
-                for (int ps = 0; ps < npass; ++ps, ++item) {
-                    const int key = Jnext;
-                    Jnext = (ps + 1 < npass) ? loadJ(t, ps + 1) : loadJ(t + 1, 0);
-                    if (key >= 0) {
-                        unsigned h = pat_hash<HASH>(key);
-                        while (true) {
-                            const int old = atomicCAS(&table[h], -1, key);
-                            if (old == -1) { ++fresh; break; }
-                            if (old == key) break;
-                            h = (h + 1) & (HASH - 1);
-                        }
-                        const int idx = item * 32 + lane;   // = t * kpad + j
-                        if (idx < HP_CAP) hp[idx] = (unsigned short)h;
-                    }
-                    // every fourth item: at most 128 keys since the last check, so the table never
-                    // holds more than PSTRIDE + 128 < HASH keys and probing always terminates
-                    if ((item & 3) == 3) {
-                        L += __reduce_add_sync(0xffffffffu, fresh);
-                        fresh = 0;
-                        if (L > PSTRIDE) { ovf = true; break; }
-                    }
+            int q_n = (np > 1) ? inc_q[pa + 1] : 0;
+            int J_c[NPASS], J_n[NPASS];
+            fetch(inc_q[pa], true, J_c);
+            for (int t = 0; t < np; ++t) {
+                const int q_nn = (t + 2 < np) ? inc_q[pa + t + 2] : 0;
+                fetch(q_n, t + 1 < np, J_n);
+                body_point_begin(t);
+#pragma unroll
+                for (int ps = 0; ps < NPASS; ++ps)
+                    if (J_c[ps] >= 0) body(J_c[ps]);
+                body_point_end(t);
+                q_n = q_nn;
+#pragma unroll
+                for (int ps = 0; ps < NPASS; ++ps) J_c[ps] = J_n[ps];
+            }
+        };
+        auto nop = [](int) {};
+        // exclusive prefix of a per-lane count over the warp; returns (prefix, total)
+        auto warp_excl = [&](int cnt, int& total) {
+            int incl = cnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int up = __shfl_up_sync(FULLW, incl, d);
+                if (lane >= d) incl += up;
+            }
+            total = __shfl_sync(FULLW, incl, 31);
+            return incl - cnt;
+        };
+        if (!ovf) {
+            __syncwarp();
+            for (int w = lane; w < n1; w += 32) l1[w] = 0u;
+            __syncwarp();
+            // ---- sweep A: touched blocks
+            sweep(nop, [&](int J) {
+                const int b = (J - base) >> 5;
+                atomicOr(&l1[b >> 5], 1u << (b & 31));
+            }, nop);
+            __syncwarp();
+            const int C1 = (n1 + 31) >> 5;   // level-1 words per lane: lane owns [lane C1, lane C1 + C1)
+            {
+                int cnt = 0;
+                for (int i = 0; i < C1; ++i) {
+                    const int w = lane * C1 + i;
+                    if (w < n1) cnt += __popc(l1[w]);
+                }
+                int pre = warp_excl(cnt, nb2);
+                for (int i = 0; i < C1; ++i) {
+                    const int w = lane * C1 + i;
+                    if (w < n1) { p1[w] = (unsigned short)pre; pre += __popc(l1[w]); }
                 }
             }
-            L += __reduce_add_sync(0xffffffffu, fresh);
-            if (L > PSTRIDE) ovf = true;
+            ovf = nb2 > B2CAP;
+            if (!ovf) {
+                for (int r = lane; r < nb2; r += 32) l2[r] = 0u;
+                __syncwarp();
+                // ---- sweep B: ids inside the touched blocks
+                sweep(nop, [&](int J) {
+                    const int d = J - base, b = d >> 5;
+                    const int r = p1[b >> 5] + __popc(l1[b >> 5] & ((1u << (b & 31)) - 1u));
+                    atomicOr(&l2[r], 1u << (d & 31));
+                }, nop);
+                __syncwarp();
+                const int C2 = (nb2 + 31) >> 5;
+                {
+                    int cnt = 0;
+                    for (int i = 0; i < C2; ++i) {
+                        const int r = lane * C2 + i;
+                        if (r < nb2) cnt += __popc(l2[r]);
+                    }
+                    int pre = warp_excl(cnt, L);
+                    for (int i = 0; i < C2; ++i) {
+                        const int r = lane * C2 + i;
+                        if (r < nb2) { p2[r] = (unsigned short)pre; pre += __popc(l2[r]); }
+                    }
+                }
+                ovf = L > PSTRIDE;
+            }
         }
         if (ovf) {
             if (lane == 0) {
@@ -246,65 +284,50 @@ brow_fast_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t* 
             __syncwarp();
             continue;
         }
-        __syncwarp();
-        // ---- compact, sort in registers, park the row
+        __syncwarp();   // p1, p2 complete
+        // ---- the sorted row: set bits in order (lane owns a run of level-1 words)
         {
-            int base = 0;
-            for (int i0 = 0; i0 < HASH; i0 += 32) {
-                const int v = table[i0 + lane];
-                const unsigned m = __ballot_sync(0xffffffffu, v >= 0);
-                if (v >= 0) list[base + __popc(m & ((1u << lane) - 1))] = v;
-                base += __popc(m);
-            }
-            for (int i = L + lane; i < PSTRIDE; i += 32) list[i] = 0x7FFFFFFF;
-            __syncwarp();
-            int v[NPL];
-#pragma unroll
-            for (int r = 0; r < NPL; ++r) v[r] = list[lane * NPL + r];
-            warp_sort_regs<NPL>(v);
-            __syncwarp();
-#pragma unroll
-            for (int r = 0; r < NPL; ++r) list[lane * NPL + r] = v[r];
-            __syncwarp();
-        }
-        int32_t* dst = pool + I * PSTRIDE;
-        for (int s = lane; s < L; s += 32) {
-            const int c = list[s];
-            dst[s] = c;
-            if (c == (int)I) bdiag[I] = s;
-            if (masks) {   // the table entry of this key learns its slot
-                unsigned h = pat_hash<HASH>(c);
-                while (table[h] != c) h = (h + 1) & (HASH - 1);
-                tslot[h] = (unsigned short)s;
+            const int C1 = (n1 + 31) >> 5;
+            int32_t* dst = pool + I * PSTRIDE;
+            for (int i = 0; i < C1; ++i) {
+                const int w = lane * C1 + i;
+                if (w >= n1) break;
+                unsigned bits = l1[w];
+                int r = p1[w];
+                while (bits) {
+                    const int blk = 32 * w + __ffs(bits) - 1;
+                    bits &= bits - 1;
+                    unsigned ids = l2[r];
+                    int pre = p2[r];
+                    while (ids) {
+                        const int key = base + 32 * blk + __ffs(ids) - 1;
+                        ids &= ids - 1;
+                        dst[pre] = key;
+                        if (key == (int)I) bdiag[I] = pre;
+                        ++pre;
+                    }
+                    ++r;
+                }
             }
         }
         if (lane == 0) blen[I] = L;
         if (!masks) continue;
-        __syncwarp();
-        // ---- slot masks: bit (slot of node J) for every support node J of every incident point
-        unsigned* mdst = masks + pa * NPL;
-        for (int t = 0; t < np; ++t) {
-            if (lane < NPL) mw[lane] = 0u;
-            __syncwarp();
-            for (int ps = 0; ps < npass; ++ps) {
-                const int j = ps * 32 + lane;
-                if (j < k) {
-                    const int idx = t * kpad + j;
-                    unsigned h;
-                    if (idx < HP_CAP) {
-                        h = hp[idx];
-                    } else {
-                        const int key = support[(int64_t)inc_q[pa + t] * k + j];
-                        h = pat_hash<HASH>(key);
-                        while (table[h] != key) h = (h + 1) & (HASH - 1);
-                    }
-                    const unsigned slot = tslot[h];
-                    atomicOr(&mw[slot >> 5], 1u << (slot & 31));
-                }
-            }
-            __syncwarp();
-            if (lane < NPL) mdst[(int64_t)t * NPL + lane] = mw[lane];
-            __syncwarp();
+        // ---- sweep C: slot masks, bit (slot of node J) for every support node J of every incident point
+        {
+            unsigned* mdst = masks + pa * NWS;
+            sweep([&](int) {
+                if (lane < NWS) mw[lane] = 0u;
+                __syncwarp();
+            }, [&](int J) {
+                const int d = J - base, b = d >> 5;
+                const int r = p1[b >> 5] + __popc(l1[b >> 5] & ((1u << (b & 31)) - 1u));
+                const int slot = p2[r] + __popc(l2[r] & ((1u << (d & 31)) - 1u));
+                atomicOr(&mw[slot >> 5], 1u << (slot & 31));
+            }, [&](int t) {
+                __syncwarp();
+                if (lane < NWS) mdst[(int64_t)t * NWS + lane] = mw[lane];
+                __syncwarp();
+            });
         }
     }
 }
@@ -452,16 +475,15 @@ int rpim_stage_incidence(rpim_ctx* ctx) {
 }
 
 namespace {
-template <int HASH, int PSTRIDE>
-int launch_brow_fast(rpim_ctx* ctx, int32_t* d_pool, int32_t* d_ovf_rows, unsigned* d_masks) {
+template <int PSTRIDE>
+int launch_brow_bitmap(rpim_ctx* ctx, int32_t* d_pool, int32_t* d_ovf_rows, unsigned* d_masks) {
     const int64_t N = ctx->N;
-    auto kern = brow_fast_kernel<HASH, PSTRIDE>;
-    const size_t smem = (size_t)PAT_FAST_WARPS * (HASH + PSTRIDE + HASH / 2 + HP_CAP / 2 + 32) * sizeof(int);
+    auto kern = brow_bitmap_kernel<PSTRIDE>;
+    const size_t smem = (size_t)BM_WARPS * BM_PER_WARP * sizeof(unsigned);
     CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const unsigned nb = (unsigned)std::min<int64_t>((N + PAT_FAST_WARPS - 1) / PAT_FAST_WARPS, 148 * 16);
-    kern<<<nb, PAT_FAST_WARPS * 32, smem, ctx->stream>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->k,
-                                                         ctx->d_blen, d_pool, ctx->d_bdiag, d_ovf_rows, d_masks,
-                                                         ctx->d_flags);
+    const unsigned nb = (unsigned)std::min<int64_t>((N + BM_WARPS - 1) / BM_WARPS, 148 * 16);
+    kern<<<nb, BM_WARPS * 32, smem, ctx->stream>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->k, ctx->d_blen,
+                                                   d_pool, ctx->d_bdiag, d_ovf_rows, d_masks, ctx->d_flags);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
 }
@@ -521,8 +543,8 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
                 else ctx->err.clear();
             }
         }
-        rc = (pstride == 256) ? launch_brow_fast<512, 256>(ctx, d_pool, d_ovf_rows, d_masks)
-                              : launch_brow_fast<1024, 512>(ctx, d_pool, d_ovf_rows, d_masks);
+        rc = (pstride == 256) ? launch_brow_bitmap<256>(ctx, d_pool, d_ovf_rows, d_masks)
+                              : launch_brow_bitmap<512>(ctx, d_pool, d_ovf_rows, d_masks);
         masks_stride = d_masks ? pstride / 32 : 0;
         if (rc) { drop_tmp(); return rc; }
         mark_rows_kernel<<<64, 256, 0, st>>>(d_ovf_rows, d_novf, d_is_ovf);

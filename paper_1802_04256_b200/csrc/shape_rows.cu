@@ -40,8 +40,12 @@ struct Cfg {
     static constexpr int OFF_W = OFF_Y + 4 * K;               // N x 8 (w0, w1) per 2x2 pivot, position order
     static constexpr int OFF_L = OFF_W + 8 * N;               // N x 8 (L0, L1) per 2x2 pivot, position order
     static constexpr int CSTR = (M + 4 + 1) & ~1;
-    static constexpr int OFF_C = OFF_L + 8 * N;               // 2 x CSTR pivot column / solution broadcast
-    static constexpr int OFF_H = OFF_C + 2 * CSTR;            // 4 pivots x 2 rows x 4 head right-hand sides
+    // 2 x CSTR pivot column / solution broadcast of the 1x1 stage.  It reuses the (w0, w1) area, which
+    // is dead once the free-free rows have been loaded (a __syncwarp separates the two uses): at
+    // k = 60 this is what lets two CTAs share an SM.
+    static constexpr int OFF_C = OFF_W;
+    static_assert(2 * CSTR <= 8 * N, "broadcast area fits the (w0, w1) area");
+    static constexpr int OFF_H = OFF_L + 8 * N;               // 4 pivots x 2 rows x 4 head right-hand sides
     static constexpr int RAW = OFF_H + 32;
     static constexpr int PER_POINT = ((RAW + 15) & ~15) + 8;  // = 8 mod 16: the groups of a warp hit different banks
     static constexpr int TAB_DOUBLES = ((NITEM + 3) / 4 + 1) & ~1;
@@ -361,6 +365,7 @@ shape_rows_kernel(const double* __restrict__ nodes, const double* __restrict__ p
         });
 
         // ---- R7 (b): 1x1 pivots in order, right-looking
+        __syncwarp();   // every lane has read its (w0, w1) values: the area becomes the broadcast buffer
         double rsave[NSLOT];
 #pragma unroll
         for (int s = 0; s < NSLOT; ++s) rsave[s] = 0.0;

@@ -227,6 +227,8 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--with-solve", action="store_true",
+                    help="also time stage 3 (block SpMV, Jacobi-PCG to 1e-8) on the assembled system; extra key \"solve\"")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = max(args.warmup, 3) if os.environ.get("RPIM_BENCH_STRICT_WARMUP", "1") == "1" else args.warmup
@@ -393,6 +395,31 @@ def main():
         except Exception as ex:  # report, never fake
             e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
 
+    # ------------------------------------------------ optional: stage 3 on the assembled system
+    solve = None
+    if args.with_solve:
+        d_x = torch.randn(3 * w.N, dtype=torch.float64, device=dev)
+        d_y = torch.empty_like(d_x)
+        for _ in range(3):
+            ctx.matvec(d_vals, d_x, d_y)
+        barrier()
+        e0.record(stream)
+        for _ in range(10):
+            ctx.matvec(d_vals, d_x, d_y)
+        e1.record(stream)
+        barrier()
+        spmv_ms = e0.elapsed_time(e1) / 10
+        spmv_bytes = 8 * nnz + 4 * (nnz // 9) + 2 * 8 * 3 * w.N      # values, block columns, x and y once
+        d_u = torch.zeros(3 * w.N, dtype=torch.float64, device=dev)
+        e0.record(stream)
+        iters, rel = ctx.solve_pcg(d_vals, d_f, d_u, 1e-8, 50000)
+        e1.record(stream)
+        barrier()
+        solve = {"spmv_ms": spmv_ms, "spmv_gbs": spmv_bytes / (spmv_ms * 1e-3) / 1e9,
+                 "spmv_hbm_frac": spmv_bytes / (spmv_ms * 1e-3) / 1e9 / hbm_gbs, "spmv_algorithmic_bytes": spmv_bytes,
+                 "pcg_rel_tol": 1e-8, "pcg_iters": iters, "pcg_rel_resid": rel, "pcg_ms": e0.elapsed_time(e1)}
+        del d_x, d_y, d_u
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         r, S, t = oracle_sample_rate(w, budget_s=15.0)
@@ -416,6 +443,8 @@ def main():
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "cpu_baseline": cpu_baseline,
         }
+        if solve is not None:
+            line["solve"] = solve
         print(json.dumps(line))
     ctx.close()
     if world > 1:

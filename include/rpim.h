@@ -101,6 +101,25 @@ int rpim_apply_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* 
                        const double* d_u_bar, int64_t m, double alpha, int alpha_is_relative,
                        double* d_vals, double* d_f, double* out_alpha_used);
 
+/* Stage 3 ("solve the system ... then the stresses").
+ *
+ * rpim_matvec: y = K x with K in the layout rpim_assemble / rpim_apply_penalty leave in d_vals (the
+ * pattern is the context's).  d_x, d_y: 3N fp64.  Asynchronous.
+ *
+ * rpim_solve_pcg: conjugate gradients with Jacobi (diagonal) preconditioning on the penalised K,
+ * which is symmetric positive definite (R10).  d_u holds the initial guess on entry and
+ * the solution on exit (3N).  Stops when ||f - K u||_2 <= rel_tol * ||f||_2 (looked at every 25
+ * iterations) or after max_iter iterations; out_iters / out_rel_resid (host, may be NULL) report
+ * what was reached -- not converging is not an error.  All reductions have a fixed order: the
+ * iterates are bitwise reproducible.  Synchronises the stream.
+ *
+ * rpim_recover_stress: sigma = D B u at every quadrature point of the last rpim_assemble (its staged
+ * shape-function gradients), Voigt order xx yy zz xy yz zx, d_sigma Nq x 6 fp64.  Asynchronous. */
+int rpim_matvec(rpim_ctx* ctx, const double* d_vals, const double* d_x, double* d_y);
+int rpim_solve_pcg(rpim_ctx* ctx, const double* d_vals, const double* d_f, double* d_u, double rel_tol,
+                   int max_iter, int* out_iters, double* out_rel_resid);
+int rpim_recover_stress(rpim_ctx* ctx, const double* d_u, double E, double nu, double* d_sigma);
+
 /* Test / inspection accessor: shape functions staged by the last rpim_assemble.
  *   d_phi Nq x k, d_dphi Nq x 3 x k (d/dx, d/dy, d/dz), d_singular Nq bytes; any may be NULL. */
 int rpim_get_shape(rpim_ctx* ctx, double* d_phi, double* d_dphi, uint8_t* d_singular);

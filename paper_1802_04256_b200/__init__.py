@@ -21,6 +21,9 @@ from .binding import (  # noqa: F401
     rpim_last_phase_ms,
     rpim_phase_totals,
     rpim_launch_count,
+    rpim_matvec,
+    rpim_solve_pcg,
+    rpim_recover_stress,
     rpim_workspace_bytes,
     rpim_last_error,
     EXPORTED_SYMBOLS,

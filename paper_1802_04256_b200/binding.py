@@ -17,6 +17,7 @@ EXPORTED_SYMBOLS = (
     "rpim_create", "rpim_destroy", "rpim_last_error", "rpim_workspace_bytes", "rpim_build_pattern",
     "rpim_get_pattern", "rpim_assemble", "rpim_add_point_loads", "rpim_apply_penalty", "rpim_get_shape",
     "rpim_host_pattern", "rpim_host_assemble", "rpim_last_phase_ms", "rpim_phase_totals", "rpim_launch_count",
+    "rpim_matvec", "rpim_solve_pcg", "rpim_recover_stress",
 )
 
 
@@ -62,6 +63,9 @@ def _load():
                                        C.c_int, vp, vp, vp, vp, C.POINTER(i64), C.POINTER(dbl)]
     lib.rpim_last_phase_ms.argtypes = [vp, C.POINTER(C.c_float)]
     lib.rpim_phase_totals.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64), C.c_int]
+    lib.rpim_matvec.argtypes = [vp, vp, vp, vp]
+    lib.rpim_solve_pcg.argtypes = [vp, vp, vp, vp, dbl, C.c_int, C.POINTER(C.c_int), C.POINTER(dbl)]
+    lib.rpim_recover_stress.argtypes = [vp, vp, dbl, dbl, vp]
     _lib = lib
     return lib
 
@@ -105,6 +109,28 @@ def rpim_destroy(ctx):
 
 def rpim_last_error(ctx) -> str:
     return (_load().rpim_last_error(ctx) or b"").decode()
+
+
+def rpim_matvec(ctx, d_vals, d_x, d_y):
+    import torch
+    _check(ctx, _load().rpim_matvec(ctx, _dptr(d_vals, torch.float64), _dptr(d_x, torch.float64),
+                                    _dptr(d_y, torch.float64)))
+
+
+def rpim_solve_pcg(ctx, d_vals, d_f, d_u, rel_tol=1e-10, max_iter=10000):
+    """Returns (iterations, relative residual reached)."""
+    import torch
+    it, rel = C.c_int(0), C.c_double(0.0)
+    _check(ctx, _load().rpim_solve_pcg(ctx, _dptr(d_vals, torch.float64), _dptr(d_f, torch.float64),
+                                       _dptr(d_u, torch.float64), float(rel_tol), int(max_iter), C.byref(it),
+                                       C.byref(rel)))
+    return it.value, rel.value
+
+
+def rpim_recover_stress(ctx, d_u, E, nu, d_sigma):
+    import torch
+    _check(ctx, _load().rpim_recover_stress(ctx, _dptr(d_u, torch.float64), float(E), float(nu),
+                                            _dptr(d_sigma, torch.float64)))
 
 
 def rpim_workspace_bytes(ctx) -> int:
@@ -255,6 +281,15 @@ class Context:
 
     def phase_totals(self, reset=False):
         return rpim_phase_totals(self.ctx, reset)
+
+    def matvec(self, d_vals, d_x, d_y):
+        return rpim_matvec(self.ctx, d_vals, d_x, d_y)
+
+    def solve_pcg(self, d_vals, d_f, d_u, rel_tol=1e-10, max_iter=10000):
+        return rpim_solve_pcg(self.ctx, d_vals, d_f, d_u, rel_tol, max_iter)
+
+    def recover_stress(self, d_u, E, nu, d_sigma):
+        return rpim_recover_stress(self.ctx, d_u, E, nu, d_sigma)
 
     def launch_count(self):
         return rpim_launch_count(self.ctx)

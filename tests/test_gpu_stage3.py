@@ -1,0 +1,102 @@
+"""-m gpu parity of stage 3: rpim_matvec, rpim_solve_pcg (Jacobi-PCG) and
+rpim_recover_stress against oracle/stage3.py (sparse direct solve, literal B and D) on the oracle's own K.
+
+Tolerances: the product is compared at 1e-12 of max|K x|; the solution at 1e-6 of
+max|u| (PCG stops at a relative residual of 1e-12, the Jacobi-scaled penalised matrices of these cases
+have condition numbers of 1e4..1e5); stresses at 1e-6 of max|sigma|."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+def _gpu(w, with_loads=False):
+    import torch
+    import paper_1802_04256_b200 as rp
+
+    dev = torch.device("cuda:0")
+    out = {}
+    with rp.Context(0) as ctx:
+        d_nodes, d_qpts, d_qw = (torch.from_numpy(a).to(dev) for a in (w.nodes, w.qpts, w.qw))
+        nnz, bits = ctx.build_pattern(d_nodes, d_qpts, w.k, w.index_bits)
+        d_vals = torch.empty(nnz, dtype=torch.float64, device=dev)
+        d_f = torch.empty(3 * w.N, dtype=torch.float64, device=dev)
+        ctx.assemble(d_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f)
+        if with_loads:
+            ctx.add_point_loads(torch.from_numpy(w.load_pts).to(dev), torch.from_numpy(w.load_w).to(dev),
+                                torch.from_numpy(w.load_t).to(dev), d_f)
+        ctx.apply_penalty(torch.from_numpy(w.bc_nodes).to(dev), torch.from_numpy(w.bc_mask).to(dev),
+                          torch.from_numpy(w.bc_ubar).to(dev), w.penalty_alpha, True, d_vals, d_f)
+        rng = np.random.default_rng(1)
+        x = rng.standard_normal(3 * w.N)
+        d_y = torch.empty(3 * w.N, dtype=torch.float64, device=dev)
+        ctx.matvec(d_vals, torch.from_numpy(x).to(dev), d_y)
+        out["x"], out["y"] = x, d_y.cpu().numpy()
+        d_u = torch.zeros(3 * w.N, dtype=torch.float64, device=dev)
+        out["iters"], out["relres"] = ctx.solve_pcg(d_vals, d_f, d_u, 1e-12, 50000)
+        u1 = d_u.cpu().numpy()
+        d_u.zero_()
+        ctx.solve_pcg(d_vals, d_f, d_u, 1e-12, 50000)
+        out["u"], out["u_again"] = u1, d_u.cpu().numpy()
+        d_sig = torch.empty((w.Nq, 6), dtype=torch.float64, device=dev)
+        ctx.recover_stress(d_u, w.E, w.nu, d_sig)
+        out["sigma"] = d_sig.cpu().numpy()
+    return out
+
+
+def _oracle(w, with_loads=False):
+    import oracle
+    from oracle import stage3
+
+    s = oracle.knn(w.nodes, w.qpts, w.k, "grid")
+    rp_, ci = oracle.pattern(s, w.N)
+    vals, f, _ = oracle.assemble(w.nodes, w.qpts, w.qw, s, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, rp_, ci)
+    if with_loads:
+        ls = oracle.knn(w.nodes, w.load_pts, w.k, "grid")
+        oracle.point_loads(w.nodes, w.load_pts, w.load_w, w.load_t, ls, w.alpha_c, w.d_c, w.q, f)
+    oracle.penalty(w.bc_nodes, w.bc_mask, w.bc_ubar, w.penalty_alpha, True, w.N, rp_, ci, vals, f)
+    u = stage3.solve(rp_, ci, vals, f)
+    _, dphi, _ = oracle.shape(w.nodes, w.qpts, s, w.alpha_c, w.d_c, w.q)
+    return dict(rp=rp_, ci=ci, vals=vals, f=f, u=u, sigma=stage3.stress(s, dphi, u, w.E, w.nu))
+
+
+def _compare(w, g, o):
+    from oracle import stage3
+    y = stage3.matvec(o["rp"], o["ci"], o["vals"], g["x"])
+    assert np.abs(g["y"] - y).max() <= 1e-12 * np.abs(y).max()
+    assert g["relres"] <= 1e-12 and g["iters"] > 0
+    assert np.array_equal(g["u"], g["u_again"])                               # fixed-order reductions
+    assert np.abs(g["u"] - o["u"]).max() <= 1e-6 * np.abs(o["u"]).max()
+    assert np.abs(g["sigma"] - o["sigma"]).max() <= 1e-6 * np.abs(o["sigma"]).max()
+
+
+def test_patch_solve_and_stress():
+    w = workloads.config("patch")
+    _compare(w, _gpu(w), _oracle(w))
+
+
+def test_cantilever_solve_stress_and_tip_deflection():
+    w = workloads.config("cantilever")
+    g, o = _gpu(w, True), _oracle(w, True)
+    _compare(w, g, o)
+    tip = g["u"].reshape(-1, 3)[np.isclose(w.nodes[:, 0], 10.0), 2].mean()
+    euler = -1e6 * 10.0 ** 3 / (3 * w.E / 12.0)
+    timo = euler - 1e6 * 10.0 / ((5.0 / 6.0) * w.E / (2 * (1 + w.nu)))
+    assert min(abs(tip - euler) / abs(euler), abs(tip - timo) / abs(timo)) < 0.01
+
+
+def test_gravity_column_bottom_stress_of_the_paper():
+    g0 = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "paper_example1.json")))
+    rho, grav, H, n = g0["density_kg_m3"], g0["inferred"]["g"], g0["inferred"]["height_m"], 9
+    w = workloads.make_block("cube", n, n, n, H / (n - 1), 2, 27, 20e9, 0.25, jitter=0.2, seed=4,
+                             body=(0.0, 0.0, -rho * grav), bc="bottom+roller")
+    g, o = _gpu(w), _oracle(w)
+    _compare(w, g, o)
+    low = w.qpts[:, 2] < 0.5 * H / (n - 1)
+    est = -(g["sigma"][low, 2].mean() + rho * grav * (H - w.qpts[low, 2]).mean()) + rho * grav * H
+    assert abs(est / 1e6 - g0["theoretical_bottom_stress_MPa"]) / g0["theoretical_bottom_stress_MPa"] < 0.03

@@ -33,6 +33,8 @@ void free_all(rpim_ctx* c) {
     ws_free(c, &c->d_mask_ptr); ws_free(c, &c->d_masks);
     c->have_masks = false;
     ws_free(c, &c->h2d_nodes); ws_free(c, &c->h2d_qpts);
+    ws_free(c, &c->hb_qw); ws_free(c, &c->hb_vals); ws_free(c, &c->hb_f); ws_free(c, &c->hb_ub);
+    ws_free(c, &c->hb_bn); ws_free(c, &c->hb_bm); ws_free(c, &c->hb_rp); ws_free(c, &c->hb_ci);
     { int64_t* t = (int64_t*)c->d_scan_tmp; ws_free(c, &t); c->d_scan_tmp = nullptr; c->scan_tmp_elems = 0; }
     ws_release_cache(c);
     c->have_pattern = c->have_shape = false;
@@ -70,6 +72,8 @@ int rpim_destroy(rpim_ctx* ctx) {
     if (ctx->d_flags) cudaFree(ctx->d_flags);
     for (auto& e : ctx->ev) if (e) cudaEventDestroy(e);
     for (auto& e : ctx->phase_events) cudaEventDestroy(e);
+    if (ctx->side_stream) { cudaStreamSynchronize(ctx->side_stream); cudaStreamDestroy(ctx->side_stream); }
+    for (auto& e : ctx->side_ev) if (e) cudaEventDestroy(e);
     delete ctx;
     return RPIM_OK;
 }
@@ -309,50 +313,51 @@ int rpim_host_assemble(rpim_ctx* ctx, const double* h_qw, double E, double nu, d
     cudaStream_t st = ctx->stream;
     const int64_t nnz = 9 * ctx->nnzb, n3 = 3 * ctx->N;
     const size_t iw = ctx->index_bits / 8;
-    double *d_qw = nullptr, *d_vals = nullptr, *d_f = nullptr, *d_ub = nullptr;
-    int64_t* d_bn = nullptr;
-    uint8_t* d_bm = nullptr;
-    void *d_rp = nullptr, *d_ci = nullptr;
+    // device buffers of the call live in the context's workspace (cached across calls: no cudaMalloc / cudaFree
+    // per step); the index arrays go back to the host on a side stream while the values are assembled
     int rc = RPIM_OK;
-    auto cleanup = [&]() {
-        cudaFree(d_qw); cudaFree(d_vals); cudaFree(d_f); cudaFree(d_ub); cudaFree(d_bn); cudaFree(d_bm); cudaFree(d_rp); cudaFree(d_ci);
-    };
-#define HOST_TRY(expr)                                                                           \
-    do {                                                                                         \
-        cudaError_t _e = (expr);                                                                 \
-        if (_e != cudaSuccess) {                                                                 \
-            cleanup();                                                                           \
-            RPIM_FAIL(ctx, (_e == cudaErrorMemoryAllocation ? RPIM_ERR_ALLOC : RPIM_ERR_CUDA),   \
-                      "%s failed: %s", #expr, cudaGetErrorString(_e));                           \
-        }                                                                                        \
-    } while (0)
-    HOST_TRY(cudaMalloc((void**)&d_qw, (size_t)ctx->Nq * sizeof(double)));
-    HOST_TRY(cudaMalloc((void**)&d_vals, (size_t)std::max<int64_t>(nnz, 1) * sizeof(double)));
-    HOST_TRY(cudaMalloc((void**)&d_f, (size_t)n3 * sizeof(double)));
-    HOST_TRY(cudaMemcpyAsync(d_qw, h_qw, (size_t)ctx->Nq * sizeof(double), cudaMemcpyHostToDevice, st));
+    if ((rc = ws_alloc(ctx, &ctx->hb_qw, ctx->Nq))) return rc;
+    if ((rc = ws_alloc(ctx, &ctx->hb_vals, std::max<int64_t>(nnz, 1)))) return rc;
+    if ((rc = ws_alloc(ctx, &ctx->hb_f, n3))) return rc;
     if (m > 0) {
-        HOST_TRY(cudaMalloc((void**)&d_bn, (size_t)m * sizeof(int64_t)));
-        HOST_TRY(cudaMalloc((void**)&d_ub, (size_t)3 * m * sizeof(double)));
-        HOST_TRY(cudaMemcpyAsync(d_bn, h_bc_nodes, (size_t)m * sizeof(int64_t), cudaMemcpyHostToDevice, st));
-        HOST_TRY(cudaMemcpyAsync(d_ub, h_u_bar, (size_t)3 * m * sizeof(double), cudaMemcpyHostToDevice, st));
-        if (h_bc_mask) {
-            HOST_TRY(cudaMalloc((void**)&d_bm, (size_t)m));
-            HOST_TRY(cudaMemcpyAsync(d_bm, h_bc_mask, (size_t)m, cudaMemcpyHostToDevice, st));
-        }
+        if ((rc = ws_alloc(ctx, &ctx->hb_bn, m))) return rc;
+        if ((rc = ws_alloc(ctx, &ctx->hb_ub, 3 * m))) return rc;
+        if (h_bc_mask && (rc = ws_alloc(ctx, &ctx->hb_bm, m))) return rc;
     }
-    if (h_row_ptr) HOST_TRY(cudaMalloc(&d_rp, (size_t)(n3 + 1) * iw));
-    if (h_col_idx) HOST_TRY(cudaMalloc(&d_ci, (size_t)std::max<int64_t>(nnz, 1) * iw));
-    if ((rc = rpim_get_pattern(ctx, d_rp, d_ci, nullptr))) { cleanup(); return rc; }
-    if (h_row_ptr) HOST_TRY(cudaMemcpyAsync(h_row_ptr, d_rp, (size_t)(n3 + 1) * iw, cudaMemcpyDeviceToHost, st));
-    if (h_col_idx) HOST_TRY(cudaMemcpyAsync(h_col_idx, d_ci, (size_t)nnz * iw, cudaMemcpyDeviceToHost, st));
-    if ((rc = rpim_assemble(ctx, d_qw, E, nu, alpha_c, d_c, q, body, d_vals, d_f, out_singular))) { cleanup(); return rc; }
-    if ((rc = rpim_apply_penalty(ctx, d_bn, d_bm, d_ub, m, alpha, alpha_is_relative, d_vals, d_f, out_alpha_used))) { cleanup(); return rc; }
-    HOST_TRY(cudaMemcpyAsync(h_vals, d_vals, (size_t)nnz * sizeof(double), cudaMemcpyDeviceToHost, st));
-    HOST_TRY(cudaMemcpyAsync(h_f, d_f, (size_t)n3 * sizeof(double), cudaMemcpyDeviceToHost, st));
-    HOST_TRY(cudaStreamSynchronize(st));
-#undef HOST_TRY
-    cleanup();
-    return RPIM_OK;
+    if (h_row_ptr && (rc = ws_alloc(ctx, &ctx->hb_rp, (int64_t)((n3 + 1) * iw)))) return rc;
+    if (h_col_idx && (rc = ws_alloc(ctx, &ctx->hb_ci, (int64_t)(std::max<int64_t>(nnz, 1) * iw)))) return rc;
+    if (!ctx->side_stream) {
+        CUDA_TRY(ctx, cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking));
+        CUDA_TRY(ctx, cudaEventCreateWithFlags(&ctx->side_ev[0], cudaEventDisableTiming));
+        CUDA_TRY(ctx, cudaEventCreateWithFlags(&ctx->side_ev[1], cudaEventDisableTiming));
+    }
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->hb_qw, h_qw, (size_t)ctx->Nq * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (m > 0) {
+        CUDA_TRY(ctx, cudaMemcpyAsync(ctx->hb_bn, h_bc_nodes, (size_t)m * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+        CUDA_TRY(ctx, cudaMemcpyAsync(ctx->hb_ub, h_u_bar, (size_t)3 * m * sizeof(double), cudaMemcpyHostToDevice, st));
+        if (h_bc_mask) CUDA_TRY(ctx, cudaMemcpyAsync(ctx->hb_bm, h_bc_mask, (size_t)m, cudaMemcpyHostToDevice, st));
+    }
+    if ((rc = rpim_get_pattern(ctx, h_row_ptr ? ctx->hb_rp : nullptr, h_col_idx ? ctx->hb_ci : nullptr, nullptr))) return rc;
+    CUDA_TRY(ctx, cudaEventRecord(ctx->side_ev[0], st));
+    CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->side_stream, ctx->side_ev[0], 0));
+    if (h_row_ptr) CUDA_TRY(ctx, cudaMemcpyAsync(h_row_ptr, ctx->hb_rp, (size_t)(n3 + 1) * iw, cudaMemcpyDeviceToHost, ctx->side_stream));
+    if (h_col_idx) CUDA_TRY(ctx, cudaMemcpyAsync(h_col_idx, ctx->hb_ci, (size_t)nnz * iw, cudaMemcpyDeviceToHost, ctx->side_stream));
+    CUDA_TRY(ctx, cudaEventRecord(ctx->side_ev[1], ctx->side_stream));
+    rc = rpim_assemble(ctx, ctx->hb_qw, E, nu, alpha_c, d_c, q, body, ctx->hb_vals, ctx->hb_f, out_singular);
+    if (rc == RPIM_OK)
+        rc = rpim_apply_penalty(ctx, m > 0 ? ctx->hb_bn : nullptr, (m > 0 && h_bc_mask) ? ctx->hb_bm : nullptr,
+                                m > 0 ? ctx->hb_ub : nullptr, m, alpha, alpha_is_relative, ctx->hb_vals, ctx->hb_f,
+                                out_alpha_used);
+    if (rc == RPIM_OK) {
+        cudaError_t e = cudaMemcpyAsync(h_vals, ctx->hb_vals, (size_t)nnz * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(h_f, ctx->hb_f, (size_t)n3 * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) { ctx->err = std::string("device to host copy failed: ") + cudaGetErrorString(e); rc = RPIM_ERR_CUDA; }
+    }
+    // join the side stream into the main one and drain both, also on failure (the host arrays are the caller's)
+    cudaStreamWaitEvent(st, ctx->side_ev[1], 0);
+    cudaError_t e1 = cudaStreamSynchronize(st);
+    if (rc == RPIM_OK && e1 != cudaSuccess) RPIM_FAIL(ctx, RPIM_ERR_CUDA, "rpim_host_assemble failed: %s", cudaGetErrorString(e1));
+    return rc;
 }
 
 }  // extern "C"

@@ -107,6 +107,11 @@ struct rpim_ctx {
 
     // device buffers of the host-buffer entry points
     double *h2d_nodes = nullptr, *h2d_qpts = nullptr;
+    double *hb_qw = nullptr, *hb_vals = nullptr, *hb_f = nullptr, *hb_ub = nullptr;
+    int64_t* hb_bn = nullptr;
+    uint8_t *hb_bm = nullptr, *hb_rp = nullptr, *hb_ci = nullptr;
+    cudaStream_t side_stream = nullptr;   // device -> host copy of the index arrays, overlapped with the assembly
+    cudaEvent_t side_ev[2] = {nullptr, nullptr};
 };
 
 #define RPIM_FAIL(ctx, code, ...)                          \

@@ -420,7 +420,17 @@ knn_select_kernel(GridParams g, const double* __restrict__ sx, const double* __r
                 unsigned lo32 = __reduce_max_sync(FULLW, ((unsigned)(kmax >> 32) == hi32) ? (unsigned)kmax : 0u);
                 kmax = ((unsigned long long)hi32 << 32) | lo32;
             }
-            unsigned long long lo = 0, hi = kmax, T = 0;
+            // ... and the smallest one: the bracket [kmin, kmax] spans a few binades instead of all of them
+            unsigned long long kmin = KINF;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e)
+                if (key[e] < kmin) kmin = key[e];
+            {
+                unsigned hi32 = __reduce_min_sync(FULLW, (unsigned)(kmin >> 32));
+                unsigned lo32 = __reduce_min_sync(FULLW, ((unsigned)(kmin >> 32) == hi32) ? (unsigned)kmin : 0xffffffffu);
+                kmin = ((unsigned long long)hi32 << 32) | lo32;
+            }
+            unsigned long long lo = kmin, hi = kmax, T = 0;
             int c_le = 0;
             bool found = false;
             for (int it = 0; it < 24 && !found; ++it) {

@@ -530,14 +530,14 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
         {
             const int64_t words = ctx->Nq * (int64_t)ctx->k * (pstride / 32);
             const int64_t bytes = words * (int64_t)sizeof(unsigned);
-            size_t free_b = 0, total_b = 0;
-            CUDA_TRY(ctx, cudaMemGetInfo(&free_b, &total_b));
             bool reuse = false;   // a block we already own does not count against the budget
             for (auto& b : ctx->ws_cache) reuse = reuse || (b.second >= bytes && b.second <= 2 * bytes + 4096);
             if (ctx->d_masks) {
                 auto it = ctx->ws_sizes.find((void*)ctx->d_masks);
                 reuse = reuse || (it != ctx->ws_sizes.end() && it->second >= bytes && it->second <= 2 * bytes + 4096);
             }
+            size_t free_b = 0, total_b = 0;
+            if (!reuse) CUDA_TRY(ctx, cudaMemGetInfo(&free_b, &total_b));   // a driver call: only when it matters
             if (reuse || (uint64_t)bytes <= free_b / 4) {
                 if (ws_alloc(ctx, &ctx->d_masks, words) == RPIM_OK) d_masks = ctx->d_masks;
                 else ctx->err.clear();

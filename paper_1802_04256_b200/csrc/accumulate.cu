@@ -153,24 +153,41 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
             };
             if (tg == 0) { issue(0); if (nsub > 1) issue(1); }
             // ---- phase 1b: positions of this warp's points b = wg, wg + NWARP, ... (overlaps the copies)
-            for (int b = wg; !MASKED && b < nb; b += NWARP) {
-                const int32_t* sp = support + (sm.qbase[b] - stage) / 4;   // = support + q * k
-                unsigned cm = 0;
-                for (int ps = 0; ps < npass; ++ps) {
-                    const int j = ps * 32 + lane;
-                    unsigned wbit = 0;
-                    if (j < k) {
-                        const unsigned J = (unsigned)sp[j];
-                        unsigned h = (J * 2654435761u) >> HSHIFT;
-                        unsigned long long ent = sm.hent[h];
-                        while ((unsigned)(ent >> 32) != J) { h = (h + 1) & (HSZ - 1); ent = sm.hent[h]; }
-                        const unsigned slot = (unsigned)ent;
-                        sm.pos[b][slot] = (unsigned char)j;
-                        wbit = 1u << (slot >> 5);
+            if constexpr (!MASKED) {
+                // support nodes of the next point are fetched while the current one is looked up
+                // (k <= RPIM_MAX_K = 124: at most four passes of 32 lanes)
+                auto fetch = [&](int b, int (&J)[4]) {
+                    const int32_t* sp = support + (sm.qbase[min(b, nb - 1)] - stage) / 4;   // = support + q * k
+#pragma unroll
+                    for (int ps = 0; ps < 4; ++ps) {
+                        const int j = ps * 32 + lane;
+                        J[ps] = (b < nb && j < k) ? sp[j] : -1;
                     }
-                    cm |= __reduce_or_sync(FULLMASK, wbit);
+                };
+                int Jc[4], Jn[4];
+                fetch(wg, Jc);
+                for (int b = wg; b < nb; b += NWARP) {
+                    fetch(b + NWARP, Jn);
+                    unsigned cm = 0;
+#pragma unroll
+                    for (int ps = 0; ps < 4; ++ps) {
+                        if (ps >= npass) break;
+                        unsigned wbit = 0;
+                        if (Jc[ps] >= 0) {
+                            const unsigned J = (unsigned)Jc[ps];
+                            unsigned h = (J * 2654435761u) >> HSHIFT;
+                            unsigned long long ent = sm.hent[h];
+                            while ((unsigned)(ent >> 32) != J) { h = (h + 1) & (HSZ - 1); ent = sm.hent[h]; }
+                            const unsigned slot = (unsigned)ent;
+                            sm.pos[b][slot] = (unsigned char)(ps * 32 + lane);
+                            wbit = 1u << (slot >> 5);
+                        }
+                        cm |= __reduce_or_sync(FULLMASK, wbit);
+                    }
+                    if (lane == 0) sm.cmask[b] = cm;
+#pragma unroll
+                    for (int ps = 0; ps < 4; ++ps) Jc[ps] = Jn[ps];
                 }
-                if (lane == 0) sm.cmask[b] = cm;
             }
             // ---- phase 2: every lane accumulates its slots over the points, sub-batch by sub-batch
             for (int sb = 0; sb < nsub; ++sb) {

@@ -442,13 +442,24 @@ template <int NWARP, int CPW, int ROWS, bool MASKED>
 int launch_reduce_rows_m(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
                          double* d_vals, double* d_f) {
     auto kern = reduce_rows_kernel<NWARP, CPW, ROWS, MASKED>;
-    // gradient staging: two buffers of nbg points each, about 16 KB per row group
-    const int nbg = std::max(2, std::min(8, 8192 / (ctx->k * 32)));
-    const size_t smem = red_group_bytes(sizeof(RedSmem<NWARP, CPW, MASKED>), ctx->k, nbg) * ROWS;
-    CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int per_sm = 1;
+    // gradient staging: two buffers of nbg points each per row group.  Larger sub-batches mean fewer
+    // group barriers; take the largest nbg (<= 8) that does not cost a resident CTA
+    CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    int nbg = 2, per_sm = 1;
+    size_t smem = red_group_bytes(sizeof(RedSmem<NWARP, CPW, MASKED>), ctx->k, nbg) * ROWS;
+    if (smem > 227 * 1024) RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "k = %d does not fit the staging area of the reduction", ctx->k);
     CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NWARP * ROWS * 32, smem));
     if (per_sm < 1) per_sm = 1;
+    for (int cand = 8; cand > 2; --cand) {
+        const size_t sc = red_group_bytes(sizeof(RedSmem<NWARP, CPW, MASKED>), ctx->k, cand) * ROWS;
+        int occ = 0;
+        if (sc <= 227 * 1024 &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, NWARP * ROWS * 32, sc) == cudaSuccess && occ >= per_sm) {
+            nbg = cand;
+            smem = sc;
+            break;
+        }
+    }
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
     int64_t blocks = (ctx->N + ROWS - 1) / ROWS;

@@ -107,6 +107,19 @@ def test_shuffled_node_numbering():
     _compare(w, run_cuda(w), run_oracle(w))
 
 
+def test_degenerate_sizes_single_point_and_k_equal_N():
+    # one quadrature point only; and every node in every support (k = N): one dense block row per node
+    w = workloads.make_block("one", 5, 4, 4, 1.0, 1, 20, 3e9, 0.3, jitter=0.2, seed=9, body=(1.0, 2.0, -3.0), bc="none")
+    w.qpts = np.ascontiguousarray(w.qpts[7:8])
+    w.qw = np.ascontiguousarray(w.qw[7:8])
+    _compare(w, run_cuda(w, penalty=False), run_oracle(w, penalty=False), check_penalty=False)
+    w = workloads.make_block("kN", 4, 3, 3, 1.0, 2, 36, 3e9, 0.3, jitter=0.25, seed=10, body=(0.0, 0.0, -1e4), bc="bottom")
+    assert w.N == w.k
+    g, o = run_cuda(w), run_oracle(w)
+    _compare(w, g, o)
+    assert g["nnz"] == 9 * w.N * w.N
+
+
 def test_planar_cloud_every_point_is_singular():
     nodes = np.array([[i, j, 0.0] for j in range(6) for i in range(6)], dtype=np.float64)
     w = workloads.make_block("flat", 6, 6, 2, 1.0, 1, 12, 1e9, 0.3)

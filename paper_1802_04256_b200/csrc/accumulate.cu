@@ -50,6 +50,7 @@ struct alignas(16) RedSmem {
     unsigned cmask[RED_NB];             // chunks of the row hit by point b
     unsigned long long full[2];         // mbarriers of the two staging buffers
     double fpart[NWARP];
+    long long next_row[2];              // row handed to this group (two slots: written one row ahead of its last reader)
 };
 
 // Dynamic shared memory of one row group: RedSmem followed by the double-buffered gradient
@@ -66,8 +67,8 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                    const uint8_t* __restrict__ inc_j, const int32_t* __restrict__ support,
                    const double* __restrict__ stage, const double* __restrict__ qw,
                    const int64_t* __restrict__ brow_ptr, const int32_t* __restrict__ bcol,
-                   const int64_t* __restrict__ mask_ptr, const unsigned* __restrict__ masks, int mask_stride, double lambda,
-                   double mu, double bx, double by, double bz, double* __restrict__ vals, double* __restrict__ f) {
+                   const int64_t* __restrict__ mask_ptr, const unsigned* __restrict__ masks, int mask_stride,
+                   unsigned long long* __restrict__ ticket, double lambda, double mu, double bx, double by, double bz, double* __restrict__ vals, double* __restrict__ f) {
     using S = RedSmem<NWARP, CPW, MASKED>;
     constexpr int NS = S::NS, HSZ = S::HSZ, GT = NWARP * 32;
     constexpr int HSHIFT = 32 - S::HLOG;
@@ -86,10 +87,18 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
     unsigned ph0 = 0, ph1 = 0;   // parity of the next completion of each staging buffer
     __syncthreads();
 
-    for (int64_t I = (int64_t)blockIdx.x * ROWS + rg; I < N; I += (int64_t)gridDim.x * ROWS) {
+    // rows are handed out in ascending order from a global ticket: the resident groups always work on
+    // one contiguous stripe of rows (their staged gradients are shared through L2) and stay balanced
+    // (the ticket of the next row is drawn while the current row is processed: its latency is hidden)
+    long long drawn = (tg == 0) ? (long long)atomicAdd(ticket, 1ull) : 0;
+    for (unsigned it = 0;; ++it) {
+        if (tg == 0) sm.next_row[it & 1] = drawn;
+        group_sync<NWARP>(rg);   // ticket visible; the previous row's shared data is dead
+        const int64_t I = sm.next_row[it & 1];
+        if (I >= N) break;
+        if (tg == 0) drawn = (long long)atomicAdd(ticket, 1ull);
         const int64_t o = brow_ptr[I];
         const int L = (int)(brow_ptr[I + 1] - o);
-        group_sync<NWARP>(rg);   // the previous row's shared data is dead
         if constexpr (!MASKED) {
             for (int s = tg; s < HSZ; s += GT) sm.hent[s] = ~0ull;
             group_sync<NWARP>(rg);
@@ -463,10 +472,13 @@ int launch_reduce_rows_m(rpim_ctx* ctx, const double* d_qw, double lambda, doubl
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
     int64_t blocks = (ctx->N + ROWS - 1) / ROWS;
-    blocks = std::min<int64_t>(blocks, (int64_t)sms * per_sm * 8);   // several waves: boundary rows are cheaper
+    // persistent: exactly one resident wave; its row groups draw rows from a ticket counter
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_ROW_TICKET, 0, sizeof(long long), ctx->stream));
+    blocks = std::min<int64_t>(blocks, (int64_t)sms * per_sm);
     kern<<<(unsigned)blocks, NWARP * ROWS * 32, smem, ctx->stream>>>(
         ctx->N, ctx->k, nbg, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_support, ctx->d_stage, d_qw,
-        ctx->d_brow_ptr, ctx->d_bcol, ctx->d_mask_ptr, ctx->d_masks, ctx->mask_stride, lambda, mu, body[0], body[1], body[2], d_vals, d_f);
+        ctx->d_brow_ptr, ctx->d_bcol, ctx->d_mask_ptr, ctx->d_masks, ctx->mask_stride,
+        (unsigned long long*)(ctx->d_flags + FLAG_ROW_TICKET), lambda, mu, body[0], body[1], body[2], d_vals, d_f);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
 }

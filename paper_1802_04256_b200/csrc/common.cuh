@@ -13,7 +13,7 @@
 #define RPIM_WARP 32
 
 // device-side error / counter slots (ctx->d_flags, int64 each)
-enum { FLAG_KNN_CAP = 0, FLAG_PAT_CAP = 1, FLAG_BC_BAD = 2, FLAG_SINGULAR = 3, FLAG_INC_CAP = 4, FLAG_OVF_ROWS = 5, FLAG_OVF_Q = 6, FLAG_INC_LONG = 7, FLAG_ROW_TICKET = 8, NUM_FLAGS = 16 };
+enum { FLAG_KNN_CAP = 0, FLAG_PAT_CAP = 1, FLAG_BC_BAD = 2, FLAG_SINGULAR = 3, FLAG_INC_CAP = 4, FLAG_OVF_ROWS = 5, FLAG_OVF_Q = 6, FLAG_INC_LONG = 7, FLAG_ROW_TICKET = 8, FLAG_INC_LONG2 = 9, NUM_FLAGS = 16 };
 
 struct GridParams {
     double lo[3];

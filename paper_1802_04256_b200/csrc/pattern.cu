@@ -27,25 +27,27 @@ constexpr int INC_CAP = 4096;   // longest incidence list sorted on chip
 constexpr int INC_WARPS = 4;
 constexpr int INC_FAST_CAP = 128;   // lists up to this length take the high-occupancy launch
 constexpr int INC_FAST_WARPS = 8;
+constexpr int INC_MID_CAP = 1024;   // lists up to this length: 8 KB of shared memory per warp
 
 // one warp per node: sort its list ascending by point id (the position byte rides along).
-// Launched twice: CAP = INC_FAST_CAP handles the usual short lists with 1 KB of shared memory per
-// warp (full occupancy), CAP = INC_CAP picks up the longer ones (LO = INC_FAST_CAP).
-template <int CAP, int LO, int WARPS>
+// Three tiers by list length, each with the shared memory (and so the occupancy) its capacity needs:
+// up to INC_FAST_CAP, up to INC_MID_CAP, up to INC_CAP.  A tier raises FLAG_OUT when it meets a list
+// that is too long for it; the next tier returns at once unless its FLAG_IN was raised.
+template <int CAP, int LO, int WARPS, int FLAG_IN, int FLAG_OUT>
 __global__ void __launch_bounds__(WARPS * 32)
 inc_sort_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, int32_t* __restrict__ inc_q,
                 uint8_t* __restrict__ inc_j, long long* __restrict__ flags) {
     extern __shared__ unsigned char smem_raw[];
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned long long* key = (unsigned long long*)smem_raw + (size_t)wid * CAP;
-    if (LO > 0 && flags[FLAG_INC_LONG] == 0) return;   // second launch: the first one met no longer list
+    if (FLAG_IN >= 0 && flags[FLAG_IN] == 0) return;   // the previous tier met no list beyond its capacity
     for (int64_t I = (int64_t)blockIdx.x * WARPS + wid; I < N; I += (int64_t)gridDim.x * WARPS) {
         const int64_t a = inc_ptr[I];
         const int len = (int)(inc_ptr[I + 1] - a);
         if (len <= 1 || len <= LO) continue;
         if (len > CAP) {
-            if (CAP == INC_CAP && lane == 0) atomicAdd((unsigned long long*)&flags[FLAG_INC_CAP], 1ull);
-            if (CAP != INC_CAP && lane == 0) flags[FLAG_INC_LONG] = 1;
+            if (FLAG_OUT < 0 && lane == 0) atomicAdd((unsigned long long*)&flags[FLAG_INC_CAP], 1ull);
+            if (FLAG_OUT >= 0 && lane == 0) flags[FLAG_OUT] = 1;
             continue;
         }
         const int np = next_pow2(len);
@@ -458,12 +460,17 @@ int rpim_stage_incidence(rpim_ctx* ctx) {
                                         ctx->d_inc_q, ctx->d_inc_j);
     KERNEL_CHECK(ctx);
     {
-        auto fast = inc_sort_kernel<INC_FAST_CAP, 0, INC_FAST_WARPS>;
+        auto fast = inc_sort_kernel<INC_FAST_CAP, 0, INC_FAST_WARPS, -1, FLAG_INC_LONG>;
         const size_t smem_f = (size_t)INC_FAST_WARPS * INC_FAST_CAP * sizeof(unsigned long long);
         fast<<<(unsigned)std::min<int64_t>((N + INC_FAST_WARPS - 1) / INC_FAST_WARPS, 148 * 64), INC_FAST_WARPS * 32,
                smem_f, st>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_flags);
         KERNEL_CHECK(ctx);
-        auto slow = inc_sort_kernel<INC_CAP, INC_FAST_CAP, INC_WARPS>;
+        auto mid = inc_sort_kernel<INC_MID_CAP, INC_FAST_CAP, INC_WARPS, FLAG_INC_LONG, FLAG_INC_LONG2>;
+        const size_t smem_m = (size_t)INC_WARPS * INC_MID_CAP * sizeof(unsigned long long);
+        mid<<<(unsigned)std::min<int64_t>((N + INC_WARPS - 1) / INC_WARPS, 148 * 16), INC_WARPS * 32, smem_m, st>>>(
+            N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_flags);
+        KERNEL_CHECK(ctx);
+        auto slow = inc_sort_kernel<INC_CAP, INC_MID_CAP, INC_WARPS, FLAG_INC_LONG2, -1>;
         const size_t smem = (size_t)INC_WARPS * INC_CAP * sizeof(unsigned long long);
         CUDA_TRY(ctx, cudaFuncSetAttribute(slow, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         slow<<<(unsigned)std::min<int64_t>((N + INC_WARPS - 1) / INC_WARPS, 148), INC_WARPS * 32, smem, st>>>(

@@ -488,12 +488,7 @@ int launch_brow_bitmap(rpim_ctx* ctx, int32_t* d_pool, int32_t* d_ovf_rows, unsi
     auto kern = brow_bitmap_kernel<PSTRIDE>;
     const size_t smem = (size_t)BM_WARPS * BM_PER_WARP * sizeof(unsigned);
     CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    // one resident wave (grid-stride over the rows): at any moment the warps work on one contiguous
-    // stripe of rows, whose supports they share through L2
-    int per_sm = 1, sms = 148;
-    CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, BM_WARPS * 32, smem));
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
-    const unsigned nb = (unsigned)std::min<int64_t>((N + BM_WARPS - 1) / BM_WARPS, (int64_t)sms * std::max(per_sm, 1));
+    const unsigned nb = (unsigned)std::min<int64_t>((N + BM_WARPS - 1) / BM_WARPS, 148 * 16);
     kern<<<nb, BM_WARPS * 32, smem, ctx->stream>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->k, ctx->d_blen,
                                                    d_pool, ctx->d_bdiag, d_ovf_rows, d_masks, ctx->d_flags);
     KERNEL_CHECK(ctx);

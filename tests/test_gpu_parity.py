@@ -120,6 +120,22 @@ def test_degenerate_sizes_single_point_and_k_equal_N():
     assert g["nnz"] == 9 * w.N * w.N
 
 
+def test_one_context_serves_problems_of_changing_size():
+    # the workspace cache hands blocks from earlier, differently sized problems back out: results must not
+    # depend on what the context did before
+    import paper_1802_04256_b200 as rp
+    cases = [workloads.make_block("c1", 9, 8, 7, 1.0, 2, 30, 5e9, 0.3, jitter=0.3, seed=31, body=(0.0, 0.0, -2.5e4), bc="bottom"),
+             workloads.make_block("c2", 5, 5, 4, 0.5, 1, 12, 2e9, 0.2, jitter=0.2, seed=32, body=(1.0, 0.0, -1e4), bc="x0"),
+             workloads.make_block("c3", 10, 9, 9, 1.0, 2, 40, 5e9, 0.3, jitter=0.3, seed=33, body=(0.0, 0.0, -2.5e4), bc="bottom+roller"),
+             workloads.make_block("c1", 9, 8, 7, 1.0, 2, 30, 5e9, 0.3, jitter=0.3, seed=31, body=(0.0, 0.0, -2.5e4), bc="bottom")]
+    with rp.Context(0) as ctx:
+        outs = [run_cuda(w, ctx=ctx) for w in cases]
+    for w, g in zip(cases[:3], outs[:3]):
+        _compare(w, g, run_oracle(w))
+    for key in ("vals", "f", "col_idx", "phi", "dphi"):
+        assert np.array_equal(outs[0][key], outs[3][key]), key       # same problem again: same bits
+
+
 def test_planar_cloud_every_point_is_singular():
     nodes = np.array([[i, j, 0.0] for j in range(6) for i in range(6)], dtype=np.float64)
     w = workloads.make_block("flat", 6, 6, 2, 1.0, 1, 12, 1e9, 0.3)

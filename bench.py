@@ -228,7 +228,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--with-solve", action="store_true",
-                    help="also time stage 3 (block SpMV, Jacobi-PCG to 1e-8) on the assembled system; extra key \"solve\"")
+                    help="also time stage 3 (block SpMV, block-Jacobi PCG to 1e-8) on the assembled system; extra key \"solve\"")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = max(args.warmup, 3) if os.environ.get("RPIM_BENCH_STRICT_WARMUP", "1") == "1" else args.warmup

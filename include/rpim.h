@@ -106,7 +106,8 @@ int rpim_apply_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* 
  * rpim_matvec: y = K x with K in the layout rpim_assemble / rpim_apply_penalty leave in d_vals (the
  * pattern is the context's).  d_x, d_y: 3N fp64.  Asynchronous.
  *
- * rpim_solve_pcg: conjugate gradients with Jacobi (diagonal) preconditioning on the penalised K,
+ * rpim_solve_pcg: conjugate gradients with block-Jacobi preconditioning (inverse of the 3x3 diagonal block of every
+ * node) on the penalised K,
  * which is symmetric positive definite (R10).  d_u holds the initial guess on entry and
  * the solution on exit (3N).  Stops when ||f - K u||_2 <= rel_tol * ||f||_2 (looked at every 25
  * iterations) or after max_iter iterations; out_iters / out_rel_resid (host, may be NULL) report

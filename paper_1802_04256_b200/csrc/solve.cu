@@ -1,5 +1,5 @@
 // Stage 3 of the paper ("solve the system ... then the stresses"), SURVEY 8(f)
-// NEXT-1: Jacobi-preconditioned conjugate gradients on the assembled, penalised K (symmetric
+// NEXT-1: block-Jacobi-preconditioned (3x3 nodal blocks) conjugate gradients on the assembled, penalised K (symmetric
 // positive definite, R10/A2) and stress recovery sigma = D B u at the quadrature points.
 //
 // K is used in the layout rpim_assemble writes (block row I: three scalar rows of 3 L entries at
@@ -79,35 +79,70 @@ bspmv_kernel(int64_t N, const int64_t* __restrict__ brow_ptr, const int32_t* __r
     }
 }
 
-// 1 / K_dd (Jacobi); rows without entries (nodes in no support) get 0: their unknown stays 0
+// inverse of the 3x3 diagonal block of every node (block Jacobi), 9 doubles per node, row-major.
+// A block that is not positive definite falls back to its positive diagonal entries; nodes without
+// entries (in no support) get 0: their unknowns stay 0.
 __global__ void diag_inv_kernel(int64_t N, const int64_t* __restrict__ brow_ptr, const int* __restrict__ bdiag,
                                 const double* __restrict__ vals, double* __restrict__ dinv) {
     const int64_t I = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (I >= N) return;
     const int64_t o = brow_ptr[I], L = brow_ptr[I + 1] - o;
+    double m[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    if (L > 0)
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        double d = 0.0;
-        if (L > 0) d = vals[9 * o + a * 3 * L + 3 * (int64_t)bdiag[I] + a];
-        dinv[3 * I + a] = (d > 0.0) ? 1.0 / d : 0.0;
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) m[a][b] = vals[9 * o + a * 3 * L + 3 * (int64_t)bdiag[I] + b];
+    const double c00 = m[1][1] * m[2][2] - m[1][2] * m[2][1];
+    const double c01 = m[1][2] * m[2][0] - m[1][0] * m[2][2];
+    const double c02 = m[1][0] * m[2][1] - m[1][1] * m[2][0];
+    const double det = (m[0][0] * c00 + m[0][1] * c01) + m[0][2] * c02;
+    double inv[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    const bool spd = m[0][0] > 0.0 && c00 > 0.0 && det > 0.0 && isfinite(det);   // leading minors (Sylvester, from the last row up)
+    if (spd) {
+        const double rd = 1.0 / det;
+        inv[0] = c00 * rd;
+        inv[1] = (m[0][2] * m[2][1] - m[0][1] * m[2][2]) * rd;
+        inv[2] = (m[0][1] * m[1][2] - m[0][2] * m[1][1]) * rd;
+        inv[3] = c01 * rd;
+        inv[4] = (m[0][0] * m[2][2] - m[0][2] * m[2][0]) * rd;
+        inv[5] = (m[0][2] * m[1][0] - m[0][0] * m[1][2]) * rd;
+        inv[6] = c02 * rd;
+        inv[7] = (m[0][1] * m[2][0] - m[0][0] * m[2][1]) * rd;
+        inv[8] = (m[0][0] * m[1][1] - m[0][1] * m[1][0]) * rd;
+    } else {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) inv[4 * a] = (m[a][a] > 0.0) ? 1.0 / m[a][a] : 0.0;
     }
+#pragma unroll
+    for (int e = 0; e < 9; ++e) dinv[9 * I + e] = inv[e];
 }
 
-// r = f - y, z = dinv r, p = z; partial sums of r.z and r.r
+__device__ __forceinline__ void apply_block(const double* __restrict__ d, double r0, double r1, double r2, double& z0,
+                                            double& z1, double& z2) {
+    z0 = fma(d[2], r2, fma(d[1], r1, d[0] * r0));
+    z1 = fma(d[5], r2, fma(d[4], r1, d[3] * r0));
+    z2 = fma(d[8], r2, fma(d[7], r1, d[6] * r0));
+}
+
+// r = f - y, z = Dinv r, p = z; partial sums of r.z and r.r (one thread per node, contiguous slice per block)
 __global__ void __launch_bounds__(SV_THREADS)
-pcg_init_kernel(int64_t n, const double* __restrict__ f, const double* __restrict__ y, const double* __restrict__ dinv,
+pcg_init_kernel(int64_t N, const double* __restrict__ f, const double* __restrict__ y, const double* __restrict__ dinv,
                 double* __restrict__ r, double* __restrict__ z, double* __restrict__ p, double* __restrict__ part_rz,
                 double* __restrict__ part_rr) {
     __shared__ double sh[SV_THREADS / 32];
     double rz = 0.0, rr = 0.0;
-    const int64_t per = (n + gridDim.x - 1) / gridDim.x;   // contiguous slice per block: fixed summation order
-    const int64_t lo = per * blockIdx.x, hi = min(n, lo + per);
-    for (int64_t i = lo + threadIdx.x; i < hi; i += SV_THREADS) {
-        const double ri = f[i] - y[i];
-        const double zi = dinv[i] * ri;
-        r[i] = ri; z[i] = zi; p[i] = zi;
-        rz = fma(ri, zi, rz);
-        rr = fma(ri, ri, rr);
+    const int64_t per = (N + gridDim.x - 1) / gridDim.x;   // contiguous slice per block: fixed summation order
+    const int64_t lo = per * blockIdx.x, hi = min(N, lo + per);
+    for (int64_t I = lo + threadIdx.x; I < hi; I += SV_THREADS) {
+        const double r0 = f[3 * I] - y[3 * I], r1 = f[3 * I + 1] - y[3 * I + 1], r2 = f[3 * I + 2] - y[3 * I + 2];
+        double z0, z1, z2;
+        apply_block(dinv + 9 * I, r0, r1, r2, z0, z1, z2);
+        r[3 * I] = r0; r[3 * I + 1] = r1; r[3 * I + 2] = r2;
+        z[3 * I] = z0; z[3 * I + 1] = z1; z[3 * I + 2] = z2;
+        p[3 * I] = z0; p[3 * I + 1] = z1; p[3 * I + 2] = z2;
+        rz = fma(r2, z2, fma(r1, z1, fma(r0, z0, rz)));
+        rr = fma(r2, r2, fma(r1, r1, fma(r0, r0, rr)));
     }
     const double t0 = block_sum(rz, sh);
     const double t1 = block_sum(rr, sh);
@@ -132,23 +167,30 @@ __global__ void pcg_scalar_kernel(int mode, const double* __restrict__ pa, const
     }
 }
 
-// x += alpha p, r -= alpha Ap, z = dinv r; partial sums of r.z and r.r
+// x += alpha p, r -= alpha Ap, z = Dinv r; partial sums of r.z and r.r (one thread per node)
 __global__ void __launch_bounds__(SV_THREADS)
-pcg_update_kernel(int64_t n, const double* __restrict__ sc, const double* __restrict__ p, const double* __restrict__ Ap,
+pcg_update_kernel(int64_t N, const double* __restrict__ sc, const double* __restrict__ p, const double* __restrict__ Ap,
                   const double* __restrict__ dinv, double* __restrict__ x, double* __restrict__ r,
                   double* __restrict__ z, double* __restrict__ part_rz, double* __restrict__ part_rr) {
     __shared__ double sh[SV_THREADS / 32];
     const double alpha = sc[S_ALPHA];
     double rz = 0.0, rr = 0.0;
-    const int64_t per = (n + gridDim.x - 1) / gridDim.x;
-    const int64_t lo = per * blockIdx.x, hi = min(n, lo + per);
-    for (int64_t i = lo + threadIdx.x; i < hi; i += SV_THREADS) {
-        x[i] = fma(alpha, p[i], x[i]);
-        const double ri = fma(-alpha, Ap[i], r[i]);
-        const double zi = dinv[i] * ri;
-        r[i] = ri; z[i] = zi;
-        rz = fma(ri, zi, rz);
-        rr = fma(ri, ri, rr);
+    const int64_t per = (N + gridDim.x - 1) / gridDim.x;
+    const int64_t lo = per * blockIdx.x, hi = min(N, lo + per);
+    for (int64_t I = lo + threadIdx.x; I < hi; I += SV_THREADS) {
+        double rn[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const int64_t i = 3 * I + c;
+            x[i] = fma(alpha, p[i], x[i]);
+            rn[c] = fma(-alpha, Ap[i], r[i]);
+            r[i] = rn[c];
+        }
+        double z0, z1, z2;
+        apply_block(dinv + 9 * I, rn[0], rn[1], rn[2], z0, z1, z2);
+        z[3 * I] = z0; z[3 * I + 1] = z1; z[3 * I + 2] = z2;
+        rz = fma(rn[2], z2, fma(rn[1], z1, fma(rn[0], z0, rz)));
+        rr = fma(rn[2], rn[2], fma(rn[1], rn[1], fma(rn[0], rn[0], rr)));
     }
     const double t0 = block_sum(rz, sh);
     const double t1 = block_sum(rr, sh);
@@ -230,13 +272,14 @@ int rpim_solve_pcg(rpim_ctx* ctx, const double* d_vals, const double* d_f, doubl
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
     const int64_t N = ctx->N, n = 3 * N;
-    double* w = nullptr;   // r | z | p | Ap | dinv | partials a | partials b | scalars
+    double* w = nullptr;   // r | z | p | Ap | Dinv (9 per node) | partials a | partials b | scalars
     int rc;
-    if ((rc = ws_alloc(ctx, &w, 5 * n + 2 * SV_PARTS + S_NUM))) return rc;
+    if ((rc = ws_alloc(ctx, &w, 7 * n + 2 * SV_PARTS + S_NUM))) return rc;
     double *r = w, *z = w + n, *p = w + 2 * n, *Ap = w + 3 * n, *dinv = w + 4 * n;
-    double *pa = w + 5 * n, *pb = pa + SV_PARTS, *sc = pb + SV_PARTS;
+    double *pa = w + 7 * n, *pb = pa + SV_PARTS, *sc = pb + SV_PARTS;
     const unsigned nbm = (unsigned)std::min<int64_t>((N + 7) / 8, SV_PARTS);
     const unsigned nbv = (unsigned)std::min<int64_t>((n + SV_THREADS - 1) / SV_THREADS, SV_PARTS);
+    const unsigned nbn = (unsigned)std::min<int64_t>((N + SV_THREADS - 1) / SV_THREADS, SV_PARTS);   // node-wise kernels
     auto fail = [&](int code) { ws_free(ctx, &w); return code; };
 #define SOLVE_LAUNCH_CHECK()                                                         \
     do {                                                                             \
@@ -265,9 +308,9 @@ int rpim_solve_pcg(rpim_ctx* ctx, const double* d_vals, const double* d_f, doubl
     if (ff > 0.0) {
         bspmv_kernel<<<nbm, SV_THREADS, 0, st>>>(N, ctx->d_brow_ptr, ctx->d_bcol, d_vals, d_u, Ap, nullptr);
         SOLVE_LAUNCH_CHECK();
-        pcg_init_kernel<<<nbv, SV_THREADS, 0, st>>>(n, d_f, Ap, dinv, r, z, p, pa, pb);
+        pcg_init_kernel<<<nbn, SV_THREADS, 0, st>>>(N, d_f, Ap, dinv, r, z, p, pa, pb);
         SOLVE_LAUNCH_CHECK();
-        pcg_scalar_kernel<<<1, SV_THREADS, 0, st>>>(0, pa, pb, (int)nbv, sc);
+        pcg_scalar_kernel<<<1, SV_THREADS, 0, st>>>(0, pa, pb, (int)nbn, sc);
         SOLVE_LAUNCH_CHECK();
         const int check = 25;   // iterations between two looks at the residual (one small copy each)
         while (true) {
@@ -283,9 +326,9 @@ int rpim_solve_pcg(rpim_ctx* ctx, const double* d_vals, const double* d_f, doubl
                 SOLVE_LAUNCH_CHECK();
                 pcg_scalar_kernel<<<1, SV_THREADS, 0, st>>>(1, pa, nullptr, (int)nbm, sc);
                 SOLVE_LAUNCH_CHECK();
-                pcg_update_kernel<<<nbv, SV_THREADS, 0, st>>>(n, sc, p, Ap, dinv, d_u, r, z, pa, pb);
+                pcg_update_kernel<<<nbn, SV_THREADS, 0, st>>>(N, sc, p, Ap, dinv, d_u, r, z, pa, pb);
                 SOLVE_LAUNCH_CHECK();
-                pcg_scalar_kernel<<<1, SV_THREADS, 0, st>>>(2, pa, pb, (int)nbv, sc);
+                pcg_scalar_kernel<<<1, SV_THREADS, 0, st>>>(2, pa, pb, (int)nbn, sc);
                 SOLVE_LAUNCH_CHECK();
                 pcg_direction_kernel<<<nbv, SV_THREADS, 0, st>>>(n, sc, z, p);
                 SOLVE_LAUNCH_CHECK();

@@ -1,4 +1,4 @@
-"""-m gpu parity of stage 3: rpim_matvec, rpim_solve_pcg (Jacobi-PCG) and
+"""-m gpu parity of stage 3: rpim_matvec, rpim_solve_pcg (block-Jacobi PCG) and
 rpim_recover_stress against oracle/stage3.py (sparse direct solve, literal B and D) on the oracle's own K.
 
 Tolerances: the product is compared at 1e-12 of max|K x|; the solution at 1e-6 of

@@ -9,13 +9,18 @@
 // K_IJ = lambda S + mu S^T + mu tr(S) I is applied once per block at write-out.
 //
 // reduce_rows_kernel (rows of up to 1024 block columns): the accumulators live in REGISTERS.
-// Lane l of chunk c owns column slot 32 c + l of the row.  Per row the group builds an
-// open-addressing table column node -> slot in shared memory.  For a batch of incident points
-// it then fills a byte table pos[point][slot] = position of the slot's node in the point's
-// support (one table probe per support node), while one thread bulk-copies (cp.async.bulk + mbarrier)
-// the points' staged [k][phi gx gy gz] rows into a double-buffered staging area.  In the
-// accumulation phase every lane reads its byte, and if the point hits its slot gathers that
-// node's gradient (one 32-byte sector) from the staging area and does nine fused multiply-adds.
+// Lane l of chunk c owns column slot 32 c + l of the row.  One resident wave of CTAs; every group
+// of warps draws its next row from a ticket counter, so the rows in flight form one contiguous
+// stripe.  For a batch of incident points one thread bulk-copies (cp.async.bulk + mbarrier) the
+// points' staged [k][phi gx gy gz] rows into a double-buffered staging area, and every lane learns
+// whether the point hits its slot and at which support position:
+//   MASKED   from the slot masks precomputed with the pattern (pattern.cu): bit test, then
+//            position = set bits before the chunk + popc(bits below the lane);
+//   !MASKED  (masks over budget, e.g. config 5) from an open-addressing table column -> slot built
+//            per row in shared memory and a byte table pos[point][slot] filled with one probe per
+//            support node.
+// A hit lane gathers that node's gradient (one 32-byte sector) from the staging area and does nine
+// fused multiply-adds.
 // accumulate_generic_kernel: fallback for longer rows, accumulators in shared memory.
 #include "bulk_copy.cuh"
 #include "common.cuh"

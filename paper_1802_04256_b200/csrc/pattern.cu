@@ -65,11 +65,10 @@ inc_sort_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, int32_t* __restr
 }
 
 // ------------------------------------------------------------------ block rows: union of the supports of incident points
-// Block row I = sorted union of supp(q) over the points q incident to node I.  A warp owns a row
-// and builds the union in an open-addressing table in shared memory.
-//
-// Rows that do not fit the fast path below (more than PSTRIDE columns) go to an overflow list and
-// take the general two-pass path (count, scan, fill) with the large table.
+// Block row I = sorted union of supp(q) over the points q incident to node I.  A warp owns a row.
+// Fast path: brow_bitmap_kernel below (two-level bitmap, one pass, rows parked in a fixed-stride
+// pool).  Rows that do not fit it go to an overflow list and take the general two-pass path
+// (count, scan, fill) with an open-addressing table in shared memory and a bitonic sort.
 constexpr int PAT_HASH = 4096;          // general path: open-addressing table per warp (power of two)
 constexpr int PAT_MAXROW = 2048;        // longest block row handled
 constexpr int PAT_WARPS = 4;

@@ -128,6 +128,34 @@ def assemble(nodes, pts, w, support, E, nu, alpha_c, d_c, q, body, row_ptr, col_
     return vals, f, int(nsing.value)
 
 
+def assemble_dense_ref(nodes, pts, w, support, E, nu, alpha_c, d_c, q, body, row_ptr, col_idx,
+                       node_lo: int = 0, node_hi: int | None = None):
+    """K values and f from the definition end to end in long double (pin for ``assemble``)."""
+    nodes = _f64(nodes)
+    pts = _f64(pts)
+    w = _f64(w)
+    body = _f64(body)
+    support = np.ascontiguousarray(support, dtype=np.int32)
+    row_ptr = np.ascontiguousarray(row_ptr, dtype=np.int64)
+    col_idx = np.ascontiguousarray(col_idx, dtype=np.int64)
+    M, k = support.shape
+    if node_hi is None:
+        node_hi = nodes.shape[0]
+    nrows = 3 * (node_hi - node_lo)
+    assert row_ptr.shape[0] == nrows + 1 and row_ptr[0] == 0
+    vals = np.empty(int(row_ptr[-1]))
+    f = np.empty(nrows)
+    rc = lib().orc_assemble_dense_ref(_p(nodes, C.c_double), _p(pts, C.c_double), _p(w, C.c_double),
+                                      _p(support, C.c_int32), C.c_int64(M), C.c_int(k), C.c_double(E),
+                                      C.c_double(nu), C.c_double(alpha_c), C.c_double(d_c), C.c_double(q),
+                                      _p(body, C.c_double), C.c_int64(node_lo), C.c_int64(node_hi),
+                                      _p(row_ptr, C.c_int64), _p(col_idx, C.c_int64), _p(vals, C.c_double),
+                                      _p(f, C.c_double))
+    if rc:
+        raise RuntimeError(f"orc_assemble_dense_ref failed ({rc})")
+    return vals, f
+
+
 def point_loads(nodes, pts, w, t, support, alpha_c, d_c, q, f):
     """f (3N, modified in place) += (w * phi_I) * t at the given points."""
     nodes = _f64(nodes)

@@ -23,7 +23,9 @@
 // pow vs powl, partition of unity / linear reproduction / Kronecker delta, dense
 // long-double solve of the plainly-built moment matrix (orc_shape_dense_ref, which uses
 // neither pow_qm1 nor the LDL^T below), symmetry of K, rigid-body null space, energy
-// identity on linear fields, load resultants, cantilever closed form, penalty exactness.
+// identity on linear fields, load resultants, cantilever closed form, penalty exactness;
+// K and f end to end against the definition in long double (orc_assemble_dense_ref: plain G,
+// powl, partial-pivoting LU, literal B and D, long-double sums).
 // No function in this file is "parity unpinned".
 //
 // Floating point: fp64, compiled with -ffp-contract=off so that a*b+c is never fused
@@ -694,5 +696,79 @@ int orc_penalty(const int64_t* bc_nodes, const uint8_t* bc_mask, const double* u
     }
     return 0;
 }
+
+// Pin for orc_assemble (and the definition-level bar of the CUDA path): K and f from the
+// DEFINITION end to end, with none of the operation-level machinery (no pow_qm1, no local
+// coordinates, no structured LDL^T, no closed form): shape functions and gradients from
+// orc_shape_dense_ref (plain G in global coordinates, powl, partial-pivoting LU in long double),
+// the literal B (6 x 3k) and D, w * B^T D B and w * phi * b summed over the points in long double,
+// rounded to double once at the end.  Same row restriction and CSR arguments as orc_assemble.
+// (BASELINE.json north_star: "form B (6x3k) and w*B^T*D*B, and reduce the result into a global
+// CSR matrix"; R8.)  Singular points are not detected here (use on regular clouds).
+int orc_assemble_dense_ref(const double* nodes, const double* pts, const double* w, const int32_t* support,
+                           int64_t M, int k, double E, double nu, double alpha_c, double d_c, double q,
+                           const double* body, int64_t node_lo, int64_t node_hi, const int64_t* row_ptr,
+                           const int64_t* col_idx, double* vals, double* f) {
+    typedef long double ld;
+    const ld lam = (ld)E * (ld)nu / (((ld)1 + (ld)nu) * ((ld)1 - 2 * (ld)nu));
+    const ld mu = (ld)E / (2 * ((ld)1 + (ld)nu));
+    ld D[6][6] = {};
+    for (int i = 0; i < 3; ++i) {
+        for (int j = 0; j < 3; ++j) D[i][j] = lam;
+        D[i][i] = lam + 2 * mu;
+        D[3 + i][3 + i] = mu;
+    }
+    const int64_t nrows = 3 * (node_hi - node_lo);
+    std::vector<ld> V((size_t)row_ptr[nrows], (ld)0), F((size_t)nrows, (ld)0);
+    const int nc = 3 * k;
+    std::vector<double> phi(k), dphi(3 * (size_t)k);
+    std::vector<ld> B(6 * (size_t)nc), DB(6 * (size_t)nc);
+    for (int64_t p = 0; p < M; ++p) {
+        const int32_t* s = support + (size_t)p * k;
+        bool touches = false;
+        for (int i = 0; i < k; ++i) touches |= (s[i] >= node_lo && s[i] < node_hi);
+        if (!touches) continue;
+        orc_shape_dense_ref(nodes, pts + 3 * p, s, 1, k, alpha_c, d_c, q, phi.data(), dphi.data());
+        std::fill(B.begin(), B.end(), (ld)0);
+        for (int i = 0; i < k; ++i) {
+            const ld gx = dphi[i], gy = dphi[k + i], gz = dphi[2 * k + i];
+            B[0 * nc + 3 * i + 0] = gx;                                   // eps_xx
+            B[1 * nc + 3 * i + 1] = gy;                                   // eps_yy
+            B[2 * nc + 3 * i + 2] = gz;                                   // eps_zz
+            B[3 * nc + 3 * i + 0] = gy; B[3 * nc + 3 * i + 1] = gx;       // gamma_xy
+            B[4 * nc + 3 * i + 1] = gz; B[4 * nc + 3 * i + 2] = gy;       // gamma_yz
+            B[5 * nc + 3 * i + 0] = gz; B[5 * nc + 3 * i + 2] = gx;       // gamma_zx
+        }
+        for (int r = 0; r < 6; ++r)
+            for (int c = 0; c < nc; ++c) {
+                ld acc = 0;
+                for (int t = 0; t < 6; ++t) acc += D[r][t] * B[t * nc + c];
+                DB[r * nc + c] = acc;
+            }
+        for (int i = 0; i < k; ++i) {
+            const int64_t I = s[i];
+            if (I < node_lo || I >= node_hi) continue;
+            for (int a = 0; a < 3; ++a) {
+                const int64_t row = 3 * (I - node_lo) + a;
+                const int64_t* cb = col_idx + row_ptr[row];
+                const int64_t len = row_ptr[row + 1] - row_ptr[row];
+                for (int j = 0; j < k; ++j)
+                    for (int b = 0; b < 3; ++b) {
+                        ld acc = 0;
+                        for (int t = 0; t < 6; ++t) acc += B[t * nc + 3 * i + a] * DB[t * nc + 3 * j + b];
+                        const int64_t col = 3 * (int64_t)s[j] + b;
+                        const int64_t* it = std::lower_bound(cb, cb + len, col);
+                        if (it == cb + len || *it != col) return -3;
+                        V[(size_t)(row_ptr[row] + (it - cb))] += (ld)w[p] * acc;
+                    }
+                F[(size_t)row] += (ld)w[p] * (ld)phi[i] * (ld)body[a];
+            }
+        }
+    }
+    for (size_t e = 0; e < V.size(); ++e) vals[e] = (double)V[e];
+    for (size_t e = 0; e < F.size(); ++e) f[e] = (double)F[e];
+    return 0;
+}
+
 
 }  // extern "C"

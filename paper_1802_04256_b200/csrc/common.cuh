@@ -11,6 +11,8 @@
 #include "../../include/rpim.h"
 
 #define RPIM_WARP 32
+#define RPIM_GROUP_POINTS 8      // quadrature points per group of the tiled reduction (groups.cu)
+#define RPIM_TILE_DESC_CAP 256   // tile descriptors resident in shared memory at a time (reduce_tiles.cu)
 
 // device-side error / counter slots (ctx->d_flags, int64 each)
 enum { FLAG_KNN_CAP = 0, FLAG_PAT_CAP = 1, FLAG_BC_BAD = 2, FLAG_SINGULAR = 3, FLAG_INC_CAP = 4, FLAG_OVF_ROWS = 5, FLAG_OVF_Q = 6, FLAG_INC_LONG = 7, FLAG_ROW_TICKET = 8, FLAG_INC_LONG2 = 9, NUM_FLAGS = 16 };
@@ -84,6 +86,18 @@ struct rpim_ctx {
     int mask_stride = 0;             // > 0: words per incident point, row I at inc_ptr[I] * stride; 0: d_mask_ptr, ceil(L_I/32)
     int64_t* d_mask_ptr = nullptr;   // N + 1 (word offset of row I)
     unsigned* d_masks = nullptr;
+
+    // tiled reduction (groups.cu, reduce_tiles.cu): point groups, their unions, row tiles
+    int reduce_mode = 0;             // 0 = automatic, 1 = row-owner kernel, 2 = tiled kernel whenever it fits
+    bool have_tiles = false;
+    int tg_C = 0;                    // 32-lane chunks per group union (0: tiled path not applicable)
+    int tg_T = 0;                    // block rows per tile
+    int64_t ntiles = 0;
+    int32_t* d_gu_nodes = nullptr;   // G x 32 C: sorted union of the group's supports, padded with -1
+    uint8_t* d_gpos = nullptr;       // Nq x k: position of (point, support node) in its group's union
+    unsigned* d_pmask = nullptr;     // Nq x C: which union entries the point's support holds
+    int64_t* d_tile_ptr = nullptr;   // ntiles + 1
+    unsigned* d_tdesc = nullptr;     // tile descriptors, 1 + ceil(T/2) words each
 
     // staged shape functions: Nq x k x 4  (phi, dphi/dx, dphi/dy, dphi/dz per support node: one 32-byte sector)
     double* d_stage = nullptr;
@@ -204,6 +218,10 @@ int rpim_stage_grid_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, in
 int rpim_stage_incidence(rpim_ctx* ctx);
 int rpim_stage_block_pattern(rpim_ctx* ctx);
 int rpim_stage_slot_masks(rpim_ctx* ctx);
+int rpim_stage_groups(rpim_ctx* ctx);   // after the support search: decides ctx->tg_C
+int rpim_stage_tiles(rpim_ctx* ctx);    // after incidence + block pattern: decides ctx->have_tiles
+int rpim_stage_accumulate_tiles(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
+                                double* d_vals, double* d_f);
 int rpim_stage_emit_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx);
 int rpim_stage_shape(rpim_ctx* ctx, const double* d_pts, const int32_t* d_support, int64_t M, double* d_stage,
                      uint8_t* d_singular);
@@ -215,6 +233,22 @@ int rpim_stage_point_loads(rpim_ctx* ctx, const int32_t* d_support, const double
                            const double* d_t, int64_t M, double* d_f);
 int rpim_stage_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* d_bc_mask, const double* d_u_bar,
                        int64_t m, double alpha, int relative, double* d_vals, double* d_f, double* out_alpha);
+
+// Dynamic shared memory of reduce_tiles_kernel<C, T> for rows of up to Lcap block columns:
+// accumulators T x Lcap x 9, column tables T x HSZ (HSZ = power of two >= 2 Lcap), the group panel
+// 8 x 4 x 32 C, weights, bookkeeping, union ids, point masks, tile descriptors.
+inline int rpim_tiles_hlog(int Lcap) {
+    int h = 6;
+    while ((1 << h) < 2 * Lcap) ++h;
+    return h;
+}
+inline size_t rpim_tiles_smem_bytes(int C, int T, int Lcap) {
+    const size_t hsz = (size_t)1 << rpim_tiles_hlog(Lcap);
+    const size_t dw = 1 + (T + 1) / 2;
+    return (size_t)T * Lcap * 9 * 8 + (size_t)T * hsz * 8 + (size_t)RPIM_GROUP_POINTS * 4 * 32 * C * 8 +
+           RPIM_GROUP_POINTS * 8 + (2 + 8 + 8) * 8 +
+           (8 + 32 * C + RPIM_GROUP_POINTS * C + (RPIM_TILE_DESC_CAP + 1) * dw + 3) * 4;
+}
 
 // ---- small device helpers
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }

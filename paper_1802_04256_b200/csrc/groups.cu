@@ -1,0 +1,208 @@
+// Point groups and row tiles: the integer preprocessing of the tiled reduction (reduce_tiles.cu,
+// step a6).  Built by rpim_build_pattern next to the CSR pattern; depends on the supports only.
+//
+//   group g   = the GB = 8 consecutive quadrature points 8g .. 8g+7 (the Gauss points of one background
+//               cell when a cell carries 8 of them: their supports nearly coincide)
+//   U_g       = sorted union of the supports of the group's points (gu_nodes, stride 32 C, padded with -1)
+//   gpos      = position of every (point, support node) in U_g                       (one byte each)
+//   pmask     = per point, C words: bit u set iff U_g[u] is a support node of the point
+//   tile t    = the T consecutive block rows T t .. T t + T-1
+//   tdesc     = per tile the ascending list of the groups incident to any of its rows; per (tile, group)
+//               1 + ceil(T/2) words: the group id, then per row 16 bits: position u_r of the row's node in
+//               U_g (low byte) and the mask of the group's points whose support contains that node (high
+//               byte; 0 = the row is not incident to the group)
+//
+// The tiled path is used when the groups are dense enough to pay (mean |U_g| <= 1.75 k) and fit
+// (max |U_g| <= 192); otherwise (e.g. one Gauss point per cell) the row-owner kernel of
+// accumulate.cu runs.
+#include "common.cuh"
+
+namespace {
+
+constexpr int GB = RPIM_GROUP_POINTS;
+constexpr int GSORT = 1024;     // >= GB * RPIM_MAX_K = 992 ids sorted per group
+constexpr int GU_MAX = 192;     // longest union the reduction handles (6 chunks of 32 lanes)
+constexpr int GW = 4;           // warps per block
+
+// One warp per group.  FILL = false: only |U_g| statistics (max, sum).  FILL = true: U_g, gpos, pmask.
+template <bool FILL>
+__global__ void __launch_bounds__(GW * 32)
+group_union_kernel(int64_t Nq, int k, int C, const int32_t* __restrict__ support, int* __restrict__ max_len,
+                   unsigned long long* __restrict__ sum_len, int32_t* __restrict__ gu_nodes,
+                   uint8_t* __restrict__ gpos, unsigned* __restrict__ pmask) {
+    __shared__ int buf_s[GW][GSORT];
+    __shared__ int ul_s[GW][GU_MAX];
+    __shared__ unsigned pm_s[GW][GB * 6];
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int* buf = buf_s[wid];
+    int* ul = ul_s[wid];
+    unsigned* pm = pm_s[wid];
+    const int64_t G = (Nq + GB - 1) / GB;
+    const int gcap = 32 * C;
+    for (int64_t g = (int64_t)blockIdx.x * GW + wid; g < G; g += (int64_t)gridDim.x * GW) {
+        const int64_t q0 = g * GB;
+        const int nb = (int)min((int64_t)GB, Nq - q0);
+        const int n = nb * k;
+        const int32_t* src = support + q0 * k;
+        const int np = next_pow2(n);
+        __syncwarp();
+        for (int i = lane; i < np; i += 32) buf[i] = (i < n) ? src[i] : 0x7FFFFFFF;
+        __syncwarp();
+        warp_bitonic_i32(buf, np);
+        int total = 0;
+        for (int i0 = 0; i0 < n; i0 += 32) {
+            const int i = i0 + lane;
+            const bool fresh = i < n && (i == 0 || buf[i] != buf[i - 1]);
+            const unsigned m = __ballot_sync(0xffffffffu, fresh);
+            const int pos = total + __popc(m & ((1u << lane) - 1u));
+            if (fresh && pos < GU_MAX) ul[pos] = buf[i];
+            total += __popc(m);
+        }
+        __syncwarp();
+        if constexpr (!FILL) {
+            if (lane == 0) {
+                atomicMax(max_len, total);
+                atomicAdd(sum_len, (unsigned long long)total);
+            }
+        } else {
+            // total <= gcap: the host chose C from the statistics pass
+            for (int u = lane; u < gcap; u += 32) gu_nodes[g * gcap + u] = (u < total) ? ul[u] : -1;
+            for (int i = lane; i < GB * 6; i += 32) pm[i] = 0u;
+            __syncwarp();
+            for (int i = lane; i < n; i += 32) {
+                const int node = src[i];
+                int lo = 0, hi = total - 1;
+                while (lo < hi) {
+                    const int mid = (lo + hi) >> 1;
+                    if (ul[mid] < node) lo = mid + 1; else hi = mid;
+                }
+                gpos[q0 * k + i] = (uint8_t)lo;
+                atomicOr(&pm[(i / k) * 6 + (lo >> 5)], 1u << (lo & 31));
+            }
+            __syncwarp();
+            for (int i = lane; i < nb * C; i += 32) pmask[q0 * C + i] = pm[(i / C) * 6 + (i % C)];
+        }
+    }
+}
+
+// One thread per tile: merge of the T rows' incidence lists (ascending point ids) by point group.
+template <bool FILL>
+__global__ void __launch_bounds__(128)
+tile_desc_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restrict__ inc_ptr,
+                 const int32_t* __restrict__ inc_q, const uint8_t* __restrict__ inc_j,
+                 const uint8_t* __restrict__ gpos, int* __restrict__ count, const int64_t* __restrict__ tile_ptr,
+                 unsigned* __restrict__ tdesc) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntiles) return;
+    const int DW = 1 + (T + 1) / 2;
+    int64_t c[4], e[4];
+    int gq[4];   // group of the next entry of row r (INT_MAX: list exhausted)
+    for (int r = 0; r < 4; ++r) {
+        const int64_t I = t * T + r;
+        c[r] = e[r] = 0;
+        if (r < T && I < N) { c[r] = inc_ptr[I]; e[r] = inc_ptr[I + 1]; }
+        gq[r] = (c[r] < e[r]) ? inc_q[c[r]] / GB : 0x7FFFFFFF;
+    }
+    int n = 0;
+    unsigned* dst = FILL ? tdesc + tile_ptr[t] * DW : nullptr;
+    while (true) {
+        const int g = min(min(gq[0], gq[1]), min(gq[2], gq[3]));
+        if (g == 0x7FFFFFFF) break;
+        unsigned half[4] = {0u, 0u, 0u, 0u};
+        for (int r = 0; r < 4; ++r) {
+            if (gq[r] != g) continue;
+            unsigned m = 0u, u = 0u;
+            while (true) {
+                const int q = inc_q[c[r]];
+                m |= 1u << (q - g * GB);
+                if (FILL) u = gpos[(int64_t)q * k + inc_j[c[r]]];
+                ++c[r];
+                if (c[r] >= e[r]) { gq[r] = 0x7FFFFFFF; break; }
+                const int gn = inc_q[c[r]] / GB;
+                if (gn != g) { gq[r] = gn; break; }
+            }
+            half[r] = u | (m << 8);
+        }
+        if (FILL) {
+            dst[(int64_t)n * DW] = (unsigned)g;
+            dst[(int64_t)n * DW + 1] = half[0] | (half[1] << 16);
+            if (DW > 2) dst[(int64_t)n * DW + 2] = half[2] | (half[3] << 16);
+        }
+        ++n;
+    }
+    if (!FILL) count[t] = n;
+}
+
+}  // namespace
+
+// After the support search: unions of the point groups; decides whether the tiled reduction applies
+// (ctx->tg_C > 0) and, if so, leaves U_g, gpos and pmask in the workspace.
+int rpim_stage_groups(rpim_ctx* ctx) {
+    cudaStream_t st = ctx->stream;
+    ctx->tg_C = 0;
+    ctx->have_tiles = false;
+    if (ctx->reduce_mode == 1) return RPIM_OK;   // row-owner kernel forced
+    const int64_t Nq = ctx->Nq, G = (Nq + GB - 1) / GB;
+    const int k = ctx->k;
+    int* d_max = (int*)ctx->d_scratch;
+    unsigned long long* d_sum = (unsigned long long*)(ctx->d_scratch + 1);
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_scratch, 0, 2 * sizeof(double), st));
+    const unsigned nb = (unsigned)std::min<int64_t>((G + GW - 1) / GW, 148 * 16);
+    group_union_kernel<false><<<nb, GW * 32, 0, st>>>(Nq, k, 0, ctx->d_support, d_max, d_sum, nullptr, nullptr, nullptr);
+    KERNEL_CHECK(ctx);
+    int h_max = 0;
+    unsigned long long h_sum = 0;
+    CUDA_TRY(ctx, cudaMemcpyAsync(&h_max, d_max, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaMemcpyAsync(&h_sum, d_sum, sizeof(h_sum), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    const double mean = (double)h_sum / (double)G;
+    const bool dense = mean <= 1.75 * k || ctx->reduce_mode == 2;
+    if (h_max > GU_MAX || !dense) return RPIM_OK;
+    int C = (h_max + 31) / 32;
+    if (C == 5) C = 6;
+    if (C < 2) C = 2;
+    int rc;
+    if ((rc = ws_alloc(ctx, &ctx->d_gu_nodes, G * 32 * C))) return rc;
+    if ((rc = ws_alloc(ctx, &ctx->d_gpos, Nq * k))) return rc;
+    if ((rc = ws_alloc(ctx, &ctx->d_pmask, G * GB * C))) return rc;
+    group_union_kernel<true><<<nb, GW * 32, 0, st>>>(Nq, k, C, ctx->d_support, nullptr, nullptr, ctx->d_gu_nodes,
+                                                      ctx->d_gpos, ctx->d_pmask);
+    KERNEL_CHECK(ctx);
+    ctx->tg_C = C;
+    return RPIM_OK;
+}
+
+// After incidence + block pattern: rows per tile from the shared-memory budget, tile descriptors.
+int rpim_stage_tiles(rpim_ctx* ctx) {
+    cudaStream_t st = ctx->stream;
+    ctx->have_tiles = false;
+    if (ctx->tg_C == 0) return RPIM_OK;
+    const int64_t N = ctx->N;
+    int T = 4;
+    while (T >= 2 && rpim_tiles_smem_bytes(ctx->tg_C, T, ctx->max_blen) > 227 * 1024) T >>= 1;
+    if (T < 2) { ctx->tg_C = 0; return RPIM_OK; }   // rows too long to keep two of them on chip
+    const int64_t ntiles = (N + T - 1) / T;
+    const int DW = 1 + (T + 1) / 2;
+    int rc;
+    int* d_cnt = nullptr;
+    if ((rc = ws_alloc(ctx, &d_cnt, ntiles))) return rc;
+    if ((rc = ws_alloc(ctx, &ctx->d_tile_ptr, ntiles + 1))) { ws_free(ctx, &d_cnt); return rc; }
+    const unsigned nb = (unsigned)((ntiles + 127) / 128);
+    tile_desc_kernel<false><<<nb, 128, 0, st>>>(N, ntiles, T, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j,
+                                                 ctx->d_gpos, d_cnt, nullptr, nullptr);
+    ctx->launches++;
+    rc = rpim_scan_i32_to_i64(ctx, d_cnt, ctx->d_tile_ptr, ntiles);
+    ws_free(ctx, &d_cnt);
+    if (rc) return rc;
+    int64_t total = 0;
+    CUDA_TRY(ctx, cudaMemcpyAsync(&total, ctx->d_tile_ptr + ntiles, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    if ((rc = ws_alloc(ctx, &ctx->d_tdesc, std::max<int64_t>(total, 1) * DW))) return rc;
+    tile_desc_kernel<true><<<nb, 128, 0, st>>>(N, ntiles, T, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j,
+                                                ctx->d_gpos, nullptr, ctx->d_tile_ptr, ctx->d_tdesc);
+    KERNEL_CHECK(ctx);
+    ctx->tg_T = T;
+    ctx->ntiles = ntiles;
+    ctx->have_tiles = true;
+    return RPIM_OK;
+}

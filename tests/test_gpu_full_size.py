@@ -1,80 +1,107 @@
-"""-m gpu parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+"""-m gpu parity at BASELINE.json's FULL sizes (configs 3, 4, 5), in the launch configuration bench.py times.
 
-The oracle cannot assemble a 3M x 3M matrix in seconds, so the comparison is on SAMPLED block rows that
-it can compute one by one (its row-slab mode): for a few slabs of consecutive node ids (interior, a
-corner with boundary conditions, the last rows) every quadrature point incident to the slab is taken,
-the oracle searches its support among ALL nodes, evaluates its shape functions and assembles the
-slab's rows.  Bars as everywhere (BASELINE.json north_star): supports and CSR rows bit-exact, shape
-functions bitwise, K and f within 1e-10 relative to max|K_ii|; plus properties that hold at any size
-(monotone row_ptr, ascending supports, penalty changes exactly the constrained diagonals by alpha)."""
+What is compared, and with what (tests/gpu_harness.py `run_full_config`):
+
+* a1: the oracle searches the supports of ALL quadrature points itself; the WHOLE support table is compared
+  bit for bit.  Nothing the oracle works on is taken from the CUDA path: the points incident to a row slab
+  come from the oracle's own table.
+* a2-a6, `slope` and `large`: EVERY block row -- the node range is cut into slabs of consecutive ids, the
+  oracle (its row-slab mode, spread over the host cores) builds the CSR rows, values and loads of each slab:
+  row_ptr / col_idx bit-exact, K and f within 1e-10 of max|K_ii| (of the slab: stricter than the matrix-wide
+  scale of BASELINE.json north_star), shape functions of all points bitwise.
+* `stress` (62 GB of values): the same on seven slabs of 64 block rows -- the origin corner (bottom + two
+  roller faces), the interior, the last rows, a lateral face, a bottom edge, the first and the last z-plane.
+* a7: exactly the diagonal entries of the constrained DOFs moved, each by alpha (whole matrix on the device
+  for `slope` / `large`, the sampled rows for `stress`).
+* whole-matrix invariants of the CUDA result through rpim_matvec (SURVEY.md section 8(c) pins; PAPER.md:33 calls
+  K "asymmetric", with one support per quadrature point it is symmetric): x^T(Ky) = y^T(Kx), K r = 0
+  for the six rigid-body modes before the penalty, sum_I f_I = b * Vol; and the product itself on the sampled /
+  all rows against K[rows, :] x formed from the ORACLE's rows (offsets beyond 2^31 at `stress`).
+"""
+import os
+
 import numpy as np
 import pytest
 
 import workloads
-from gpu_harness import oracle_rows, run_cuda_rows
+from gpu_harness import run_full_config
 
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-10
 
 
-def _slabs(w, width):
-    nx, ny, nz = w.grid
-    mid = nx * ny * (nz // 2) + nx * (ny // 2) + nx // 3
-    return [(0, width), (mid, mid + width), (w.N - width, w.N)]
+def _cover(N, nslab):
+    edges = np.linspace(0, N, nslab + 1).astype(np.int64)
+    return [(int(a), int(b)) for a, b in zip(edges[:-1], edges[1:]) if b > a]
 
 
-def _check(w, g, *, want_shape):
-    assert g["row_ptr_monotone"] and g["support_sorted"]
-    assert g["nsing"] == 0
-    bc = {int(n): int(m) for n, m in zip(w.bc_nodes, w.bc_mask)}
-    for s in g["slabs"]:
-        o = oracle_rows(w, s)
-        assert o["nsing"] == 0
-        assert np.array_equal(s["support"], o["support"])                      # a1 bit-exact
-        assert np.array_equal(s["row_ptr"], o["row_ptr"])                      # a2 bit-exact
-        assert np.array_equal(s["col_idx"], o["col_idx"])
-        if want_shape:
-            assert np.array_equal(s["phi"], o["phi"])                          # a3 + a4 bitwise
-            assert np.array_equal(s["dphi"], o["dphi"])
-        # a5 + a6: scale = largest diagonal entry among the sampled rows (<= max|K_ii| of the matrix: stricter)
-        rows = np.repeat(np.arange(len(s["row_ptr"]) - 1), np.diff(s["row_ptr"]))
-        diag = s["col_idx"] == rows + 3 * s["lo"]
-        assert diag.sum() == 3 * (s["hi"] - s["lo"])
-        km = np.abs(o["vals0"][diag]).max()
-        assert np.abs(s["vals0"] - o["vals0"]).max() <= TOL * km
-        assert np.abs(s["f0"] - o["f0"]).max() <= TOL * max(np.abs(o["f0"]).max(), 1e-300)
-        # a7: alpha = 1e8 * max K_ii is at least 1e8 * (largest sampled diagonal); exactly the constrained
-        # diagonals moved, each by alpha; u_bar = 0 on these configs so f is untouched
-        assert g["alpha"] >= w.penalty_alpha * np.abs(s["vals0"][diag]).max()
-        changed = s["vals"] != s["vals0"]
-        expect = np.zeros_like(changed)
-        dpos = np.nonzero(diag)[0]
-        for r, p in zip(rows[dpos], dpos):
-            node, c = divmod(int(r), 3)
-            if (bc.get(node + s["lo"], 0) >> c) & 1:
-                expect[p] = True
-        assert np.array_equal(changed, expect)
-        if expect.any():
-            assert np.allclose(s["vals"][expect] - s["vals0"][expect], g["alpha"], rtol=1e-12, atol=0)
-        assert np.array_equal(s["f"], s["f0"])
+def _check_common(w, r):
+    assert r["nsing"] == 0
+    assert r["support_equal"], "support table differs from the oracle's"            # a1, whole table
+    assert r["row_ptr_monotone"]
+    km = r["alpha"] / w.penalty_alpha                                                # max_i K_ii (R10)
+    inv = r["invariants"]
+    print(f"{w.name}: nnz={r['nnz']} sym={inv['sym']:.2e} rigid/Kmax={inv['rigid'] / km:.2e} "
+          f"fsum_err={inv['fsum_err']:.2e} torque_err={inv['torque_err']:.2e}")
+    # measured on B200 (round 2): sym 7e-20..2e-19, rigid 7e-16..2e-15 of max|K_ii|, fsum <= 1 ulp
+    assert inv["sym"] <= 1e-13
+    assert inv["rigid"] <= 1e-13 * km                         # max|K r| / max|r| for the six rigid-body modes
+    assert inv["fsum_err"] <= 1e-13 and inv["qw_err"] <= 1e-12
+    assert inv["torque_err"] <= 1e-12
+    worst = 0.0
+    for s in r["slabs"]:
+        assert s["pattern_ok"], (s["lo"], s["hi"])                                   # a2 bit-exact
+        assert s["nsing"] == 0 and s["ndiag"] == 3 * (s["hi"] - s["lo"])
+        assert s["km"] <= km * (1 + 1e-12)
+        assert s["err_K"] <= TOL * s["km"], (s["lo"], s["err_K"] / s["km"])          # a5 + a6
+        assert s["err_f"] <= TOL * max(s["fmax"], 1e-300)
+        assert s["err_Kx"] <= 1e-12 * km
+        worst = max(worst, s["err_K"] / s["km"])
+    print(f"{w.name}: {sum(s['hi'] - s['lo'] for s in r['slabs'])} block rows compared in {len(r['slabs'])} slabs, "
+          f"{sum(s['npts'] for s in r['slabs'])} point evaluations, max|dK|/max|K_ii| = {worst:.2e}")
 
 
-@pytest.mark.parametrize("name,width", [("slope", 48), ("large", 64)])
-def test_full_size_sampled_rows(name, width):
+@pytest.mark.parametrize("name", ["slope", "large"])
+def test_full_size_every_block_row(name):
     w = workloads.config(name)
-    g = run_cuda_rows(w, _slabs(w, width), want_shape=True)
-    assert g["bits"] == (64 if name == "large" else 32)
-    _check(w, g, want_shape=True)
+    r = run_full_config(w, whole=True, slabs=_cover(w.N, 16 if name == "slope" else 20), want_shape=True)
+    assert r["bits"] == (64 if name == "large" else 32)
+    _check_common(w, r)
+    assert sum(s["hi"] - s["lo"] for s in r["slabs"]) == w.N                         # all rows, once
+    assert r["phi_equal"] and r["dphi_equal"] and r["oracle_nsing"] == 0             # a3 + a4 bitwise, all points
+    assert np.array_equal(np.sort(r["penalty_changed"]), r["penalty_expected"])      # a7
+    assert np.allclose(r["penalty_delta"], r["alpha"], rtol=1e-12, atol=0)
+    assert r["f_untouched"]
+
+
+def _stress_slabs(w, width=64):
+    nx, ny, nz = w.grid
+    node = lambda ix, iy, iz: ix + nx * (iy + ny * iz)
+    starts = [0,                                     # origin corner: bottom + both roller faces
+              node(nx // 3, ny // 2, nz // 2),       # interior
+              w.N - width,                           # last rows (far top corner)
+              node(nx // 4, 0, nz // 2),             # lateral face y = 0
+              node(nx // 2, ny - 1, 0),              # bottom edge y = max
+              node(nx // 2, ny // 2, 0),             # first z-plane (bottom, fully constrained)
+              node(16, ny // 2, nz - 1)]             # last z-plane (free surface)
+    return [(s, s + width) for s in starts]
 
 
 def test_stress_full_size_sampled_rows():
-    """Config 5 (2,048,000 nodes, 16M points, k = 60, nnz 7.8e9, int64 CSR): needs ~172 GB of HBM."""
+    """Config 5 (2,048,000 nodes, 16M points, k = 60, nnz 7.8e9, int64 CSR): needs ~172 GB of HBM.
+    Not having that memory is a FAILURE unless RPIM_TEST_SKIP_STRESS=1 is set explicitly."""
     import torch
     free_b, _ = torch.cuda.mem_get_info()
-    if free_b < 176 * 2**30:
-        pytest.skip(f"needs about 172 GiB of free device memory, {free_b / 2**30:.0f} GiB free")
+    if free_b < 174 * 2**30:
+        if os.environ.get("RPIM_TEST_SKIP_STRESS") == "1":
+            pytest.skip(f"RPIM_TEST_SKIP_STRESS=1 and only {free_b / 2**30:.0f} GiB free")
+        pytest.fail(f"config 5 needs about 172 GiB of free device memory, {free_b / 2**30:.0f} GiB free "
+                    "(set RPIM_TEST_SKIP_STRESS=1 to opt out)")
     w = workloads.config("stress")
-    g = run_cuda_rows(w, _slabs(w, 16), want_shape=False)
-    assert g["bits"] == 64 and g["nnz"] > 2**31
-    _check(w, g, want_shape=False)
+    slabs = _stress_slabs(w)
+    r = run_full_config(w, whole=False, slabs=slabs, want_shape=False)
+    assert r["bits"] == 64 and r["nnz"] > 2**31
+    _check_common(w, r)
+    for s in r["slabs"]:
+        assert s["penalty_ok"], (s["lo"], s["hi"])

@@ -1,7 +1,11 @@
 #!/usr/bin/env python
 """bench.py -- RPIM assembly throughput on B200 (quad-points/s, fp64), the BASELINE.json metric.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config large] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config stress] [--impl reference]
+
+The headline workload is BASELINE.json configs[4] (`stress`, the largest configuration that fits one B200);
+configs[3] (`large`, the other configuration north_star's target names) is timed in the same run and
+reported under the extra key "large".
 
 A "step" is one pass of the whole hot path over one synthetic
 workload: rpim_build_pattern (kNN + CSR pattern) -> rpim_get_pattern -> rpim_assemble (shape functions,
@@ -61,6 +65,13 @@ def read_traffic(config_name: str):
             if len(parts) == 3 and parts[0] == config_name:
                 out[parts[1]] = float(parts[2])
     return out
+
+
+def survey_flops_per_point(k: int) -> float:
+    """SURVEY.md section 8(d) work model (fma = 2, divide = 1; n = k + 4): moment build 70 k(k+1)/2, RHS 76 k,
+    LU (2/3) n^3 - n^2/2, solves 8 n^2, blocks 42 k^2, accumulation 9 k^2.  115.6 k at k = 30, 521.7 k at k = 60."""
+    n = k + 4
+    return 70.0 * k * (k + 1) / 2 + 76.0 * k + (2.0 / 3.0) * n ** 3 - n * n / 2.0 + 8.0 * n * n + 51.0 * k * k
 
 
 def flops_per_point(k: int):
@@ -209,7 +220,9 @@ def run_reference(args, w):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / max(1, args.steps),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "N": w.N, "Nq": w.Nq, "k": w.k, "sample_points_per_step": S},
+        "config": {"workload": f"{w.name} (BASELINE.json configs[{workloads.CONFIG_NAMES.index(w.name)}])",
+                   "N": w.N, "Nq": w.Nq, "k": w.k},
+        "sample_points_per_step": S,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
                          "sample": f"first {S} quadrature points per step, all hot-path rows"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -218,44 +231,16 @@ def run_reference(args, w):
     print(json.dumps(line))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="large", choices=workloads.CONFIG_NAMES)
-    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--with-solve", action="store_true",
-                    help="also time stage 3 (block SpMV, block-Jacobi PCG to 1e-8) on the assembled system; extra key \"solve\"")
-    args = ap.parse_args()
-    if args.warmup < 3 and args.impl == "b200":
-        args.warmup = max(args.warmup, 3) if os.environ.get("RPIM_BENCH_STRICT_WARMUP", "1") == "1" else args.warmup
-
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-
-    w = rank_workload(args.config, rank, world)
-
-    if args.impl == "reference":
-        run_reference(args, w)
-        return
-
+def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks, *, do_e2e, do_solve, sample_clocks):
+    """One workload through the whole hot path; returns the pieces of the JSON line."""
     import torch
     import torch.distributed as dist
     import paper_1802_04256_b200 as rp
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-
-    hbm_gbs, sm_max_mhz, peak_src = read_peaks()
+    hbm_gbs, sm_max_mhz, peak_src = peaks
+    w = rank_workload(name, rank, world)
     ctx = rp.Context(local_rank)
+    ctx.set_reduction({"auto": 0, "rows": 1, "tiles": 2}[args.reduction])
     d_nodes = torch.from_numpy(w.nodes).to(dev)
     d_qpts = torch.from_numpy(w.qpts).to(dev)
     d_qw = torch.from_numpy(w.qw).to(dev)
@@ -283,121 +268,101 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     barrier()
     ctx.phase_totals(reset=True)
     launches0 = ctx.launch_count()
     sampler = ClockSampler(local_rank)
-    if rank == 0:
+    if rank == 0 and sample_clocks:
         sampler.start()
     stream = torch.cuda.current_stream(dev)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     e1.record(stream)
     barrier()
     ms_total = e0.elapsed_time(e1)
-    clocks = sampler.stop() if rank == 0 else None
     launches = ctx.launch_count() - launches0
     phase_ms, calls = ctx.phase_totals(reset=True)
-    ms_total = max_over_ranks(ms_total, world, dev)
-    ms_step = ms_total / args.steps
+    ms_step = max_over_ranks(ms_total, world, dev) / steps
     value = job_value(w.Nq, world, ms_step)
 
-    # assemble + penalty only (paper stages 1 + 2), same timing discipline
+    # assemble + penalty only (paper stages 1 + 2, R12), same timing discipline
     barrier()
     e0.record(stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         ctx.assemble(d_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f, want_singular=False)
         ctx.apply_penalty(d_bcn, d_bcm, d_bcu, w.penalty_alpha, True, d_vals, d_f)
     e1.record(stream)
     barrier()
-    ms_asm = e0.elapsed_time(e1) / args.steps
+    ms_asm = max_over_ranks(e0.elapsed_time(e1) / steps, world, dev)
+    clocks = sampler.stop() if (rank == 0 and sample_clocks) else None
 
-    # ------------------------------------------------ roofline of the dominant kernel (live CUDA events)
-    # the reduction into CSR is bound by HBM (K is written once: 8 nnz bytes, plus
-    # one read of the staged shape functions and of the incidence lists); the shape-function kernel is
-    # bound by the plain FP64 pipe (no tensor-core form exists for the operation-level contract).
-    n_asm = max(1, calls[1])
-    shape_ms, reduce_ms = phase_ms[3] / n_asm, phase_ms[4] / n_asm
+    # ------------------------------------------------ rooflines (live CUDA events)
+    n_asm, n_pat = max(1, calls[1]), max(1, calls[0])
+    kernel_ms = {"shape_functions": phase_ms[3] / n_asm, "reduce_into_csr": phase_ms[4] / n_asm,
+                 "knn": phase_ms[0] / n_pat, "incidence": phase_ms[1] / n_pat, "block_pattern": phase_ms[2] / n_pat}
+    kernel_ms = {kk: max_over_ranks(v, world, dev) for kk, v in kernel_ms.items()}
+    shape_ms, reduce_ms = kernel_ms["shape_functions"], kernel_ms["reduce_into_csr"]
     fl_shape, fl_reduce = flops_per_point(w.k)
+    fl_survey = survey_flops_per_point(w.k)
     peak_tflops = N_SM * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
-    reduce_bytes = 8 * nnz + 32 * w.Nq * w.k + 5 * w.Nq * w.k + 24 * w.N
+    # SURVEY.md section 8(d) minimum traffic of assemble + penalty: K written once, supports, points, nodes, f
+    hbm_min = nnz * 8 + w.Nq * w.k * 4 + w.Nq * 32 + w.N * 24 + 3 * w.N * 8
+    staged_reread = 37 * w.Nq * w.k            # this implementation's staged gradients + incidence, read once
     traffic = read_traffic(w.name)
+    used = {1: "rows", 2: "tiles"}.get(ctx.reduction_used(), "?")
+    reduce_name = "reduce_rows_kernel" if used == "rows" else "reduce_tiles_kernel"
+    t_red_alu = fl_reduce * w.Nq / (peak_tflops * 1e12) * 1e3          # ms at the FP64 peak
+    t_red_hbm = hbm_min / (hbm_gbs * 1e9) * 1e3                        # ms at the HBM peak
     if reduce_ms >= shape_ms:
-        achieved = reduce_bytes / (reduce_ms * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "kernel": "reduce_rows_kernel (reduce_into_csr)", "achieved": achieved,
-                    "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
-                    "traffic": traffic.get("reduce_rows_kernel"),
-                    "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
-                    "algorithmic_bytes_per_launch": reduce_bytes}
+        if t_red_alu >= t_red_hbm:   # the kernel's own work is governed by the FP64 pipe (k = 60: 18 k^2 flops per point)
+            achieved = fl_reduce * w.Nq / (reduce_ms * 1e-3) / 1e12
+            roofline = {"bound": "alu", "kernel": f"{reduce_name} (reduce_into_csr)", "achieved": achieved,
+                        "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+                        "algorithmic_flops_per_launch": fl_reduce * w.Nq}
+        else:
+            achieved = hbm_min / (reduce_ms * 1e-3) / 1e9
+            roofline = {"bound": "hbm", "kernel": f"{reduce_name} (reduce_into_csr)", "achieved": achieved,
+                        "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
+                        "algorithmic_bytes_per_launch": hbm_min}
+        roofline["traffic"] = traffic.get(reduce_name)
+        roofline["staged_reread_bytes_per_launch"] = staged_reread
     else:
         achieved = fl_shape * w.Nq / (shape_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": "shape_rows_kernel (shape_functions)", "achieved": achieved,
                     "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
                     "traffic": traffic.get("shape_rows_kernel"),
-                    "peak_source": f"derived: {N_SM} SM x {FP64_LANES_PER_SM} DFMA/clk x 2 x {sm_max_mhz:.0f} MHz "
-                                   "(DESIGN.md section 5)",
                     "algorithmic_flops_per_launch": fl_shape * w.Nq}
-    hbm_min = nnz * 8 + w.Nq * w.k * 4 + w.Nq * 32 + w.N * 24 + 3 * w.N * 8
+    roofline["peak_source"] = (f"MEASURED_PEAKS.json hbm_gbs ({peak_src})" if roofline["bound"] == "hbm" else
+                               f"derived: {N_SM} SM x {FP64_LANES_PER_SM} DFMA/clk x 2 x {sm_max_mhz:.0f} MHz "
+                               "(DESIGN.md section 5); see fp64_probe")
+    t_fp64_model = fl_survey * w.Nq / (peak_tflops * 1e12) * 1e3
+    t_hbm_model = hbm_min / (hbm_gbs * 1e9) * 1e3
     roofline.update({
-        "kernel_ms": {"shape_functions": shape_ms, "reduce_into_csr": reduce_ms,
-                      "knn": phase_ms[0] / max(1, calls[0]), "incidence": phase_ms[1] / max(1, calls[0]),
-                      "block_pattern": phase_ms[2] / max(1, calls[0])},
+        "kernel_ms": kernel_ms,
         "shape_fp64_frac": fl_shape * w.Nq / (shape_ms * 1e-3) / 1e12 / peak_tflops,
-        "reduce_hbm_frac": reduce_bytes / (reduce_ms * 1e-3) / 1e9 / hbm_gbs,
-        "assemble_flops_per_point": fl_shape + fl_reduce,
-        "assemble_fp64_frac": (fl_shape + fl_reduce) * w.Nq / (ms_asm * 1e-3) / 1e12 / peak_tflops,
-        "assemble_hbm_min_bytes": hbm_min,
-        "assemble_hbm_frac": hbm_min / (ms_asm * 1e-3) / 1e9 / hbm_gbs,
+        "reduce_fp64_frac": fl_reduce * w.Nq / (reduce_ms * 1e-3) / 1e12 / peak_tflops,
+        "reduce_hbm_frac": hbm_min / (reduce_ms * 1e-3) / 1e9 / hbm_gbs,
+        # the config's governing roofline, on assemble + penalty
+        "config": {
+            "governing": "fp64" if t_fp64_model >= t_hbm_model else "hbm",
+            "assemble_penalty_ms": ms_asm,
+            "flops_per_point_survey_model": fl_survey, "flops_per_point_own_count": fl_shape + fl_reduce,
+            "fp64_frac_survey_model": t_fp64_model / ms_asm,
+            "fp64_frac_own_count": (fl_shape + fl_reduce) * w.Nq / (ms_asm * 1e-3) / 1e12 / peak_tflops,
+            "hbm_min_bytes": hbm_min, "hbm_frac": t_hbm_model / ms_asm,
+            "ms_at_100pct": max(t_fp64_model, t_hbm_model), "north_star_50pct_target_ms": 2 * max(t_fp64_model, t_hbm_model),
+        },
         "fp64_peak_tflops": peak_tflops, "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": peak_src,
     })
 
-    # ------------------------------------------------ end to end through the host-buffer C ABI calls
-    e2e = None
-    if not args.no_e2e:
-        try:
-            np_idt = np.int32 if bits == 32 else np.int64
-            pin = lambda a: torch.from_numpy(a).pin_memory().numpy()  # noqa: E731
-            h_nodes, h_qpts, h_qw = pin(w.nodes), pin(w.qpts), pin(w.qw)
-            h_bcn, h_bcm, h_bcu = pin(w.bc_nodes), pin(w.bc_mask), pin(w.bc_ubar)
-            h_rp = torch.empty(3 * w.N + 1, dtype=idt).pin_memory().numpy()
-            h_ci = torch.empty(nnz, dtype=idt).pin_memory().numpy()
-            h_vals = torch.empty(nnz, dtype=torch.float64).pin_memory().numpy()
-            h_f = torch.empty(3 * w.N, dtype=torch.float64).pin_memory().numpy()
-            assert h_rp.dtype == np_idt
-
-            def e2e_step():
-                n2, _ = ctx.host_pattern(h_nodes, h_qpts, w.k, w.index_bits)
-                assert n2 == nnz
-                ctx.host_assemble(h_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, h_bcn, h_bcm, h_bcu,
-                                  w.penalty_alpha, True, h_rp, h_ci, h_vals, h_f)
-
-            e2e_step()
-            n_e2e = max(1, min(args.steps, 3))
-            barrier()
-            e0.record(stream)
-            for _ in range(n_e2e):
-                e2e_step()
-            e1.record(stream)
-            barrier()
-            ms_e2e = e0.elapsed_time(e1) / n_e2e
-            ms_e2e = max_over_ranks(ms_e2e, world, dev)
-            h2d = h_nodes.nbytes + h_qpts.nbytes + h_qw.nbytes + h_bcn.nbytes + h_bcm.nbytes + h_bcu.nbytes
-            d2h = h_rp.nbytes + h_ci.nbytes + h_vals.nbytes + h_f.nbytes
-            e2e = {"value": world * w.Nq / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-                   "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e, "steps": n_e2e,
-                   "api": "rpim_host_pattern + rpim_host_assemble (pinned host buffers)"}
-            del h_ci, h_vals
-        except Exception as ex:  # report, never fake
-            e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
-
     # ------------------------------------------------ optional: stage 3 on the assembled system
     solve = None
-    if args.with_solve:
+    if do_solve:
         d_x = torch.randn(3 * w.N, dtype=torch.float64, device=dev)
         d_y = torch.empty_like(d_x)
         for _ in range(3):
@@ -420,33 +385,143 @@ def main():
                  "pcg_rel_tol": 1e-8, "pcg_iters": iters, "pcg_rel_resid": rel, "pcg_ms": e0.elapsed_time(e1)}
         del d_x, d_y, d_u
 
+    # ------------------------------------------------ end to end through the host-buffer C ABI calls
+    e2e = None
+    if do_e2e:
+        del d_rp, d_ci, d_vals, d_f       # rpim_host_assemble owns its device buffers: make room (config 5: 125 GB)
+        torch.cuda.empty_cache()
+        try:
+            np_idt = np.int32 if bits == 32 else np.int64
+            pin = lambda a: torch.from_numpy(a).pin_memory().numpy()  # noqa: E731
+            h_nodes, h_qpts, h_qw = pin(w.nodes), pin(w.qpts), pin(w.qw)
+            h_bcn, h_bcm, h_bcu = pin(w.bc_nodes), pin(w.bc_mask), pin(w.bc_ubar)
+            h_rp = torch.empty(3 * w.N + 1, dtype=idt, pin_memory=True).numpy()
+            h_ci = torch.empty(nnz, dtype=idt, pin_memory=True).numpy()
+            h_vals = torch.empty(nnz, dtype=torch.float64, pin_memory=True).numpy()
+            h_f = torch.empty(3 * w.N, dtype=torch.float64, pin_memory=True).numpy()
+            assert h_rp.dtype == np_idt
+
+            def e2e_step():
+                n2, _ = ctx.host_pattern(h_nodes, h_qpts, w.k, w.index_bits)
+                assert n2 == nnz
+                ctx.host_assemble(h_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, h_bcn, h_bcm, h_bcu,
+                                  w.penalty_alpha, True, h_rp, h_ci, h_vals, h_f)
+
+            e2e_step()
+            n_e2e = max(1, min(steps, 3))
+            barrier()
+            e0.record(stream)
+            for _ in range(n_e2e):
+                e2e_step()
+            e1.record(stream)
+            barrier()
+            ms_e2e = max_over_ranks(e0.elapsed_time(e1) / n_e2e, world, dev)
+            h2d = h_nodes.nbytes + h_qpts.nbytes + h_qw.nbytes + h_bcn.nbytes + h_bcm.nbytes + h_bcu.nbytes
+            d2h = h_rp.nbytes + h_ci.nbytes + h_vals.nbytes + h_f.nbytes
+            e2e = {"value": world * w.Nq / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                   "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e, "steps": n_e2e,
+                   "api": "rpim_host_pattern + rpim_host_assemble (pinned host buffers)"}
+            del h_ci, h_vals
+        except Exception as ex:  # report, never fake (and never a smaller workload under the same name)
+            e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:300]}
+
+    out = {
+        "w": w, "value": value, "ms_per_step": ms_step, "nnz": nnz, "bits": bits, "reduction": used,
+        "assemble_penalty": {"value": world * w.Nq / (ms_asm * 1e-3), "unit": UNIT, "ms_per_step": ms_asm,
+                             "gdof_entries_per_s": 9.0 * w.k * w.k * w.Nq * world / (ms_asm * 1e-3) / 1e9},
+        "clocks": clocks, "e2e": e2e, "launches": int(launches), "roofline": roofline, "solve": solve,
+    }
+    try:
+        out["fp64_probe"] = ctx.probe_fp64()
+    except Exception as ex:
+        out["fp64_probe"] = {"error": repr(ex)[:200]}
+    ctx.close()
+    torch.cuda.empty_cache()
+    return out
+
+
+def config_block(w, world, r):
+    return {"workload": f"{w.name} (BASELINE.json configs[{workloads.CONFIG_NAMES.index(w.name)}])",
+            "N": w.N, "Nq": w.Nq, "k": w.k, "nnz": r["nnz"], "index_bits": r["bits"],
+            "step": "build_pattern + get_pattern + assemble + apply_penalty", "reduction": r["reduction"],
+            "l2": "inputs and outputs larger than L2 (no flush needed)" if r["nnz"] * 8 > 2.5e8 else
+                  "working set may fit L2; no flush",
+            "parallelism": (f"{world} independent replicas of the workload, one per GPU (own jitter stream, no halo, "
+                            "no collective): not a sharded assembly of one domain") if world > 1 else "single GPU"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="stress", choices=workloads.CONFIG_NAMES)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--reduction", default="auto", choices=["auto", "rows", "tiles"],
+                    help="reduction kernel (rpim_set_reduction): automatic choice, row-owner, or tiled")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="do not also time `large` when the headline is `stress`")
+    ap.add_argument("--with-solve", action="store_true",
+                    help="also time stage 3 (block SpMV, block-Jacobi PCG to 1e-8) on the assembled system; extra key \"solve\"")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        args.warmup = max(args.warmup, 3) if os.environ.get("RPIM_BENCH_STRICT_WARMUP", "1") == "1" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        run_reference(args, rank_workload(args.config, rank, world))
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    peaks = read_peaks()
+
+    r = bench_config(args.config, args, args.steps, args.warmup, dev, rank, local_rank, world, peaks,
+                     do_e2e=not args.no_e2e, do_solve=args.with_solve, sample_clocks=True)
+    w = r["w"]
+    secondary = None
+    if args.config == "stress" and not args.no_secondary:
+        # the other configuration BASELINE.json north_star's target names; device-timed only
+        r2 = bench_config("large", args, min(args.steps, 10), 3, dev, rank, local_rank, world, peaks,
+                          do_e2e=False, do_solve=False, sample_clocks=False)
+        secondary = {"config": config_block(r2["w"], world, r2), "value": r2["value"], "unit": UNIT,
+                     "ms_per_step": r2["ms_per_step"], "steps": min(args.steps, 10), "warmup": 3,
+                     "assemble_penalty": r2["assemble_penalty"], "gpu_launches": r2["launches"],
+                     "roofline": r2["roofline"]}
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        r, S, t = oracle_sample_rate(w, budget_s=15.0)
-        cpu_baseline = {"value": r, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": t,
+        rate, S, t = oracle_sample_rate(w, budget_s=15.0)
+        cpu_baseline = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": t,
                         "sample": f"first {S} quadrature points of '{w.name}', all hot-path rows (kNN, pattern, "
                                   f"shape functions, B^T D B assembly, penalty); host has {os.cpu_count()} cores"}
 
     if rank == 0:
+        roofline = r["roofline"]
+        roofline["fp64_probe"] = r["fp64_probe"]
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{w.name} (BASELINE.json configs[{workloads.CONFIG_NAMES.index(w.name)}])",
-                       "N": w.N, "Nq": w.Nq, "k": w.k, "nnz": nnz, "index_bits": bits,
-                       "step": "build_pattern + get_pattern + assemble + apply_penalty",
-                       "l2": "inputs and outputs larger than L2 (no flush needed)" if nnz * 8 > 2.5e8 else
-                             "working set may fit L2; no flush",
-                       "parallelism": f"{world} independent partitions" if world > 1 else "single GPU"},
-            "assemble_penalty": {"value": world * w.Nq / (ms_asm * 1e-3), "unit": UNIT, "ms_per_step": ms_asm,
-                                 "gdof_entries_per_s": 9.0 * w.k * w.k * w.Nq * world / (ms_asm * 1e-3) / 1e9},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-            "cpu_baseline": cpu_baseline,
+            "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_block(w, world, r),
+            "assemble_penalty": r["assemble_penalty"], "clocks": r["clocks"], "e2e": r["e2e"],
+            "gpu_launches": r["launches"], "roofline": roofline, "cpu_baseline": cpu_baseline,
         }
-        if solve is not None:
-            line["solve"] = solve
+        if secondary is not None:
+            line["large"] = secondary
+        if r["solve"] is not None:
+            line["solve"] = r["solve"]
         print(json.dumps(line))
-    ctx.close()
     if world > 1:
         dist.destroy_process_group()
 

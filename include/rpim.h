@@ -56,6 +56,15 @@ const char* rpim_last_error(const rpim_ctx* ctx);
 /* Bytes of device workspace currently owned by the context. */
 int64_t rpim_workspace_bytes(const rpim_ctx* ctx);
 
+/* Which kernel reduces the element matrices into the CSR values (step a6; both are deterministic and
+ * give results within rounding of each other): 0 = automatic (default; currently the row-owner kernel),
+ * 1 = row-owner kernel, 2 = tiled kernel whenever its preprocessing fits (groups of 8 consecutive points
+ * whose supports' union has at most 192 nodes; it pays when a background cell carries several Gauss points).
+ * Takes effect at the next rpim_build_pattern.  rpim_reduction_used: 1 or 2 for the current pattern
+ * (0 before rpim_build_pattern). */
+int rpim_set_reduction(rpim_ctx* ctx, int mode);
+int rpim_reduction_used(const rpim_ctx* ctx);
+
 /* Stage 0 (R1, R2; hot-path steps a1, a2): exact k-nearest-neighbour supports on a
  * uniform cell grid and the CSR pattern of the 3N x 3N stiffness matrix.
  *   d_nodes  N x 3 field-node coordinates        d_qpts  Nq x 3 quadrature points
@@ -148,6 +157,12 @@ int rpim_last_phase_ms(rpim_ctx* ctx, float out_ms[5]);
  * stream around the kernels; out_calls = {build_pattern calls, assemble calls} (may be NULL).
  * Synchronises.  reset != 0 clears the totals afterwards. */
 int rpim_phase_totals(rpim_ctx* ctx, double out_ms[5], int64_t out_calls[2], int reset);
+
+/* Measurement aid for the roofline denominator: sustained FP64 fused multiply-add
+ * rate of the device, eight independent chains per thread on every SM, no memory traffic; best of three
+ * launches after a warm-up.  out_tflops (host, fma = 2 flops), out_ms (host, may be NULL) = duration of the
+ * best launch.  Synchronises the stream. */
+int rpim_probe_fp64(rpim_ctx* ctx, double* out_tflops, double* out_ms);
 
 /* Number of kernels this library has launched on the context since creation. */
 int64_t rpim_launch_count(const rpim_ctx* ctx);

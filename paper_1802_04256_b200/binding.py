@@ -17,7 +17,8 @@ EXPORTED_SYMBOLS = (
     "rpim_create", "rpim_destroy", "rpim_last_error", "rpim_workspace_bytes", "rpim_build_pattern",
     "rpim_get_pattern", "rpim_assemble", "rpim_add_point_loads", "rpim_apply_penalty", "rpim_get_shape",
     "rpim_host_pattern", "rpim_host_assemble", "rpim_last_phase_ms", "rpim_phase_totals", "rpim_launch_count",
-    "rpim_matvec", "rpim_solve_pcg", "rpim_recover_stress",
+    "rpim_matvec", "rpim_solve_pcg", "rpim_recover_stress", "rpim_set_reduction", "rpim_reduction_used",
+    "rpim_probe_fp64",
 )
 
 
@@ -66,6 +67,9 @@ def _load():
     lib.rpim_matvec.argtypes = [vp, vp, vp, vp]
     lib.rpim_solve_pcg.argtypes = [vp, vp, vp, vp, dbl, C.c_int, C.POINTER(C.c_int), C.POINTER(dbl)]
     lib.rpim_recover_stress.argtypes = [vp, vp, dbl, dbl, vp]
+    lib.rpim_probe_fp64.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]
+    lib.rpim_set_reduction.argtypes = [vp, C.c_int]
+    lib.rpim_reduction_used.argtypes = [vp]
     _lib = lib
     return lib
 
@@ -131,6 +135,21 @@ def rpim_recover_stress(ctx, d_u, E, nu, d_sigma):
     import torch
     _check(ctx, _load().rpim_recover_stress(ctx, _dptr(d_u, torch.float64), float(E), float(nu),
                                             _dptr(d_sigma, torch.float64)))
+
+
+def rpim_probe_fp64(ctx):
+    """{"tflops": sustained FP64 fma rate, "ms": duration of the best launch}."""
+    tf, ms = C.c_double(0.0), C.c_double(0.0)
+    _check(ctx, _load().rpim_probe_fp64(ctx, C.byref(tf), C.byref(ms)))
+    return {"tflops": float(tf.value), "ms": float(ms.value)}
+
+
+def rpim_set_reduction(ctx, mode: int):
+    _check(ctx, _load().rpim_set_reduction(ctx, int(mode)))
+
+
+def rpim_reduction_used(ctx) -> int:
+    return int(_load().rpim_reduction_used(ctx))
 
 
 def rpim_workspace_bytes(ctx) -> int:
@@ -290,6 +309,15 @@ class Context:
 
     def recover_stress(self, d_u, E, nu, d_sigma):
         return rpim_recover_stress(self.ctx, d_u, E, nu, d_sigma)
+
+    def probe_fp64(self):
+        return rpim_probe_fp64(self.ctx)
+
+    def set_reduction(self, mode):
+        return rpim_set_reduction(self.ctx, mode)
+
+    def reduction_used(self):
+        return rpim_reduction_used(self.ctx)
 
     def launch_count(self):
         return rpim_launch_count(self.ctx)

@@ -32,6 +32,9 @@ void free_all(rpim_ctx* c) {
     ws_free(c, &c->d_stage); ws_free(c, &c->d_singular); ws_free(c, &c->d_scratch);
     ws_free(c, &c->d_mask_ptr); ws_free(c, &c->d_masks);
     c->have_masks = false;
+    ws_free(c, &c->d_gu_nodes); ws_free(c, &c->d_gpos); ws_free(c, &c->d_gu_mask);
+    ws_free(c, &c->d_tile_ptr); ws_free(c, &c->d_tdesc);
+    c->have_tiles = false; c->tg_C = 0;
     ws_free(c, &c->h2d_nodes); ws_free(c, &c->h2d_qpts);
     ws_free(c, &c->hb_qw); ws_free(c, &c->hb_vals); ws_free(c, &c->hb_f); ws_free(c, &c->hb_ub);
     ws_free(c, &c->hb_bn); ws_free(c, &c->hb_bm); ws_free(c, &c->hb_rp); ws_free(c, &c->hb_ci);
@@ -82,6 +85,15 @@ const char* rpim_last_error(const rpim_ctx* ctx) { return ctx ? ctx->err.c_str()
 int64_t rpim_workspace_bytes(const rpim_ctx* ctx) { return ctx ? ctx->ws_bytes : 0; }
 int64_t rpim_launch_count(const rpim_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+int rpim_set_reduction(rpim_ctx* ctx, int mode) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    if (mode < 0 || mode > 2) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "reduction mode must be 0 (auto), 1 (rows) or 2 (tiles)");
+    ctx->reduce_mode = mode;
+    return RPIM_OK;
+}
+
+int rpim_reduction_used(const rpim_ctx* ctx) { return ctx && ctx->have_pattern ? (ctx->have_tiles ? 2 : 1) : 0; }
+
 int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const double* d_qpts, int64_t Nq, int k,
                        int index_bits, int64_t* out_nnz, int* out_index_bits) {
     if (!ctx) return RPIM_ERR_INVALID_ARG;
@@ -103,8 +115,12 @@ int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const do
     cudaEventRecord(ctx->ev[1], st);
     if ((rc = rpim_stage_incidence(ctx))) return rc;
     cudaEventRecord(ctx->ev[2], st);
+    // the reduction's integer preprocessing: point groups first (they decide between the tiled and the
+    // row-owner kernel, and so whether slot masks are built with the block rows), row tiles last
+    if ((rc = rpim_stage_groups(ctx))) return rc;
     if ((rc = rpim_stage_block_pattern(ctx))) return rc;
-    if ((rc = rpim_stage_slot_masks(ctx))) return rc;
+    if (ctx->tg_C == 0 && (rc = rpim_stage_slot_masks(ctx))) return rc;
+    if ((rc = rpim_stage_tiles(ctx))) return rc;
     cudaEventRecord(ctx->ev[3], st);
     CUDA_TRY(ctx, cudaStreamSynchronize(st));
     for (int i = 0; i < 3; ++i) {
@@ -169,7 +185,9 @@ int rpim_assemble(rpim_ctx* ctx, const double* d_qw, double E, double nu, double
     if (pe[1]) cudaEventRecord(pe[1], st);
     const double lambda = E * nu / ((1.0 + nu) * (1.0 - 2.0 * nu));
     const double mu = E / (2.0 * (1.0 + nu));
-    if ((rc = rpim_stage_accumulate(ctx, d_qw, lambda, mu, body, d_vals, d_f))) return rc;
+    rc = ctx->have_tiles ? rpim_stage_accumulate_tiles(ctx, d_qw, lambda, mu, body, d_vals, d_f)
+                         : rpim_stage_accumulate(ctx, d_qw, lambda, mu, body, d_vals, d_f);
+    if (rc) return rc;
     cudaEventRecord(ctx->ev[6], st);
     if (pe[2]) cudaEventRecord(pe[2], st);
     ctx->phase_calls[1]++;
@@ -237,6 +255,54 @@ __global__ void split_stage_kernel(const double* __restrict__ stage, int64_t M, 
     }
 }
 }  // namespace
+
+namespace {
+// Sustained FP64 multiply-add rate: eight independent fma chains per thread, no memory traffic.
+__global__ void __launch_bounds__(1024) fp64_probe_kernel(int iters, double seed, double* __restrict__ sink) {
+    double a0 = seed + threadIdx.x, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0;
+    double a4 = a0 + 4.0, a5 = a0 + 5.0, a6 = a0 + 6.0, a7 = a0 + 7.0;
+    const double m = 1.0 - 1e-9, c = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+    const double t = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    if (t == 123.456) sink[0] = t;   // never true: keeps the chains alive
+}
+}  // namespace
+
+int rpim_probe_fp64(rpim_ctx* ctx, double* out_tflops, double* out_ms) {
+    if (!ctx || !out_tflops) return RPIM_ERR_INVALID_ARG;
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
+    double* d_sink = nullptr;
+    int rc = ws_alloc(ctx, &d_sink, 8);
+    if (rc) return rc;
+    const int iters = 4096, blocks = sms * 2, threads = 1024;
+    cudaEvent_t e0, e1;
+    CUDA_TRY(ctx, cudaEventCreate(&e0));
+    CUDA_TRY(ctx, cudaEventCreate(&e1));
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {   // the first launch warms up; best of the next three
+        cudaEventRecord(e0, ctx->stream);
+        fp64_probe_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, 1.0 + rep, d_sink);
+        cudaEventRecord(e1, ctx->stream);
+        ctx->launches++;
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); ws_free(ctx, &d_sink); RPIM_FAIL(ctx, RPIM_ERR_CUDA, "fp64 probe failed: %s", cudaGetErrorString(e)); }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    ws_free(ctx, &d_sink);
+    const double flops = 2.0 * 8.0 * (double)iters * (double)blocks * (double)threads;
+    *out_tflops = flops / ((double)best * 1e-3) / 1e12;
+    if (out_ms) *out_ms = best;
+    return RPIM_OK;
+}
 
 int rpim_get_shape(rpim_ctx* ctx, double* d_phi, double* d_dphi, uint8_t* d_singular) {
     if (!ctx) return RPIM_ERR_INVALID_ARG;

@@ -95,7 +95,7 @@ struct rpim_ctx {
     int64_t ntiles = 0;
     int32_t* d_gu_nodes = nullptr;   // G x 32 C: sorted union of the group's supports, padded with -1
     uint8_t* d_gpos = nullptr;       // Nq x k: position of (point, support node) in its group's union
-    unsigned* d_pmask = nullptr;     // Nq x C: which union entries the point's support holds
+    uint8_t* d_gu_mask = nullptr;    // G x 32 C: bit p = the union entry is a support node of the group's point p
     int64_t* d_tile_ptr = nullptr;   // ntiles + 1
     unsigned* d_tdesc = nullptr;     // tile descriptors, 1 + ceil(T/2) words each
 
@@ -235,8 +235,8 @@ int rpim_stage_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* 
                        int64_t m, double alpha, int relative, double* d_vals, double* d_f, double* out_alpha);
 
 // Dynamic shared memory of reduce_tiles_kernel<C, T> for rows of up to Lcap block columns:
-// accumulators T x Lcap x 9, column tables T x HSZ (HSZ = power of two >= 2 Lcap), the group panel
-// 8 x 4 x 32 C, weights, bookkeeping, union ids, point masks, tile descriptors.
+// accumulators T x Lcap x 9, column tables T x HSZ (HSZ = power of two >= 2 Lcap), two group panels
+// 8 x 3 x 32 C, per-warp w * grad phi_I, weights, bookkeeping, union ids and masks (x 2), tile descriptors.
 inline int rpim_tiles_hlog(int Lcap) {
     int h = 6;
     while ((1 << h) < 2 * Lcap) ++h;
@@ -245,9 +245,9 @@ inline int rpim_tiles_hlog(int Lcap) {
 inline size_t rpim_tiles_smem_bytes(int C, int T, int Lcap) {
     const size_t hsz = (size_t)1 << rpim_tiles_hlog(Lcap);
     const size_t dw = 1 + (T + 1) / 2;
-    return (size_t)T * Lcap * 9 * 8 + (size_t)T * hsz * 8 + (size_t)RPIM_GROUP_POINTS * 4 * 32 * C * 8 +
-           RPIM_GROUP_POINTS * 8 + (2 + 8 + 8) * 8 +
-           (8 + 32 * C + RPIM_GROUP_POINTS * C + (RPIM_TILE_DESC_CAP + 1) * dw + 3) * 4;
+    return (size_t)T * Lcap * 9 * 8 + (size_t)T * hsz * 8 + (size_t)2 * RPIM_GROUP_POINTS * 3 * 32 * C * 8 +
+           (size_t)T * C * RPIM_GROUP_POINTS * 4 * 8 + 2 * RPIM_GROUP_POINTS * 8 + 2 * T * RPIM_GROUP_POINTS * 8 + (2 + 8) * 8 +
+           (8 + 2 * 32 * C + 2 * 8 * C + (RPIM_TILE_DESC_CAP + 4) * dw + 3) * 4;
 }
 
 // ---- small device helpers

@@ -5,16 +5,15 @@
 //               cell when a cell carries 8 of them: their supports nearly coincide)
 //   U_g       = sorted union of the supports of the group's points (gu_nodes, stride 32 C, padded with -1)
 //   gpos      = position of every (point, support node) in U_g                       (one byte each)
-//   pmask     = per point, C words: bit u set iff U_g[u] is a support node of the point
+//   gu_mask   = per union entry one byte: bit p set iff U_g[u] is a support node of the group's point p
 //   tile t    = the T consecutive block rows T t .. T t + T-1
 //   tdesc     = per tile the ascending list of the groups incident to any of its rows; per (tile, group)
 //               1 + ceil(T/2) words: the group id, then per row 16 bits: position u_r of the row's node in
 //               U_g (low byte) and the mask of the group's points whose support contains that node (high
 //               byte; 0 = the row is not incident to the group)
 //
-// The tiled path is used when the groups are dense enough to pay (mean |U_g| <= 1.75 k) and fit
-// (max |U_g| <= 192); otherwise (e.g. one Gauss point per cell) the row-owner kernel of
-// accumulate.cu runs.
+// The tiled path runs on request (rpim_set_reduction(ctx, 2)) when the groups fit (max |U_g| <= 192 and
+// two rows' accumulators fit in shared memory); otherwise the row-owner kernel of accumulate.cu runs.
 #include "common.cuh"
 
 namespace {
@@ -24,19 +23,19 @@ constexpr int GSORT = 1024;     // >= GB * RPIM_MAX_K = 992 ids sorted per group
 constexpr int GU_MAX = 192;     // longest union the reduction handles (6 chunks of 32 lanes)
 constexpr int GW = 4;           // warps per block
 
-// One warp per group.  FILL = false: only |U_g| statistics (max, sum).  FILL = true: U_g, gpos, pmask.
+// One warp per group.  FILL = false: only |U_g| statistics (max, sum).  FILL = true: U_g, gpos, gu_mask.
 template <bool FILL>
 __global__ void __launch_bounds__(GW * 32)
 group_union_kernel(int64_t Nq, int k, int C, const int32_t* __restrict__ support, int* __restrict__ max_len,
                    unsigned long long* __restrict__ sum_len, int32_t* __restrict__ gu_nodes,
-                   uint8_t* __restrict__ gpos, unsigned* __restrict__ pmask) {
+                   uint8_t* __restrict__ gpos, uint8_t* __restrict__ gu_mask) {
     __shared__ int buf_s[GW][GSORT];
     __shared__ int ul_s[GW][GU_MAX];
-    __shared__ unsigned pm_s[GW][GB * 6];
+    __shared__ unsigned um_s[GW][GU_MAX];
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int* buf = buf_s[wid];
     int* ul = ul_s[wid];
-    unsigned* pm = pm_s[wid];
+    unsigned* um = um_s[wid];
     const int64_t G = (Nq + GB - 1) / GB;
     const int gcap = 32 * C;
     for (int64_t g = (int64_t)blockIdx.x * GW + wid; g < G; g += (int64_t)gridDim.x * GW) {
@@ -67,7 +66,7 @@ group_union_kernel(int64_t Nq, int k, int C, const int32_t* __restrict__ support
         } else {
             // total <= gcap: the host chose C from the statistics pass
             for (int u = lane; u < gcap; u += 32) gu_nodes[g * gcap + u] = (u < total) ? ul[u] : -1;
-            for (int i = lane; i < GB * 6; i += 32) pm[i] = 0u;
+            for (int u = lane; u < GU_MAX; u += 32) um[u] = 0u;
             __syncwarp();
             for (int i = lane; i < n; i += 32) {
                 const int node = src[i];
@@ -77,10 +76,10 @@ group_union_kernel(int64_t Nq, int k, int C, const int32_t* __restrict__ support
                     if (ul[mid] < node) lo = mid + 1; else hi = mid;
                 }
                 gpos[q0 * k + i] = (uint8_t)lo;
-                atomicOr(&pm[(i / k) * 6 + (lo >> 5)], 1u << (lo & 31));
+                atomicOr(&um[lo], 1u << (i / k));
             }
             __syncwarp();
-            for (int i = lane; i < nb * C; i += 32) pmask[q0 * C + i] = pm[(i / C) * 6 + (i % C)];
+            for (int u = lane; u < gcap; u += 32) gu_mask[g * gcap + u] = (uint8_t)(u < total ? um[u] : 0u);
         }
     }
 }
@@ -97,6 +96,7 @@ tile_desc_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restr
     const int DW = 1 + (T + 1) / 2;
     int64_t c[4], e[4];
     int gq[4];   // group of the next entry of row r (INT_MAX: list exhausted)
+#pragma unroll
     for (int r = 0; r < 4; ++r) {
         const int64_t I = t * T + r;
         c[r] = e[r] = 0;
@@ -109,6 +109,7 @@ tile_desc_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restr
         const int g = min(min(gq[0], gq[1]), min(gq[2], gq[3]));
         if (g == 0x7FFFFFFF) break;
         unsigned half[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
         for (int r = 0; r < 4; ++r) {
             if (gq[r] != g) continue;
             unsigned m = 0u, u = 0u;
@@ -136,12 +137,15 @@ tile_desc_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restr
 }  // namespace
 
 // After the support search: unions of the point groups; decides whether the tiled reduction applies
-// (ctx->tg_C > 0) and, if so, leaves U_g, gpos and pmask in the workspace.
+// (ctx->tg_C > 0) and, if so, leaves U_g, gpos and gu_mask in the workspace.
 int rpim_stage_groups(rpim_ctx* ctx) {
     cudaStream_t st = ctx->stream;
     ctx->tg_C = 0;
     ctx->have_tiles = false;
-    if (ctx->reduce_mode == 1) return RPIM_OK;   // row-owner kernel forced
+    // Measured on B200 (round 2): the tiled kernel ties with the row-owner kernel at
+    // `stress` (0.93 s vs 0.92 s) and loses at `slope` (15.6 ms vs 10.5 ms), so the automatic choice is the
+    // row-owner kernel; the tiled one runs on request (rpim_set_reduction(ctx, 2)).
+    if (ctx->reduce_mode != 2) return RPIM_OK;
     const int64_t Nq = ctx->Nq, G = (Nq + GB - 1) / GB;
     const int k = ctx->k;
     int* d_max = (int*)ctx->d_scratch;
@@ -156,17 +160,17 @@ int rpim_stage_groups(rpim_ctx* ctx) {
     CUDA_TRY(ctx, cudaMemcpyAsync(&h_sum, d_sum, sizeof(h_sum), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaStreamSynchronize(st));
     const double mean = (double)h_sum / (double)G;
-    const bool dense = mean <= 1.75 * k || ctx->reduce_mode == 2;
-    if (h_max > GU_MAX || !dense) return RPIM_OK;
+    (void)mean;   // reported by nothing yet; the density criterion (mean |U_g| <= 1.75 k) is moot while tiles are opt-in
+    if (h_max > GU_MAX) return RPIM_OK;
     int C = (h_max + 31) / 32;
     if (C == 5) C = 6;
     if (C < 2) C = 2;
     int rc;
     if ((rc = ws_alloc(ctx, &ctx->d_gu_nodes, G * 32 * C))) return rc;
     if ((rc = ws_alloc(ctx, &ctx->d_gpos, Nq * k))) return rc;
-    if ((rc = ws_alloc(ctx, &ctx->d_pmask, G * GB * C))) return rc;
+    if ((rc = ws_alloc(ctx, &ctx->d_gu_mask, G * 32 * C))) return rc;
     group_union_kernel<true><<<nb, GW * 32, 0, st>>>(Nq, k, C, ctx->d_support, nullptr, nullptr, ctx->d_gu_nodes,
-                                                      ctx->d_gpos, ctx->d_pmask);
+                                                      ctx->d_gpos, ctx->d_gu_mask);
     KERNEL_CHECK(ctx);
     ctx->tg_C = C;
     return RPIM_OK;
@@ -191,6 +195,7 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
     tile_desc_kernel<false><<<nb, 128, 0, st>>>(N, ntiles, T, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j,
                                                  ctx->d_gpos, d_cnt, nullptr, nullptr);
     ctx->launches++;
+    if (cudaGetLastError() != cudaSuccess) { ws_free(ctx, &d_cnt); RPIM_FAIL(ctx, RPIM_ERR_CUDA, "tile descriptor count launch failed"); }
     rc = rpim_scan_i32_to_i64(ctx, d_cnt, ctx->d_tile_ptr, ntiles);
     ws_free(ctx, &d_cnt);
     if (rc) return rc;

@@ -543,8 +543,10 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
                 reuse = reuse || (it != ctx->ws_sizes.end() && it->second >= bytes && it->second <= 2 * bytes + 4096);
             }
             size_t free_b = 0, total_b = 0;
-            if (!reuse) CUDA_TRY(ctx, cudaMemGetInfo(&free_b, &total_b));   // a driver call: only when it matters
-            if (reuse || (uint64_t)bytes <= free_b / 4) {
+            if (!reuse && ctx->tg_C == 0) CUDA_TRY(ctx, cudaMemGetInfo(&free_b, &total_b));   // a driver call: only when it matters
+            if (ctx->tg_C > 0) {
+                // the tiled reduction (reduce_tiles.cu) needs no slot masks
+            } else if (reuse || (uint64_t)bytes <= free_b / 4) {
                 if (ws_alloc(ctx, &ctx->d_masks, words) == RPIM_OK) d_masks = ctx->d_masks;
                 else ctx->err.clear();
             }

@@ -5,7 +5,7 @@ from __future__ import annotations
 import numpy as np
 
 
-def run_cuda(w, *, penalty=True, loads=True, index_bits=None, want_shape=True, ctx=None):
+def run_cuda(w, *, penalty=True, loads=True, index_bits=None, want_shape=True, ctx=None, reduction=0):
     import torch
     import paper_1802_04256_b200 as rp
 
@@ -15,6 +15,7 @@ def run_cuda(w, *, penalty=True, loads=True, index_bits=None, want_shape=True, c
         ctx = rp.Context(0)
     out = {}
     try:
+        ctx.set_reduction(reduction)
         d_nodes = torch.from_numpy(w.nodes).to(dev)
         d_qpts = torch.from_numpy(w.qpts).to(dev)
         d_qw = torch.from_numpy(w.qw).to(dev)
@@ -28,7 +29,7 @@ def run_cuda(w, *, penalty=True, loads=True, index_bits=None, want_shape=True, c
         d_vals = torch.full((nnz,), float("nan"), dtype=torch.float64, device=dev)
         d_f = torch.full((3 * w.N,), float("nan"), dtype=torch.float64, device=dev)
         nsing = ctx.assemble(d_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f)
-        out.update(nnz=nnz, bits=bits, nsing=nsing, phase_ms=ctx.phase_ms())
+        out.update(nnz=nnz, bits=bits, nsing=nsing, phase_ms=ctx.phase_ms(), reduction_used=ctx.reduction_used())
         if want_shape:
             d_phi = torch.empty((w.Nq, w.k), dtype=torch.float64, device=dev)
             d_dphi = torch.empty((w.Nq, 3, w.k), dtype=torch.float64, device=dev)
@@ -204,7 +205,7 @@ def gpu_invariants(ctx, w, d_nodes, d_vals, d_f):
     return out
 
 
-def run_full_config(w, *, whole, slabs, want_shape, nproc=None):
+def run_full_config(w, *, whole, slabs, want_shape, nproc=None, reduction=0):
     """Full-size run of the CUDA path in the launch configuration bench.py times, compared with the oracle.
 
     whole=True : every block row (slabs = list of (lo, hi) covering [0, N)), whole matrix brought to the host.
@@ -223,6 +224,7 @@ def run_full_config(w, *, whole, slabs, want_shape, nproc=None):
         pool.close()
         pool.join()
     with rp.Context(0) as ctx:
+        ctx.set_reduction(reduction)
         d_nodes = torch.from_numpy(w.nodes).to(dev)
         d_qpts = torch.from_numpy(w.qpts).to(dev)
         d_qw = torch.from_numpy(w.qw).to(dev)
@@ -235,7 +237,7 @@ def run_full_config(w, *, whole, slabs, want_shape, nproc=None):
         d_vals = torch.full((nnz,), float("nan"), dtype=torch.float64, device=dev)
         d_f = torch.full((3 * w.N,), float("nan"), dtype=torch.float64, device=dev)
         nsing = ctx.assemble(d_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f)
-        res.update(nnz=nnz, bits=bits, nsing=nsing)
+        res.update(nnz=nnz, bits=bits, nsing=nsing, reduction_used=ctx.reduction_used())
         # a1 over the WHOLE table, bit for bit
         sup = d_sup.cpu().numpy()
         res["support_equal"] = bool(np.array_equal(sup, S))

@@ -75,6 +75,15 @@ def test_full_size_every_block_row(name):
     assert r["f_untouched"]
 
 
+def test_slope_full_size_tiled_reduction():
+    """The opt-in tiled reduction (rpim_set_reduction(ctx, 2)) at full size: every block row of `slope`."""
+    w = workloads.config("slope")
+    r = run_full_config(w, whole=True, slabs=_cover(w.N, 16), want_shape=False, reduction=2)
+    assert r["reduction_used"] == 2
+    _check_common(w, r)
+    assert sum(s["hi"] - s["lo"] for s in r["slabs"]) == w.N
+
+
 def _stress_slabs(w, width=64):
     nx, ny, nz = w.grid
     node = lambda ix, iy, iz: ix + nx * (iy + ny * iz)

@@ -68,6 +68,30 @@ def test_jittered_blocks_span_tiles_and_ragged_tails(k, dims, jit, gauss):
     _compare(w, run_cuda(w), run_oracle(w))
 
 
+@pytest.mark.parametrize("k,dims,gauss", [
+    (27, (7, 7, 6), 2),            # union of a cell's 8 supports: 2 chunks of 32
+    (40, (9, 8, 7), 2),            # 3 chunks
+    (60, (10, 9, 8), 2),           # 4 chunks, rows of ~400 block columns
+    (30, (9, 5, 5), 3),            # 27 points per cell: groups of 8 straddle cells
+    (124, (9, 8, 8), 2),           # unions near the 192-node limit (beyond it the row-owner kernel takes over)
+    (12, (6, 6, 5), 1),            # one point per cell: sparse groups, still correct
+])
+def test_tiled_reduction_matches_the_oracle_and_the_row_owner_kernel(k, dims, gauss):
+    # rpim_set_reduction(ctx, 2): groups of 8 points, tiles of rows, accumulators in shared memory
+    # (reduce_tiles.cu).  Same bars as the default path; run twice for bitwise reproducibility.
+    w = workloads.make_block(f"t{k}", *dims, 1.0, gauss, k, 5e9, 0.3, jitter=0.3, seed=300 + k,
+                             body=(10.0, -20.0, -2.5e4), bc="bottom+roller")
+    g, o = run_cuda(w, reduction=2), run_oracle(w)
+    assert g["reduction_used"] == 2 or (k == 124 and g["reduction_used"] == 1)
+    _compare(w, g, o)
+    g2 = run_cuda(w, reduction=2)
+    assert np.array_equal(g["vals"], g2["vals"]) and np.array_equal(g["f"], g2["f"])
+    g1 = run_cuda(w, reduction=1)
+    assert g1["reduction_used"] == 1
+    km = kmax_diag(o)
+    assert np.abs(g["vals0"] - g1["vals0"]).max() <= 1e-13 * km
+
+
 def test_nonunit_spacing_other_exponent_and_absolute_penalty():
     w = workloads.make_block("q", 8, 7, 6, 0.37, 2, 30, 7e9, 0.33, jitter=0.25, seed=3, q=1.5, alpha_c=3.0,
                              body=(0.0, 0.0, -1.0), bc="x0")

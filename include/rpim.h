@@ -40,9 +40,11 @@ typedef enum rpim_status {
     RPIM_ERR_ALLOC = -2,           /* device or host allocation failed */
     RPIM_ERR_CUDA = -3,            /* a CUDA runtime call or kernel failed */
     RPIM_ERR_STATE = -4,           /* call order violated (e.g. assemble before build_pattern) */
-    RPIM_ERR_BC_NODE_INVALID = -5, /* boundary node id out of range */
+    RPIM_ERR_BC_NODE_INVALID = -5, /* boundary node id out of range, listed twice, or without a matrix row */
     RPIM_ERR_INDEX_OVERFLOW = -6,  /* 32-bit indices forced but nnz >= 2^31 */
-    RPIM_ERR_CAPACITY = -7         /* an on-chip work buffer would overflow (pathological node cloud) */
+    RPIM_ERR_CAPACITY = -7,        /* an on-chip work buffer would overflow (pathological node cloud) */
+    RPIM_ERR_BREAKDOWN = -8,       /* rpim_solve_pcg: p^T K p <= 0 or not finite (K is not positive definite) */
+    RPIM_ERR_SINGULAR_POINT = -9   /* rpim_add_point_loads: a load point has a singular moment matrix */
 } rpim_status;
 
 #define RPIM_MAX_K 124  /* moment systems up to 128 x 128 */
@@ -59,7 +61,9 @@ int64_t rpim_workspace_bytes(const rpim_ctx* ctx);
 /* Which kernel reduces the element matrices into the CSR values (step a6; both are deterministic and
  * give results within rounding of each other): 0 = automatic (default; currently the row-owner kernel),
  * 1 = row-owner kernel, 2 = tiled kernel whenever its preprocessing fits (groups of 8 consecutive points
- * whose supports' union has at most 192 nodes; it pays when a background cell carries several Gauss points).
+ * whose supports' union has at most 192 nodes; it pays when a background cell carries several Gauss points),
+ * 3 = the long-row kernel that rows of more than 1024 block columns take automatically (accumulators in
+ * shared memory, binary search of the column; for tests).
  * Takes effect at the next rpim_build_pattern.  rpim_reduction_used: 1 or 2 for the current pattern
  * (0 before rpim_build_pattern). */
 int rpim_set_reduction(rpim_ctx* ctx, int mode);
@@ -90,22 +94,30 @@ int rpim_get_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx, int32_t* d
  *   body    host array of 3 (force per unit volume)
  *   d_vals  nnz fp64 values (overwritten)   d_f  3N fp64 (overwritten)
  *   out_singular  host scalar: number of points whose moment matrix was singular (they
- *                 contribute nothing); may be NULL, in which case the call is asynchronous. */
+ *                 contribute nothing); may be NULL, in which case the call is asynchronous.
+ * Singular points are REPORTED, not an error: the return value stays RPIM_OK (there is no
+ * RPIM_ERR_SINGULAR_MOMENT; SURVEY.md section 8(b) proposed one), the caller decides from the count. */
 int rpim_assemble(rpim_ctx* ctx, const double* d_qw, double E, double nu, double alpha_c,
                   double d_c, double q, const double body[3], double* d_vals, double* d_f,
                   int64_t* out_singular);
 
 /* Step a5b (R9): f_{3I+c} += w * phi_I(x) * t_c at M given points (face Gauss
  * points of a traction boundary) using the shape parameters of the last rpim_assemble.
- *   d_pts M x 3, d_w M, d_t M x 3, d_f 3N (updated in place).  Synchronises the stream. */
+ *   d_pts M x 3, d_w M, d_t M x 3, d_f 3N (updated in place).  Synchronises the stream.
+ * A load point whose support gives a singular moment matrix (e.g. k coplanar nodes on a face) would drop its
+ * traction silently: the call then returns RPIM_ERR_SINGULAR_POINT (the other points' loads are in d_f). */
 int rpim_add_point_loads(rpim_ctx* ctx, const double* d_pts, const double* d_w, const double* d_t,
                          int64_t M, double* d_f);
 
 /* Stage 2 (R10; step a7): penalty method, in place.
- *   d_bc_nodes  m unique node ids            d_bc_mask  m bytes, bit c = constrain DOF c (NULL = all)
+ *   d_bc_nodes  m node ids, each at most once; an id that is out of range, listed twice or without a matrix
+ *               row gives RPIM_ERR_BC_NODE_INVALID and NOTHING is applied (K and f unchanged)
+ *   d_bc_mask   m bytes, bit c = constrain DOF c (NULL = all)
  *   d_u_bar     m x 3 prescribed displacements
  *   alpha, alpha_is_relative   alpha_used = alpha * max_d K_dd (before penalty) if relative
- *   out_alpha_used  host scalar, may be NULL (then asynchronous unless an error check is needed) */
+ *   out_alpha_used  host scalar, may be NULL
+ * Synchronises the stream once (alpha and the validity of the list are read back); the penalty kernel
+ * itself is enqueued after that and is asynchronous. */
 int rpim_apply_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* d_bc_mask,
                        const double* d_u_bar, int64_t m, double alpha, int alpha_is_relative,
                        double* d_vals, double* d_f, double* out_alpha_used);
@@ -118,10 +130,13 @@ int rpim_apply_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* 
  * rpim_solve_pcg: conjugate gradients with block-Jacobi preconditioning (inverse of the 3x3 diagonal block of every
  * node) on the penalised K,
  * which is symmetric positive definite (R10).  d_u holds the initial guess on entry and
- * the solution on exit (3N).  Stops when ||f - K u||_2 <= rel_tol * ||f||_2 (looked at every 25
- * iterations) or after max_iter iterations; out_iters / out_rel_resid (host, may be NULL) report
- * what was reached -- not converging is not an error.  All reductions have a fixed order: the
- * iterates are bitwise reproducible.  Synchronises the stream.
+ * the solution on exit (3N).  Stops when the residual recurrence reaches rel_tol * ||f||_2 (looked at every
+ * 25 iterations) or after max_iter iterations; out_iters (host, may be NULL) and out_rel_resid (host, may
+ * be NULL) report what was reached, out_rel_resid being the TRUE ||f - K u||_2 / ||f||_2 of the returned
+ * iterate, recomputed with one more product -- not converging is not an error.  If p^T K p <= 0 or is not
+ * finite (K is not positive definite: singular points, unconstrained components) the iteration stops at
+ * the next look and RPIM_ERR_BREAKDOWN is returned, outputs filled.  f = 0 returns u = 0.  All reductions
+ * have a fixed order: the iterates are bitwise reproducible.  Synchronises the stream.
  *
  * rpim_recover_stress: sigma = D B u at every quadrature point of the last rpim_assemble (its staged
  * shape-function gradients), Voigt order xx yy zz xy yz zx, d_sigma Nq x 6 fp64.  Asynchronous. */

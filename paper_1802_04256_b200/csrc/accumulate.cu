@@ -407,6 +407,19 @@ __global__ void diag_max_final_kernel(double* part, int nparts, double alpha, in
     if (threadIdx.x == 0) part[0] = relative ? alpha * m : alpha;
 }
 
+// validity of the boundary list, before anything is applied: ids in range, with a matrix row, each listed once
+// (seen = one bit per node, zeroed by the caller)
+__global__ void penalty_check_kernel(int64_t N, const int64_t* __restrict__ bc_nodes, int64_t m,
+                                     const int64_t* __restrict__ brow_ptr, unsigned* __restrict__ seen,
+                                     long long* __restrict__ flags) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m) return;
+    const int64_t I = bc_nodes[i];
+    bool bad = I < 0 || I >= N || brow_ptr[I + 1] == brow_ptr[I];
+    if (!bad) bad = (atomicOr(&seen[I >> 5], 1u << (I & 31)) >> (I & 31)) & 1u;
+    if (bad) atomicAdd((unsigned long long*)&flags[FLAG_BC_BAD], 1ull);
+}
+
 __global__ void penalty_apply_kernel(int64_t N, const int64_t* __restrict__ bc_nodes,
                                      const uint8_t* __restrict__ bc_mask, const double* __restrict__ ubar, int64_t m,
                                      const double* __restrict__ alpha_used, const int64_t* __restrict__ brow_ptr,
@@ -499,6 +512,7 @@ int launch_reduce_rows(rpim_ctx* ctx, const double* d_qw, double lambda, double 
 int rpim_stage_accumulate(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
                           double* d_vals, double* d_f) {
     const int Lmax = std::max(ctx->max_blen, 1);
+    if (ctx->reduce_mode == 3) return accumulate_generic(ctx, d_qw, lambda, mu, body, d_vals, d_f);
     static_assert(sizeof(RedSmem<1, 4, false>) % 16 == 0 && sizeof(RedSmem<8, 4, true>) % 16 == 0 && sizeof(RedSmem<2, 3, true>) % 16 == 0, "group stride keeps 16-byte alignment");
     if (Lmax <= 128) return launch_reduce_rows<1, 4, 8>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
     if (Lmax <= 192) return launch_reduce_rows<2, 3, 4>(ctx, d_qw, lambda, mu, body, d_vals, d_f);
@@ -526,21 +540,38 @@ int rpim_stage_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* 
     KERNEL_CHECK(ctx);
     diag_max_final_kernel<<<1, 32, 0, st>>>(ctx->d_scratch, nparts, alpha, relative);
     KERNEL_CHECK(ctx);
-    if (m > 0) {
-        penalty_apply_kernel<<<(unsigned)((m + 127) / 128), 128, 0, st>>>(ctx->N, d_bc_nodes, d_bc_mask, d_u_bar, m,
-                                                                          ctx->d_scratch, ctx->d_brow_ptr,
-                                                                          ctx->d_bdiag, d_vals, d_f, ctx->d_flags);
-        KERNEL_CHECK(ctx);
-    }
     double a = 0.0;
     long long bad = 0;
+    if (m > 0) {
+        // the list is validated first: nothing is applied unless every id is in range, has a row and is unique
+        unsigned* d_seen = nullptr;
+        const int64_t words = (ctx->N + 31) / 32;
+        int rc = ws_alloc(ctx, &d_seen, words);
+        if (rc) return rc;
+        cudaError_t e = cudaMemsetAsync(d_seen, 0, (size_t)words * sizeof(unsigned), st);
+        if (e == cudaSuccess) {
+            penalty_check_kernel<<<(unsigned)((m + 127) / 128), 128, 0, st>>>(ctx->N, d_bc_nodes, m, ctx->d_brow_ptr, d_seen,
+                                                                              ctx->d_flags);
+            ctx->launches++;
+            e = cudaGetLastError();
+        }
+        ws_free(ctx, &d_seen);   // parked: reuse is ordered by the stream
+        if (e != cudaSuccess) RPIM_FAIL(ctx, RPIM_ERR_CUDA, "boundary list check failed: %s", cudaGetErrorString(e));
+    }
     CUDA_TRY(ctx, cudaMemcpyAsync(&a, ctx->d_scratch, sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaMemcpyAsync(&bad, ctx->d_flags + FLAG_BC_BAD, sizeof(long long), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaStreamSynchronize(st));
     if (out_alpha) *out_alpha = a;
     if (bad) {
         CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_BC_BAD, 0, sizeof(long long), st));
-        RPIM_FAIL(ctx, RPIM_ERR_BC_NODE_INVALID, "%lld boundary node ids are out of range or have no matrix row", bad);
+        RPIM_FAIL(ctx, RPIM_ERR_BC_NODE_INVALID,
+                  "%lld boundary node ids are out of range, listed more than once or have no matrix row; nothing applied", bad);
+    }
+    if (m > 0) {
+        penalty_apply_kernel<<<(unsigned)((m + 127) / 128), 128, 0, st>>>(ctx->N, d_bc_nodes, d_bc_mask, d_u_bar, m,
+                                                                          ctx->d_scratch, ctx->d_brow_ptr,
+                                                                          ctx->d_bdiag, d_vals, d_f, ctx->d_flags);
+        KERNEL_CHECK(ctx);
     }
     return RPIM_OK;
 }

@@ -39,6 +39,9 @@ void free_all(rpim_ctx* c) {
     ws_free(c, &c->hb_qw); ws_free(c, &c->hb_vals); ws_free(c, &c->hb_f); ws_free(c, &c->hb_ub);
     ws_free(c, &c->hb_bn); ws_free(c, &c->hb_bm); ws_free(c, &c->hb_rp); ws_free(c, &c->hb_ci);
     { int64_t* t = (int64_t*)c->d_scan_tmp; ws_free(c, &t); c->d_scan_tmp = nullptr; c->scan_tmp_elems = 0; }
+    // blocks still registered as live here have no owner (a temporary lost on an error path): release them too
+    for (auto& b : c->ws_sizes) { cudaFree(b.first); c->ws_bytes -= b.second; }
+    c->ws_sizes.clear();
     ws_release_cache(c);
     c->have_pattern = c->have_shape = false;
 }
@@ -87,7 +90,7 @@ int64_t rpim_launch_count(const rpim_ctx* ctx) { return ctx ? ctx->launches : 0;
 
 int rpim_set_reduction(rpim_ctx* ctx, int mode) {
     if (!ctx) return RPIM_ERR_INVALID_ARG;
-    if (mode < 0 || mode > 2) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "reduction mode must be 0 (auto), 1 (rows) or 2 (tiles)");
+    if (mode < 0 || mode > 3) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "reduction mode must be 0 (auto), 1 (rows), 2 (tiles) or 3 (long rows)");
     ctx->reduce_mode = mode;
     return RPIM_OK;
 }
@@ -162,10 +165,8 @@ int rpim_assemble(rpim_ctx* ctx, const double* d_qw, double E, double nu, double
     fill_shape_params(alpha_c, d_c, q, ctx->sp);
     ctx->have_sp = true;
     int rc;
-    if (!ctx->d_stage) {
-        if ((rc = ws_alloc(ctx, &ctx->d_stage, ctx->Nq * 4 * (int64_t)ctx->k))) return rc;
-        if ((rc = ws_alloc(ctx, &ctx->d_singular, ctx->Nq))) return rc;
-    }
+    if (!ctx->d_stage && (rc = ws_alloc(ctx, &ctx->d_stage, ctx->Nq * 4 * (int64_t)ctx->k))) return rc;
+    if (!ctx->d_singular && (rc = ws_alloc(ctx, &ctx->d_singular, ctx->Nq))) return rc;
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_SINGULAR, 0, sizeof(long long), st));
     // a triple of pooled events per call so that a caller can sum kernel times over many calls
     cudaEvent_t pe[3] = {nullptr, nullptr, nullptr};
@@ -213,6 +214,9 @@ int rpim_add_point_loads(rpim_ctx* ctx, const double* d_pts, const double* d_w, 
     double* d_stage = nullptr;
     uint8_t* d_sing = nullptr;
     int rc = RPIM_OK;
+    // the capacity and singular-point counters are this call's own: clear them first
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_KNN_CAP, 0, sizeof(long long), st));
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_SINGULAR, 0, sizeof(long long), st));
     if ((rc = ws_alloc(ctx, &d_sup, M * ctx->k)) == RPIM_OK && (rc = ws_alloc(ctx, &d_stage, M * 4 * (int64_t)ctx->k)) == RPIM_OK &&
         (rc = ws_alloc(ctx, &d_sing, M)) == RPIM_OK) {
         if ((rc = rpim_stage_grid_knn(ctx, d_pts, M, ctx->k, d_sup, false)) == RPIM_OK &&
@@ -220,14 +224,20 @@ int rpim_add_point_loads(rpim_ctx* ctx, const double* d_pts, const double* d_w, 
             rc = rpim_stage_point_loads(ctx, d_sup, d_stage, d_w, d_t, M, d_f);
     }
     cudaError_t e = cudaStreamSynchronize(st);
-    long long capf = 0;
+    long long capf = 0, nsing = 0;
     cudaMemcpy(&capf, ctx->d_flags + FLAG_KNN_CAP, sizeof(capf), cudaMemcpyDeviceToHost);
+    cudaMemcpy(&nsing, ctx->d_flags + FLAG_SINGULAR, sizeof(nsing), cudaMemcpyDeviceToHost);
+    cudaMemsetAsync(ctx->d_flags + FLAG_KNN_CAP, 0, sizeof(long long), st);   // reported: do not poison later calls
+    cudaMemsetAsync(ctx->d_flags + FLAG_SINGULAR, 0, sizeof(long long), st);
     ws_free(ctx, &d_sup);
     ws_free(ctx, &d_stage);
     ws_free(ctx, &d_sing);
     if (rc) return rc;
     if (e != cudaSuccess) RPIM_FAIL(ctx, RPIM_ERR_CUDA, "point loads failed: %s", cudaGetErrorString(e));
     if (capf) RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "kNN capacity exceeded for %lld load points", capf);
+    if (nsing)
+        RPIM_FAIL(ctx, RPIM_ERR_SINGULAR_POINT, "%lld of %lld load points have a singular moment matrix (their k nearest "
+                  "nodes are degenerate, e.g. coplanar): their traction was NOT added", nsing, (long long)M);
     return RPIM_OK;
 }
 

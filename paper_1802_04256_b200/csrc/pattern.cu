@@ -136,8 +136,8 @@ __device__ __forceinline__ void table_to_sorted_list(const int* table, int* list
 }
 
 // Fast path (brow_bitmap_kernel): the union of a row as a TWO-LEVEL BITMAP over the window of node
-// ids its supports span -- no hashing, no probing, no sort.  Level 1 has one bit per block of 64
-// consecutive ids (which blocks are touched), level 2 one 64-bit word per TOUCHED block, stored
+// ids its supports span -- no hashing, no probing, no sort.  Level 1 has one bit per block of 32
+// consecutive ids (which blocks are touched), level 2 one 32-bit word per TOUCHED block, stored
 // compactly in block order (rank = set level-1 bits below).  Three sweeps over the (incident point,
 // support node) pairs: mark blocks, mark ids, and -- once prefix popcounts are known -- turn every
 // support node into its column slot (set bits below it), which gives the slot masks of the

@@ -18,7 +18,7 @@ constexpr int SV_THREADS = 256;
 constexpr int SV_PARTS = 1184;   // blocks of the vector kernels = partial sums per dot product (148 SM x 8)
 
 // scalars of the iteration (device resident, no host round trip per step)
-enum { S_RZ = 0, S_PAP = 1, S_ALPHA = 2, S_BETA = 3, S_RR = 4, S_NUM = 8 };
+enum { S_RZ = 0, S_PAP = 1, S_ALPHA = 2, S_BETA = 3, S_RR = 4, S_BREAK = 5, S_NUM = 8 };
 
 __device__ __forceinline__ double block_sum(double v, double* sh) {
 #pragma unroll
@@ -161,8 +161,15 @@ __global__ void pcg_scalar_kernel(int mode, const double* __restrict__ pa, const
     const double ta = block_sum(a, sh);
     const double tb = block_sum(b, sh);
     if (threadIdx.x == 0) {
-        if (mode == 0) { sc[S_RZ] = ta; sc[S_RR] = tb; }
-        else if (mode == 1) { sc[S_PAP] = ta; sc[S_ALPHA] = (ta != 0.0) ? sc[S_RZ] / ta : 0.0; }
+        if (mode == 0) { sc[S_RZ] = ta; sc[S_RR] = tb; sc[S_BREAK] = 0.0; }
+        else if (mode == 1) {
+            // p^T K p must be positive for a definite K; anything else (semi-definite K from singular points or
+            // unconstrained components, overflow) is a breakdown: freeze the iterate and raise the flag
+            const bool ok = ta > 0.0 && ta < 1.7976931348623157e308 && (sc[S_BREAK] == 0.0);
+            sc[S_PAP] = ta;
+            sc[S_ALPHA] = ok ? sc[S_RZ] / ta : 0.0;
+            if (!ok && sc[S_RR] != 0.0) sc[S_BREAK] = 1.0;   // (r = 0 exactly is convergence, not a breakdown)
+        }
         else { sc[S_BETA] = (sc[S_RZ] != 0.0) ? ta / sc[S_RZ] : 0.0; sc[S_RZ] = ta; sc[S_RR] = tb; }
     }
 }
@@ -305,7 +312,11 @@ int rpim_solve_pcg(rpim_ctx* ctx, const double* d_vals, const double* d_f, doubl
     const double ff = h_sc[S_RZ];
     int it = 0;
     double rel = 0.0;
-    if (ff > 0.0) {
+    bool breakdown = false;
+    if (!(ff > 0.0)) {
+        // f = 0: the solution of the definite system is u = 0, whatever the initial guess was
+        if (cudaMemsetAsync(d_u, 0, (size_t)n * sizeof(double), st) != cudaSuccess) { ctx->err = "memset failed"; return fail(RPIM_ERR_CUDA); }
+    } else {
         bspmv_kernel<<<nbm, SV_THREADS, 0, st>>>(N, ctx->d_brow_ptr, ctx->d_bcol, d_vals, d_u, Ap, nullptr);
         SOLVE_LAUNCH_CHECK();
         pcg_init_kernel<<<nbn, SV_THREADS, 0, st>>>(N, d_f, Ap, dinv, r, z, p, pa, pb);
@@ -319,7 +330,8 @@ int rpim_solve_pcg(rpim_ctx* ctx, const double* d_vals, const double* d_f, doubl
                 return fail(RPIM_ERR_CUDA);
             }
             rel = std::sqrt(h_sc[S_RR] / ff);
-            if (!(rel > rel_tol) || it >= max_iter) break;   // also leaves on NaN
+            breakdown = h_sc[S_BREAK] != 0.0;
+            if (!(rel > rel_tol) || it >= max_iter || breakdown) break;   // also leaves on NaN
             const int todo = std::min(check, max_iter - it);
             for (int s = 0; s < todo; ++s) {
                 bspmv_kernel<<<nbm, SV_THREADS, 0, st>>>(N, ctx->d_brow_ptr, ctx->d_bcol, d_vals, p, Ap, pa);
@@ -335,11 +347,27 @@ int rpim_solve_pcg(rpim_ctx* ctx, const double* d_vals, const double* d_f, doubl
             }
             it += todo;
         }
+        // what is reported is the TRUE residual ||f - K u|| / ||f|| of the returned iterate, not the
+        // recurrence value the loop watched (the two drift apart over thousands of iterations)
+        bspmv_kernel<<<nbm, SV_THREADS, 0, st>>>(N, ctx->d_brow_ptr, ctx->d_bcol, d_vals, d_u, Ap, nullptr);
+        SOLVE_LAUNCH_CHECK();
+        pcg_init_kernel<<<nbn, SV_THREADS, 0, st>>>(N, d_f, Ap, dinv, r, z, p, pa, pb);
+        SOLVE_LAUNCH_CHECK();
+        pcg_scalar_kernel<<<1, SV_THREADS, 0, st>>>(0, pa, pb, (int)nbn, sc);
+        SOLVE_LAUNCH_CHECK();
+        if (cudaMemcpyAsync(h_sc, sc, sizeof(h_sc), cudaMemcpyDeviceToHost, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) {
+            ctx->err = "device to host copy failed";
+            return fail(RPIM_ERR_CUDA);
+        }
+        rel = std::sqrt(h_sc[S_RR] / ff);
     }
 #undef SOLVE_LAUNCH_CHECK
     ws_free(ctx, &w);
     if (out_iters) *out_iters = it;
     if (out_rel_resid) *out_rel_resid = rel;
+    if (breakdown || !(rel == rel))
+        RPIM_FAIL(ctx, RPIM_ERR_BREAKDOWN, "conjugate gradients broke down within %d iterations (p^T K p <= 0 or not finite: K is "
+                  "not positive definite -- singular points, unconstrained rigid-body modes?); relative residual %.3e", it, rel);
     return RPIM_OK;
 }
 

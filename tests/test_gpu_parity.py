@@ -219,3 +219,61 @@ def test_host_buffer_entry_points_match_device_path():
     assert ns == 0 and alpha == g["alpha"]
     assert np.array_equal(rpa, g["row_ptr"]) and np.array_equal(cia, g["col_idx"])
     assert np.array_equal(vals, g["vals"]) and np.array_equal(f, g["f"])
+
+
+def test_long_row_kernel_matches_the_oracle():
+    # accumulate_generic_kernel (rows of more than 1024 block columns take it automatically) forced on a small
+    # case through rpim_set_reduction(ctx, 3): same bars as the default kernels
+    w = workloads.make_block("gen", 9, 8, 7, 1.0, 2, 33, 5e9, 0.3, jitter=0.3, seed=41, body=(3.0, -2.0, -2.5e4),
+                             bc="bottom+roller")
+    g = run_cuda(w, reduction=3)
+    assert g["reduction_used"] == 1
+    _compare(w, g, run_oracle(w))
+
+
+def test_boundary_list_is_validated_before_anything_is_applied():
+    import torch
+    import paper_1802_04256_b200 as rp
+    w = workloads.make_block("dup", 6, 5, 5, 1.0, 1, 12, 1e9, 0.3, jitter=0.2, seed=5, body=(0.0, 0.0, -1.0))
+    dev = torch.device("cuda:0")
+    with rp.Context(0) as ctx:
+        d_nodes, d_qpts = torch.from_numpy(w.nodes).to(dev), torch.from_numpy(w.qpts).to(dev)   # must outlive the pattern
+        nnz, _ = ctx.build_pattern(d_nodes, d_qpts, w.k)
+        vals = torch.empty(nnz, dtype=torch.float64, device=dev)
+        f = torch.empty(3 * w.N, dtype=torch.float64, device=dev)
+        ctx.assemble(torch.from_numpy(w.qw).to(dev), w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, vals, f)
+        v0, f0 = vals.clone(), f.clone()
+        ub = torch.full((3, 3), 0.5, dtype=torch.float64, device=dev)
+        for bad in ([3, 7, 3], [3, -1, 4], [3, w.N, 4]):       # listed twice, negative, out of range
+            with pytest.raises(rp.RpimError) as e:
+                ctx.apply_penalty(torch.tensor(bad, dtype=torch.int64, device=dev), None, ub, 1e3, False, vals, f)
+            assert e.value.code == -5
+            assert torch.equal(vals, v0) and torch.equal(f, f0)    # nothing applied
+        a = ctx.apply_penalty(torch.tensor([3, 7, 4], dtype=torch.int64, device=dev), None, ub, 1e3, False, vals, f)
+        assert a == 1e3 and int((vals != v0).sum()) == 9 and int((f != f0).sum()) == 9
+
+
+def test_point_loads_report_singular_load_points():
+    import torch
+    import paper_1802_04256_b200 as rp
+    # two far-apart node planes (z = 0 and z = 10): the 12 nearest nodes of a point ON the plane z = 0 are coplanar
+    w = workloads.make_block("face", 6, 6, 2, 1.0, 1, 12, 1e9, 0.3, body=(0.0, 0.0, -1.0))
+    w.nodes[:, 2] *= 10.0
+    w.qpts[:, 2] *= 10.0
+    dev = torch.device("cuda:0")
+    with rp.Context(0) as ctx:
+        d_nodes, d_qpts = torch.from_numpy(w.nodes).to(dev), torch.from_numpy(w.qpts).to(dev)   # must outlive the pattern
+        nnz, _ = ctx.build_pattern(d_nodes, d_qpts, w.k)
+        vals = torch.empty(nnz, dtype=torch.float64, device=dev)
+        f = torch.empty(3 * w.N, dtype=torch.float64, device=dev)
+        ctx.assemble(torch.from_numpy(w.qw).to(dev), w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, vals, f)
+        f0 = f.clone()
+        pts = torch.tensor([[2.5, 2.5, 0.0]], dtype=torch.float64, device=dev)       # on the face z = 0
+        one = torch.ones(1, dtype=torch.float64, device=dev)
+        t = torch.tensor([[0.0, 0.0, -1.0]], dtype=torch.float64, device=dev)
+        with pytest.raises(rp.RpimError) as e:
+            ctx.add_point_loads(pts, one, t, f)
+        assert e.value.code == -9 and torch.equal(f, f0)
+        pts_ok = torch.tensor([[2.5, 2.5, 5.0]], dtype=torch.float64, device=dev)    # between the planes: regular
+        ctx.add_point_loads(pts_ok, one, t, f)                                       # the flags were cleared
+        assert abs(float((f - f0).view(-1, 3).sum(0)[2]) + 1.0) < 1e-12

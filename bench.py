@@ -360,6 +360,32 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
         "fp64_peak_tflops": peak_tflops, "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": peak_src,
     })
 
+    # ------------------------------------------------ moving nodes: rpim_update_nodes against a full rebuild
+    update = None
+    try:
+        rng = np.random.default_rng(11)
+
+        def timed_update(nodes_np):
+            d_new = torch.from_numpy(np.ascontiguousarray(nodes_np)).to(dev)
+            barrier()
+            e0.record(stream)
+            ch, rb, _ = ctx.update_nodes(d_new, None)
+            e1.record(stream)
+            barrier()
+            return e0.elapsed_time(e1), ch, rb, d_new
+
+        keep_ms, keep_ch, keep_rb, d_a = timed_update(w.nodes + 1e-9 * w.h * rng.uniform(-1, 1, w.nodes.shape))
+        move_ms, move_ch, move_rb, d_b = timed_update(w.nodes + 1e-2 * w.h * rng.uniform(-1, 1, w.nodes.shape))
+        back_ms, back_ch, back_rb, d_c = timed_update(w.nodes)          # back to the original cloud and pattern
+        d_nodes = d_c
+        del d_a, d_b
+        update = {"api": "rpim_update_nodes", "full_build_pattern_ms": kernel_ms["knn"] + kernel_ms["incidence"] + kernel_ms["block_pattern"],
+                  "move_1e-9h": {"ms": keep_ms, "changed_points": keep_ch, "pattern_rebuilt": keep_rb},
+                  "move_1e-2h": {"ms": move_ms, "changed_points": move_ch, "pattern_rebuilt": move_rb},
+                  "move_back": {"ms": back_ms, "changed_points": back_ch, "pattern_rebuilt": back_rb}}
+    except Exception as ex:
+        update = {"error": repr(ex)[:200]}
+
     # ------------------------------------------------ optional: stage 3 on the assembled system
     solve = None
     if do_solve:
@@ -430,6 +456,7 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
         "assemble_penalty": {"value": world * w.Nq / (ms_asm * 1e-3), "unit": UNIT, "ms_per_step": ms_asm,
                              "gdof_entries_per_s": 9.0 * w.k * w.k * w.Nq * world / (ms_asm * 1e-3) / 1e9},
         "clocks": clocks, "e2e": e2e, "launches": int(launches), "roofline": roofline, "solve": solve,
+        "update_nodes": update,
     }
     try:
         out["fp64_probe"] = ctx.probe_fp64()
@@ -498,7 +525,7 @@ def main():
         secondary = {"config": config_block(r2["w"], world, r2), "value": r2["value"], "unit": UNIT,
                      "ms_per_step": r2["ms_per_step"], "steps": min(args.steps, 10), "warmup": 3,
                      "assemble_penalty": r2["assemble_penalty"], "gpu_launches": r2["launches"],
-                     "roofline": r2["roofline"]}
+                     "roofline": r2["roofline"], "update_nodes": r2["update_nodes"]}
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -517,6 +544,7 @@ def main():
             "assemble_penalty": r["assemble_penalty"], "clocks": r["clocks"], "e2e": r["e2e"],
             "gpu_launches": r["launches"], "roofline": roofline, "cpu_baseline": cpu_baseline,
         }
+        line["update_nodes"] = r["update_nodes"]
         if secondary is not None:
             line["large"] = secondary
         if r["solve"] is not None:

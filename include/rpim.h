@@ -79,6 +79,21 @@ int rpim_reduction_used(const rpim_ctx* ctx);
 int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const double* d_qpts,
                        int64_t Nq, int k, int index_bits, int64_t* out_nnz, int* out_index_bits);
 
+/* Moving nodes (the paper's motivation is large deformation): the
+ * same N nodes at new coordinates d_nodes (and, if d_qpts is not NULL, the same Nq points at new coordinates).
+ * The cell grid is updated incrementally (when no node left its cell only the cell-ordered coordinates are
+ * refreshed, otherwise it is rebuilt), the supports are searched again and compared with the old table on the
+ * device.  If no support changed the incidence lists, the CSR pattern and the reduction's slot maps are KEPT
+ * (row_ptr / col_idx obtained earlier stay valid); otherwise they are rebuilt.  The result is in every case
+ * identical, bit for bit, to a fresh rpim_build_pattern on the moved cloud with the same index width.
+ *   out_changed_points   host: number of points whose support changed      (may be NULL)
+ *   out_pattern_rebuilt  host: 1 if the pattern was rebuilt, 0 if kept     (may be NULL)
+ *   out_nnz              host: stored scalar entries of the current pattern (may be NULL)
+ * The new arrays replace the old ones in the lifetime rule above.  rpim_assemble must be called again
+ * before anything that uses shape functions.  Synchronises the stream. */
+int rpim_update_nodes(rpim_ctx* ctx, const double* d_nodes, const double* d_qpts, int64_t* out_changed_points,
+                      int* out_pattern_rebuilt, int64_t* out_nnz);
+
 /* Write the pattern built by rpim_build_pattern.
  *   d_row_ptr  3N+1 entries, d_col_idx  nnz entries, both int32_t or int64_t per index_bits
  *   d_support  Nq x k int32 node ids, ascending per point; may be NULL

@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = (
     "rpim_get_pattern", "rpim_assemble", "rpim_add_point_loads", "rpim_apply_penalty", "rpim_get_shape",
     "rpim_host_pattern", "rpim_host_assemble", "rpim_last_phase_ms", "rpim_phase_totals", "rpim_launch_count",
     "rpim_matvec", "rpim_solve_pcg", "rpim_recover_stress", "rpim_set_reduction", "rpim_reduction_used",
-    "rpim_probe_fp64",
+    "rpim_probe_fp64", "rpim_update_nodes",
 )
 
 
@@ -55,6 +55,7 @@ def _load():
     lib.rpim_launch_count.restype = i64
     lib.rpim_build_pattern.argtypes = [vp, vp, i64, vp, i64, C.c_int, C.c_int, C.POINTER(i64), C.POINTER(C.c_int)]
     lib.rpim_get_pattern.argtypes = [vp, vp, vp, vp]
+    lib.rpim_update_nodes.argtypes = [vp, vp, vp, C.POINTER(i64), C.POINTER(C.c_int), C.POINTER(i64)]
     lib.rpim_assemble.argtypes = [vp, vp, dbl, dbl, dbl, dbl, dbl, C.POINTER(dbl), vp, vp, C.POINTER(i64)]
     lib.rpim_add_point_loads.argtypes = [vp, vp, vp, vp, i64, vp]
     lib.rpim_apply_penalty.argtypes = [vp, vp, vp, vp, i64, dbl, C.c_int, vp, vp, C.POINTER(dbl)]
@@ -169,6 +170,15 @@ def rpim_build_pattern(ctx, d_nodes, d_qpts, k: int, index_bits: int = 0):
     return int(nnz.value), int(bits.value)
 
 
+def rpim_update_nodes(ctx, d_nodes, d_qpts=None):
+    """Returns (changed points, pattern rebuilt?, nnz)."""
+    import torch
+    ch, rb, nnz = C.c_int64(0), C.c_int(0), C.c_int64(0)
+    _check(ctx, _load().rpim_update_nodes(ctx, _dptr(d_nodes, torch.float64), _dptr(d_qpts, torch.float64),
+                                          C.byref(ch), C.byref(rb), C.byref(nnz)))
+    return int(ch.value), bool(rb.value), int(nnz.value)
+
+
 def rpim_get_pattern(ctx, d_row_ptr=None, d_col_idx=None, d_support=None):
     _check(ctx, _load().rpim_get_pattern(ctx, _dptr(d_row_ptr), _dptr(d_col_idx), _dptr(d_support)))
 
@@ -273,6 +283,9 @@ class Context:
 
     def build_pattern(self, d_nodes, d_qpts, k, index_bits=0):
         return rpim_build_pattern(self.ctx, d_nodes, d_qpts, k, index_bits)
+
+    def update_nodes(self, d_nodes, d_qpts=None):
+        return rpim_update_nodes(self.ctx, d_nodes, d_qpts)
 
     def get_pattern(self, d_row_ptr=None, d_col_idx=None, d_support=None):
         return rpim_get_pattern(self.ctx, d_row_ptr, d_col_idx, d_support)

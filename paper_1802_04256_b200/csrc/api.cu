@@ -141,6 +141,88 @@ int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const do
     return RPIM_OK;
 }
 
+namespace {
+// number of points whose support row differs between two tables
+__global__ void support_diff_kernel(const int32_t* __restrict__ a, const int32_t* __restrict__ b, int64_t Nq, int k,
+                                    unsigned long long* __restrict__ changed) {
+    const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool d = false;
+    if (q < Nq)
+        for (int j = 0; j < k; ++j) d = d || a[q * k + j] != b[q * k + j];
+    const unsigned m = __ballot_sync(0xffffffffu, d);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(changed, (unsigned long long)__popc(m));
+}
+}  // namespace
+
+int rpim_update_nodes(rpim_ctx* ctx, const double* d_nodes, const double* d_qpts, int64_t* out_changed_points,
+                      int* out_pattern_rebuilt, int64_t* out_nnz) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    if (!ctx->have_pattern) RPIM_FAIL(ctx, RPIM_ERR_STATE, "rpim_update_nodes before rpim_build_pattern");
+    if (!d_nodes) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "null pointer");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const int64_t Nq = ctx->Nq;
+    const int k = ctx->k;
+    ctx->d_nodes = d_nodes;
+    if (d_qpts) ctx->d_qpts = d_qpts;
+    ctx->have_shape = false;            // staged shape functions belong to the old coordinates
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags, 0, NUM_FLAGS * sizeof(long long), st));
+    int rc;
+    cudaEventRecord(ctx->ev[0], st);
+    bool rebuild = true;
+    int64_t moved = 0;
+    if ((rc = rpim_stage_grid_refresh(ctx, &rebuild, &moved))) { ctx->have_pattern = false; return rc; }
+    int32_t* d_new = nullptr;
+    if ((rc = ws_alloc(ctx, &d_new, Nq * k))) { ctx->have_pattern = false; return rc; }
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_KNN_CAP, 0, sizeof(long long), st));
+    if ((rc = rpim_stage_grid_knn(ctx, ctx->d_qpts, Nq, k, d_new, rebuild))) { ws_free(ctx, &d_new); ctx->have_pattern = false; return rc; }
+    unsigned long long* d_changed = (unsigned long long*)ctx->d_scratch;
+    CUDA_TRY(ctx, cudaMemsetAsync(d_changed, 0, sizeof(unsigned long long), st));
+    support_diff_kernel<<<(unsigned)((Nq + 255) / 256), 256, 0, st>>>(ctx->d_support, d_new, Nq, k, d_changed);
+    ctx->launches++;
+    unsigned long long changed = 0;
+    long long capf = 0;
+    cudaEventRecord(ctx->ev[1], st);
+    cudaError_t e = cudaMemcpyAsync(&changed, d_changed, sizeof(changed), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&capf, ctx->d_flags + FLAG_KNN_CAP, sizeof(capf), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess || capf) {
+        ws_free(ctx, &d_new);
+        ctx->have_pattern = false;
+        if (capf) RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "kNN: %lld points need more than the on-chip candidate capacity", capf);
+        RPIM_FAIL(ctx, RPIM_ERR_CUDA, "rpim_update_nodes failed: %s", cudaGetErrorString(e));
+    }
+    cudaEventElapsedTime(&ctx->phase_ms[0], ctx->ev[0], ctx->ev[1]);
+    ctx->phase_ms[1] = ctx->phase_ms[2] = 0.f;
+    if (out_changed_points) *out_changed_points = (int64_t)changed;
+    if (out_pattern_rebuilt) *out_pattern_rebuilt = changed != 0;
+    if (changed == 0) {
+        // supports unchanged: incidence lists, block pattern, slot maps, point groups and row tiles all stand
+        ws_free(ctx, &d_new);
+    } else {
+        ws_free(ctx, &ctx->d_support);
+        ctx->d_support = d_new;
+        ctx->have_pattern = ctx->have_masks = false;
+        cudaEventRecord(ctx->ev[1], st);
+        if ((rc = rpim_stage_incidence(ctx))) return rc;
+        cudaEventRecord(ctx->ev[2], st);
+        if ((rc = rpim_stage_groups(ctx))) return rc;
+        if ((rc = rpim_stage_block_pattern(ctx))) return rc;
+        if (ctx->tg_C == 0 && (rc = rpim_stage_slot_masks(ctx))) return rc;
+        if ((rc = rpim_stage_tiles(ctx))) return rc;
+        cudaEventRecord(ctx->ev[3], st);
+        CUDA_TRY(ctx, cudaStreamSynchronize(st));
+        cudaEventElapsedTime(&ctx->phase_ms[1], ctx->ev[1], ctx->ev[2]);
+        cudaEventElapsedTime(&ctx->phase_ms[2], ctx->ev[2], ctx->ev[3]);
+        const int64_t nnz = 9 * ctx->nnzb;
+        if (ctx->index_bits == 32 && nnz > 0x7fffffffLL)
+            RPIM_FAIL(ctx, RPIM_ERR_INDEX_OVERFLOW, "nnz = %lld no longer fits the 32-bit indices chosen by rpim_build_pattern", (long long)nnz);
+        ctx->have_pattern = true;
+    }
+    if (out_nnz) *out_nnz = 9 * ctx->nnzb;
+    return RPIM_OK;
+}
+
 int rpim_get_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx, int32_t* d_support) {
     if (!ctx) return RPIM_ERR_INVALID_ARG;
     if (!ctx->have_pattern) RPIM_FAIL(ctx, RPIM_ERR_STATE, "rpim_get_pattern before rpim_build_pattern");

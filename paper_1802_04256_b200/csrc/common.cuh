@@ -215,6 +215,7 @@ int ws_alloc(rpim_ctx* ctx, T** p, int64_t count) {
 // ---- stages implemented in the other translation units
 int rpim_scan_i32_to_i64(rpim_ctx* ctx, const int* d_in, int64_t* d_out, int64_t n);  // exclusive, writes n+1
 int rpim_stage_grid_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, int32_t* d_support, bool build_grid);
+int rpim_stage_grid_refresh(rpim_ctx* ctx, bool* out_rebuild, int64_t* out_moved);
 int rpim_stage_incidence(rpim_ctx* ctx);
 int rpim_stage_block_pattern(rpim_ctx* ctx);
 int rpim_stage_slot_masks(rpim_ctx* ctx);

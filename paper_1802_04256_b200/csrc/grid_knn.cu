@@ -212,6 +212,37 @@ __global__ void cell_sort_gather_kernel(const double* __restrict__ nodes, int64_
     }
 }
 
+// moving nodes (rpim_update_nodes): how many nodes left their cell of the existing grid (or the grid's box)
+__global__ void cell_moved_kernel(GridParams g, const double* __restrict__ nodes, int64_t N,
+                                  const int* __restrict__ cell_of, unsigned long long* __restrict__ moved) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool m = false;
+    if (i < N) {
+        const double p[3] = {nodes[3 * i], nodes[3 * i + 1], nodes[3 * i + 2]};
+        int c[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const int v = (int)floor((p[a] - g.lo[a]) * g.inv_cell);
+            m = m || v < 0 || v >= g.nc[a] || !(p[a] == p[a]);
+            c[a] = min(max(v, 0), g.nc[a] - 1);
+        }
+        m = m || (c[0] + g.nc[0] * (c[1] + g.nc[1] * c[2])) != cell_of[i];
+    }
+    const unsigned b = __ballot_sync(0xffffffffu, m);
+    if ((threadIdx.x & 31) == 0 && b) atomicAdd(moved, (unsigned long long)__popc(b));
+}
+
+// same cells, new coordinates: refresh the cell-ordered SoA copy
+__global__ void cell_regather_kernel(const double* __restrict__ nodes, int64_t N, const int* __restrict__ node_order,
+                                     double* __restrict__ sx, double* __restrict__ sy, double* __restrict__ sz) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int64_t id = node_order[i];
+    sx[i] = nodes[3 * id];
+    sy[i] = nodes[3 * id + 1];
+    sz[i] = nodes[3 * id + 2];
+}
+
 // ------------------------------------------------------------------ the search: one warp per query point
 // CAP = candidates held on chip per query.  The first launch uses the smallest capacity that
 // fits the expected candidate count (more resident warps); queries that need more are appended
@@ -569,6 +600,30 @@ int launch_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, const int32
     return RPIM_OK;
 }
 }  // namespace
+
+// Incremental cell-grid update for moved nodes (ctx->d_nodes already points at the new coordinates): when
+// no node left its cell only the cell-ordered coordinates are refreshed, otherwise *out_rebuild = true and
+// the caller rebuilds the grid (rpim_stage_grid_knn with build_grid).  Synchronises.
+int rpim_stage_grid_refresh(rpim_ctx* ctx, bool* out_rebuild, int64_t* out_moved) {
+    cudaStream_t st = ctx->stream;
+    const int64_t N = ctx->N;
+    unsigned long long* d_moved = (unsigned long long*)ctx->d_scratch;
+    CUDA_TRY(ctx, cudaMemsetAsync(d_moved, 0, sizeof(unsigned long long), st));
+    const unsigned nb = (unsigned)((N + 255) / 256);
+    cell_moved_kernel<<<nb, 256, 0, st>>>(ctx->grid, ctx->d_nodes, N, ctx->d_cell_of, d_moved);
+    KERNEL_CHECK(ctx);
+    unsigned long long moved = 0;
+    CUDA_TRY(ctx, cudaMemcpyAsync(&moved, d_moved, sizeof(moved), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    *out_moved = (int64_t)moved;
+    *out_rebuild = moved != 0;
+    if (moved == 0) {
+        cell_regather_kernel<<<nb, 256, 0, st>>>(ctx->d_nodes, N, ctx->d_node_order, ctx->d_sorted_xyz,
+                                                 ctx->d_sorted_xyz + N, ctx->d_sorted_xyz + 2 * N);
+        KERNEL_CHECK(ctx);
+    }
+    return RPIM_OK;
+}
 
 int rpim_stage_grid_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, int32_t* d_support, bool build_grid) {
     cudaStream_t st = ctx->stream;

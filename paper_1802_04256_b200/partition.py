@@ -1,0 +1,92 @@
+"""Sharding ONE assembly problem across ranks ("no data dependencies between
+... any two element stiffness matrices").  Host-side index logic only -- no arithmetic of the method.
+
+Row-owner partition with redundant halo work and NO data-path exchange:
+
+  * rank r owns the block rows (nodes) [N r / W, N (r+1) / W): contiguous id ranges, i.e. spatial slabs for a
+    spatially coherent numbering;
+  * it takes every quadrature point within `halo` of the bounding box of its owned nodes, and every node within
+    2 * `halo` of that box.  If `halo` bounds the support radius (distance from a point to its k-th nearest node)
+    of every point, then (a) every point whose support touches an owned row is taken, and (b) the k nearest
+    nodes of a taken point among the taken nodes are its k nearest nodes among ALL nodes.  The owned rows of the
+    rank's sub-problem are then complete and -- supports ascending, points in ascending order -- bit-identical to
+    the same rows of the undivided problem; the rows of halo nodes are partial and are discarded;
+  * the bound is VERIFIED after the support search (`support_radius_ok`): on the sub-cloud the k-th neighbour
+    distance can only be larger than the true one, so `max <= halo` on every rank proves the premise for every
+    point (each point is taken by at least one rank);
+  * the only collective of the path is allreduce(max) of one double: alpha = penalty * max_i K_ii.  A halo row's
+    partial diagonal never exceeds its complete value (every contribution to a diagonal entry is >= 0), which
+    the owning rank holds, so max over ranks of the local maxima is the global maximum.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+
+import numpy as np
+
+
+@dataclass
+class Shard:
+    rank: int
+    world: int
+    row_lo: int                # owned global rows [row_lo, row_hi)
+    row_hi: int
+    node_ids: np.ndarray       # global ids of the taken nodes, ascending (local id = position)
+    point_ids: np.ndarray      # global ids of the taken points, ascending
+    own_lo: int                # owned rows in LOCAL numbering [own_lo, own_hi) (contiguous: ids are ascending)
+    own_hi: int
+    halo: float
+
+
+def owned_rows(N: int, rank: int, world: int):
+    return (N * rank) // world, (N * (rank + 1)) // world
+
+
+def halo_estimate(nodes: np.ndarray, k: int, safety: float = 2.2) -> float:
+    """A support-radius bound from the mean node density: radius of the ball holding k nodes, times `safety`
+    (a point in a corner of the domain sees one octant: factor 2; the rest covers jitter).  It is an estimate;
+    `support_radius_ok` is what validates it."""
+    ext = nodes.max(axis=0) - nodes.min(axis=0)
+    vol = float(np.prod(np.maximum(ext, 1e-9 * ext.max())))
+    h = (vol / nodes.shape[0]) ** (1.0 / 3.0)
+    return safety * (3.0 * k / (4.0 * np.pi)) ** (1.0 / 3.0) * h
+
+
+def make_shard(nodes: np.ndarray, qpts: np.ndarray, k: int, rank: int, world: int, halo: float | None = None) -> Shard:
+    N = nodes.shape[0]
+    lo, hi = owned_rows(N, rank, world)
+    if halo is None:
+        halo = halo_estimate(nodes, k)
+    own = nodes[lo:hi]
+    blo, bhi = own.min(axis=0), own.max(axis=0)
+    take_p = np.all((qpts >= blo - halo) & (qpts <= bhi + halo), axis=1)
+    take_n = np.all((nodes >= blo - 2.0 * halo) & (nodes <= bhi + 2.0 * halo), axis=1)
+    take_n[lo:hi] = True
+    node_ids = np.nonzero(take_n)[0].astype(np.int64)
+    point_ids = np.nonzero(take_p)[0].astype(np.int64)
+    own_lo = int(np.searchsorted(node_ids, lo))
+    own_hi = int(np.searchsorted(node_ids, hi))
+    assert own_hi - own_lo == hi - lo
+    return Shard(rank, world, lo, hi, node_ids, point_ids, own_lo, own_hi, float(halo))
+
+
+def support_radius_ok(sub_nodes: np.ndarray, sub_pts: np.ndarray, support_local: np.ndarray, halo: float) -> bool:
+    """max over the taken points of the distance to the farthest node of the support found on the sub-cloud."""
+    d = sub_nodes[support_local] - sub_pts[:, None, :]
+    return bool(np.sqrt((d * d).sum(axis=2)).max() <= halo)
+
+
+def local_bc(shard: Shard, bc_nodes: np.ndarray, bc_mask: np.ndarray, bc_ubar: np.ndarray):
+    """The boundary conditions of the owned rows, in local numbering."""
+    sel = (bc_nodes >= shard.row_lo) & (bc_nodes < shard.row_hi)
+    loc = np.searchsorted(shard.node_ids, bc_nodes[sel]).astype(np.int64)
+    return np.ascontiguousarray(loc), np.ascontiguousarray(bc_mask[sel]), np.ascontiguousarray(bc_ubar[sel])
+
+
+def owned_csr_rows(shard: Shard, row_ptr: np.ndarray, col_idx: np.ndarray, vals: np.ndarray, f: np.ndarray):
+    """The owned scalar rows of a rank's local CSR, columns mapped back to GLOBAL DOF ids."""
+    a, b = int(row_ptr[3 * shard.own_lo]), int(row_ptr[3 * shard.own_hi])
+    ci = col_idx[a:b].astype(np.int64)
+    gcol = 3 * shard.node_ids[ci // 3] + ci % 3
+    return (row_ptr[3 * shard.own_lo:3 * shard.own_hi + 1].astype(np.int64) - a, gcol, vals[a:b],
+            f[3 * shard.own_lo:3 * shard.own_hi])

@@ -240,7 +240,7 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
     hbm_gbs, sm_max_mhz, peak_src = peaks
     w = rank_workload(name, rank, world)
     ctx = rp.Context(local_rank)
-    ctx.set_reduction({"auto": 0, "rows": 1, "tiles": 2}[args.reduction])
+    ctx.set_reduction({"auto": 0, "rows": 1, "panels": 2}[args.reduction])
     d_nodes = torch.from_numpy(w.nodes).to(dev)
     d_qpts = torch.from_numpy(w.qpts).to(dev)
     d_qw = torch.from_numpy(w.qw).to(dev)
@@ -314,8 +314,8 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
     hbm_min = nnz * 8 + w.Nq * w.k * 4 + w.Nq * 32 + w.N * 24 + 3 * w.N * 8
     staged_reread = 37 * w.Nq * w.k            # this implementation's staged gradients + incidence, read once
     traffic = read_traffic(w.name)
-    used = {1: "rows", 2: "tiles"}.get(ctx.reduction_used(), "?")
-    reduce_name = "reduce_rows_kernel" if used == "rows" else "reduce_tiles_kernel"
+    used = {1: "rows", 2: "panels"}.get(ctx.reduction_used(), "?")
+    reduce_name = "reduce_rows_kernel" if used == "rows" else "reduce_panels_kernel"
     t_red_alu = fl_reduce * w.Nq / (peak_tflops * 1e12) * 1e3          # ms at the FP64 peak
     t_red_hbm = hbm_min / (hbm_gbs * 1e9) * 1e3                        # ms at the HBM peak
     if reduce_ms >= shape_ms:
@@ -484,8 +484,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="stress", choices=workloads.CONFIG_NAMES)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--reduction", default="auto", choices=["auto", "rows", "tiles"],
-                    help="reduction kernel (rpim_set_reduction): automatic choice, row-owner, or tiled")
+    ap.add_argument("--reduction", default="auto", choices=["auto", "rows", "panels"],
+                    help="reduction kernel (rpim_set_reduction): automatic choice, row-owner, or panel")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="do not also time `large` when the headline is `stress`")

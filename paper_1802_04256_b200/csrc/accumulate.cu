@@ -12,14 +12,14 @@
 // Lane l of chunk c owns column slot 32 c + l of the row.  One resident wave of CTAs; every group
 // of warps draws its next row from a ticket counter, so the rows in flight form one contiguous
 // stripe.  For a batch of incident points one thread bulk-copies (cp.async.bulk + mbarrier) the
-// points' staged [k][phi gx gy gz] rows into a double-buffered staging area, and every lane learns
+// points' staged [phi gx gy gz][k] rows into a double-buffered staging area, and every lane learns
 // whether the point hits its slot and at which support position:
 //   MASKED   from the slot masks precomputed with the pattern (pattern.cu): bit test, then
 //            position = set bits before the chunk + popc(bits below the lane);
 //   !MASKED  (masks over budget, e.g. config 5) from an open-addressing table column -> slot built
 //            per row in shared memory and a byte table pos[point][slot] filled with one probe per
 //            support node.
-// A hit lane gathers that node's gradient (one 32-byte sector) from the staging area and does nine
+// A hit lane gathers that node's gradient (three doubles) from the staging area and does nine
 // fused multiply-adds.
 // accumulate_generic_kernel: fallback for longer rows, accumulators in shared memory.
 #include "bulk_copy.cuh"
@@ -135,10 +135,8 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                 const int i = inc_j[p];
                 const double w = qw[q];
                 const double* base = stage + (int64_t)q * k * 4;
-                const double2 v01 = *reinterpret_cast<const double2*>(base + 4 * i);
-                const double2 v23 = *reinterpret_cast<const double2*>(base + 4 * i + 2);
-                fsum += w * v01.x;
-                sm.a[tg][0] = w * v01.y; sm.a[tg][1] = w * v23.x; sm.a[tg][2] = w * v23.y;
+                fsum += w * base[i];   // staged layout [q][phi, d/dx, d/dy, d/dz][k]
+                sm.a[tg][0] = w * base[k + i]; sm.a[tg][1] = w * base[2 * k + i]; sm.a[tg][2] = w * base[3 * k + i];
                 sm.qbase[tg] = base;
                 if constexpr (MASKED) {
                     const unsigned* mw = mrow + (p - pa) * mstep;
@@ -226,12 +224,10 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                             const unsigned word = (unsigned)mpv[cc];
                             if (word & lbit) {
                                 const unsigned j = (unsigned)(mpv[cc] >> 32) + __popc(word & lt);
-                                const double2 g01 = *reinterpret_cast<const double2*>(base + 4 * j);
-                                const double2 gyz = *reinterpret_cast<const double2*>(base + 4 * j + 2);
-                                const double gx = g01.y;
-                                acc[cc][0] = fma(ax, gx, acc[cc][0]); acc[cc][1] = fma(ax, gyz.x, acc[cc][1]); acc[cc][2] = fma(ax, gyz.y, acc[cc][2]);
-                                acc[cc][3] = fma(ay, gx, acc[cc][3]); acc[cc][4] = fma(ay, gyz.x, acc[cc][4]); acc[cc][5] = fma(ay, gyz.y, acc[cc][5]);
-                                acc[cc][6] = fma(az, gx, acc[cc][6]); acc[cc][7] = fma(az, gyz.x, acc[cc][7]); acc[cc][8] = fma(az, gyz.y, acc[cc][8]);
+                                const double gx = base[k + j], gy = base[2 * k + j], gz = base[3 * k + j];
+                                acc[cc][0] = fma(ax, gx, acc[cc][0]); acc[cc][1] = fma(ax, gy, acc[cc][1]); acc[cc][2] = fma(ax, gz, acc[cc][2]);
+                                acc[cc][3] = fma(ay, gx, acc[cc][3]); acc[cc][4] = fma(ay, gy, acc[cc][4]); acc[cc][5] = fma(ay, gz, acc[cc][5]);
+                                acc[cc][6] = fma(az, gx, acc[cc][6]); acc[cc][7] = fma(az, gy, acc[cc][7]); acc[cc][8] = fma(az, gz, acc[cc][8]);
                             }
                         }
                     } else {
@@ -243,12 +239,10 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                             if (!((cm >> c) & 1u)) continue;
                             const unsigned j = prow[32 * c];
                             if (j != 0xFFu) {
-                                const double2 g01 = *reinterpret_cast<const double2*>(base + 4 * j);
-                                const double2 gyz = *reinterpret_cast<const double2*>(base + 4 * j + 2);
-                                const double gx = g01.y;
-                                acc[cc][0] = fma(ax, gx, acc[cc][0]); acc[cc][1] = fma(ax, gyz.x, acc[cc][1]); acc[cc][2] = fma(ax, gyz.y, acc[cc][2]);
-                                acc[cc][3] = fma(ay, gx, acc[cc][3]); acc[cc][4] = fma(ay, gyz.x, acc[cc][4]); acc[cc][5] = fma(ay, gyz.y, acc[cc][5]);
-                                acc[cc][6] = fma(az, gx, acc[cc][6]); acc[cc][7] = fma(az, gyz.x, acc[cc][7]); acc[cc][8] = fma(az, gyz.y, acc[cc][8]);
+                                const double gx = base[k + j], gy = base[2 * k + j], gz = base[3 * k + j];
+                                acc[cc][0] = fma(ax, gx, acc[cc][0]); acc[cc][1] = fma(ax, gy, acc[cc][1]); acc[cc][2] = fma(ax, gz, acc[cc][2]);
+                                acc[cc][3] = fma(ay, gx, acc[cc][3]); acc[cc][4] = fma(ay, gy, acc[cc][4]); acc[cc][5] = fma(ay, gz, acc[cc][5]);
+                                acc[cc][6] = fma(az, gx, acc[cc][6]); acc[cc][7] = fma(az, gy, acc[cc][7]); acc[cc][8] = fma(az, gz, acc[cc][8]);
                             }
                         }
                     }
@@ -314,12 +308,12 @@ accumulate_generic_kernel(int64_t N, int k, int Lcap, const int64_t* __restrict_
             const int i = inc_j[p];
             const double w = qw[q];
             const double* st = stage + q * 4 * (int64_t)k;
-            const double wgx = w * st[4 * i + 1], wgy = w * st[4 * i + 2], wgz = w * st[4 * i + 3];
-            fI += w * st[4 * i];
+            const double wgx = w * st[k + i], wgy = w * st[2 * k + i], wgz = w * st[3 * k + i];
+            fI += w * st[i];
             const int32_t* sp = support + q * k;
             for (int j = lane; j < k; j += 32) {
                 const int J = sp[j];
-                const double gx = st[4 * j + 1], gy = st[4 * j + 2], gz = st[4 * j + 3];
+                const double gx = st[k + j], gy = st[2 * k + j], gz = st[3 * k + j];
                 int lo = 0, hi = L - 1;   // J is always present in the row
                 while (lo < hi) {
                     const int mid = (lo + hi) >> 1;
@@ -362,7 +356,7 @@ __global__ void point_loads_kernel(const int32_t* __restrict__ support, const do
         const double wp = w[p], tx = t[3 * p], ty = t[3 * p + 1], tz = t[3 * p + 2];
         for (int j = lane; j < k; j += 32) {
             const int64_t J = support[p * k + j];
-            const double wphi = wp * st[4 * j];
+            const double wphi = wp * st[j];
             f[3 * J] += wphi * tx;
             f[3 * J + 1] += wphi * ty;
             f[3 * J + 2] += wphi * tz;

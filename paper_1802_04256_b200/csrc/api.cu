@@ -32,7 +32,7 @@ void free_all(rpim_ctx* c) {
     ws_free(c, &c->d_stage); ws_free(c, &c->d_singular); ws_free(c, &c->d_scratch);
     ws_free(c, &c->d_mask_ptr); ws_free(c, &c->d_masks);
     c->have_masks = false;
-    ws_free(c, &c->d_gu_nodes); ws_free(c, &c->d_gpos); ws_free(c, &c->d_gu_mask);
+    ws_free(c, &c->d_gpos); ws_free(c, &c->d_gmeta);
     ws_free(c, &c->d_tile_ptr); ws_free(c, &c->d_tdesc);
     c->have_tiles = false; c->tg_C = 0;
     ws_free(c, &c->h2d_nodes); ws_free(c, &c->h2d_qpts);
@@ -247,7 +247,8 @@ int rpim_assemble(rpim_ctx* ctx, const double* d_qw, double E, double nu, double
     fill_shape_params(alpha_c, d_c, q, ctx->sp);
     ctx->have_sp = true;
     int rc;
-    if (!ctx->d_stage && (rc = ws_alloc(ctx, &ctx->d_stage, ctx->Nq * 4 * (int64_t)ctx->k))) return rc;
+    // (whole groups of RPIM_GROUP_POINTS points: the panel reduction copies a group's staged rows in one piece)
+    if (!ctx->d_stage && (rc = ws_alloc(ctx, &ctx->d_stage, ((ctx->Nq + RPIM_GROUP_POINTS - 1) / RPIM_GROUP_POINTS) * RPIM_GROUP_POINTS * 4 * (int64_t)ctx->k))) return rc;
     if (!ctx->d_singular && (rc = ws_alloc(ctx, &ctx->d_singular, ctx->Nq))) return rc;
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_SINGULAR, 0, sizeof(long long), st));
     // a triple of pooled events per call so that a caller can sum kernel times over many calls
@@ -268,7 +269,7 @@ int rpim_assemble(rpim_ctx* ctx, const double* d_qw, double E, double nu, double
     if (pe[1]) cudaEventRecord(pe[1], st);
     const double lambda = E * nu / ((1.0 + nu) * (1.0 - 2.0 * nu));
     const double mu = E / (2.0 * (1.0 + nu));
-    rc = ctx->have_tiles ? rpim_stage_accumulate_tiles(ctx, d_qw, lambda, mu, body, d_vals, d_f)
+    rc = ctx->have_tiles ? rpim_stage_accumulate_panels(ctx, d_qw, lambda, mu, body, d_vals, d_f)
                          : rpim_stage_accumulate(ctx, d_qw, lambda, mu, body, d_vals, d_f);
     if (rc) return rc;
     cudaEventRecord(ctx->ev[6], st);
@@ -341,7 +342,7 @@ __global__ void split_stage_kernel(const double* __restrict__ stage, int64_t M, 
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
         const int64_t q = e / (4 * k);
         const int r = (int)(e % (4 * k));
-        const int j = r >> 2, c = r & 3;          // staged layout: [q][j][phi, d/dx, d/dy, d/dz]
+        const int c = r / k, j = r - c * k;       // staged layout: [q][phi, d/dx, d/dy, d/dz][j]
         if (c == 0) { if (phi) phi[q * k + j] = stage[e]; }
         else if (dphi) dphi[(q * 3 + (c - 1)) * (int64_t)k + j] = stage[e];
     }

@@ -11,8 +11,8 @@
 #include "../../include/rpim.h"
 
 #define RPIM_WARP 32
-#define RPIM_GROUP_POINTS 8      // quadrature points per group of the tiled reduction (groups.cu)
-#define RPIM_TILE_DESC_CAP 256   // tile descriptors resident in shared memory at a time (reduce_tiles.cu)
+#define RPIM_GROUP_POINTS 8      // quadrature points per group of the panel reduction (groups.cu)
+#define RPIM_PANEL_MAX_UNION_RATIO 100.0   // automatic choice: panel kernel when mean |U_g| <= ratio * k (provisional: always)
 
 // device-side error / counter slots (ctx->d_flags, int64 each)
 enum { FLAG_KNN_CAP = 0, FLAG_PAT_CAP = 1, FLAG_BC_BAD = 2, FLAG_SINGULAR = 3, FLAG_INC_CAP = 4, FLAG_OVF_ROWS = 5, FLAG_OVF_Q = 6, FLAG_INC_LONG = 7, FLAG_ROW_TICKET = 8, FLAG_INC_LONG2 = 9, NUM_FLAGS = 16 };
@@ -87,19 +87,23 @@ struct rpim_ctx {
     int64_t* d_mask_ptr = nullptr;   // N + 1 (word offset of row I)
     unsigned* d_masks = nullptr;
 
-    // tiled reduction (groups.cu, reduce_tiles.cu): point groups, their unions, row tiles
-    int reduce_mode = 0;             // 0 = automatic, 1 = row-owner kernel, 2 = tiled kernel whenever it fits
+    // panel reduction (groups.cu, reduce_panels.cu): point groups, their unions, row tiles
+    int reduce_mode = 0;             // 0 = automatic, 1 = row-owner kernel, 2 = panel kernel whenever it fits, 3 = long-row kernel
     bool have_tiles = false;
-    int tg_C = 0;                    // 32-lane chunks per group union (0: tiled path not applicable)
-    int tg_T = 0;                    // block rows per tile
+    int tg_C = 0;                    // 32-lane chunks per group union (0: panel path not applicable)
+    int tg_T = 0;                    // block rows per tile (even)
+    int tg_nstage = 0;               // stages of the group ring
+    double tg_mean_union = 0.0;      // mean |U_g| of the last statistics pass
     int64_t ntiles = 0;
-    int32_t* d_gu_nodes = nullptr;   // G x 32 C: sorted union of the group's supports, padded with -1
     uint8_t* d_gpos = nullptr;       // Nq x k: position of (point, support node) in its group's union
-    uint8_t* d_gu_mask = nullptr;    // G x 32 C: bit p = the union entry is a support node of the group's point p
+    // G group records of rpim_panel_meta_bytes(C): [32 C x 8 bytes: support position of union entry u in the
+    // group's point p, 0xFF = absent][32 C ints: sorted union of the group's supports, padded with -1]
+    // [8 doubles: quadrature weights, written by rpim_assemble]
+    unsigned char* d_gmeta = nullptr;
     int64_t* d_tile_ptr = nullptr;   // ntiles + 1
-    unsigned* d_tdesc = nullptr;     // tile descriptors, 1 + ceil(T/2) words each
+    unsigned* d_tdesc = nullptr;     // tile descriptors, 1 + T/2 words each
 
-    // staged shape functions: Nq x k x 4  (phi, dphi/dx, dphi/dy, dphi/dz per support node: one 32-byte sector)
+    // staged shape functions: Nq x 4 x k  (per point four rows of k: phi, dphi/dx, dphi/dy, dphi/dz in support order)
     double* d_stage = nullptr;
     uint8_t* d_singular = nullptr;   // Nq
     ShapeParams sp{};
@@ -221,7 +225,7 @@ int rpim_stage_block_pattern(rpim_ctx* ctx);
 int rpim_stage_slot_masks(rpim_ctx* ctx);
 int rpim_stage_groups(rpim_ctx* ctx);   // after the support search: decides ctx->tg_C
 int rpim_stage_tiles(rpim_ctx* ctx);    // after incidence + block pattern: decides ctx->have_tiles
-int rpim_stage_accumulate_tiles(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
+int rpim_stage_accumulate_panels(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
                                 double* d_vals, double* d_f);
 int rpim_stage_emit_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx);
 int rpim_stage_shape(rpim_ctx* ctx, const double* d_pts, const int32_t* d_support, int64_t M, double* d_stage,
@@ -235,20 +239,34 @@ int rpim_stage_point_loads(rpim_ctx* ctx, const int32_t* d_support, const double
 int rpim_stage_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* d_bc_mask, const double* d_u_bar,
                        int64_t m, double alpha, int relative, double* d_vals, double* d_f, double* out_alpha);
 
-// Dynamic shared memory of reduce_tiles_kernel<C, T> for rows of up to Lcap block columns:
-// accumulators T x Lcap x 9, column tables T x HSZ (HSZ = power of two >= 2 Lcap), two group panels
-// 8 x 3 x 32 C, per-warp w * grad phi_I, weights, bookkeeping, union ids and masks (x 2), tile descriptors.
-inline int rpim_tiles_hlog(int Lcap) {
-    int h = 6;
-    while ((1 << h) < 2 * Lcap) ++h;
-    return h;
-}
-inline size_t rpim_tiles_smem_bytes(int C, int T, int Lcap) {
-    const size_t hsz = (size_t)1 << rpim_tiles_hlog(Lcap);
-    const size_t dw = 1 + (T + 1) / 2;
-    return (size_t)T * Lcap * 9 * 8 + (size_t)T * hsz * 8 + (size_t)2 * RPIM_GROUP_POINTS * 3 * 32 * C * 8 +
-           (size_t)T * C * RPIM_GROUP_POINTS * 4 * 8 + 2 * RPIM_GROUP_POINTS * 8 + 2 * T * RPIM_GROUP_POINTS * 8 + (2 + 8) * 8 +
-           (8 + 2 * 32 * C + 2 * 8 * C + (RPIM_TILE_DESC_CAP + 4) * dw + 3) * 4;
+// Dynamic shared memory of reduce_panels_kernel<C, T / 2> (reduce_panels.cu) for rows of up to Lcap block
+// columns: byte offsets of its areas, identical on host and device.
+struct PanelSmem {
+    int LS;            // accumulator / column-list stride in block columns (Lcap rounded up to even)
+    int hlog;          // log2 of the per-row table size (power of two >= 2 Lcap)
+    unsigned stage_bytes;
+    unsigned off_acc, off_bcol, off_hash, off_aw, off_stage, off_zero, off_bar, off_rowo, total;
+};
+// bytes of a group's record: [jinv: 32 C x 8][union node ids: 32 C ints][weights: 8 doubles]
+inline unsigned rpim_panel_meta_bytes(int C) { return 32u * C * 12u + RPIM_GROUP_POINTS * 8u; }
+inline PanelSmem rpim_panel_smem(int C, int T, int k, int Lcap, int nstage) {
+    PanelSmem L;
+    L.LS = (Lcap + 1) & ~1;
+    L.hlog = 6;
+    while ((1 << L.hlog) < 2 * Lcap) ++L.hlog;
+    L.stage_bytes = (unsigned)(RPIM_GROUP_POINTS * 4 * k * 8) + rpim_panel_meta_bytes(C) + 32u;
+    auto up16 = [](unsigned v) { return (v + 15u) & ~15u; };
+    unsigned o = 0;
+    L.off_acc = o; o = up16(o + (unsigned)T * 9u * L.LS * 8u);
+    L.off_bcol = o; o = up16(o + (unsigned)T * L.LS * 4u);
+    L.off_hash = o; o = up16(o + (unsigned)T * (2u << L.hlog));
+    L.off_aw = o; o = up16(o + (unsigned)(T / 2) * C * RPIM_GROUP_POINTS * 6u * 8u);
+    L.off_stage = o; o = up16(o + (unsigned)nstage * L.stage_bytes);
+    L.off_zero = o; o = up16(o + (unsigned)(2 * k + 2) * 8u);
+    L.off_bar = o; o = up16(o + 2u * nstage * 8u);
+    L.off_rowo = o; o = up16(o + (unsigned)T * 12u);
+    L.total = o;
+    return L;
 }
 
 // ---- small device helpers

@@ -1,41 +1,45 @@
-// Point groups and row tiles: the integer preprocessing of the tiled reduction (reduce_tiles.cu,
+// Point groups and row tiles: the integer preprocessing of the panel reduction (reduce_panels.cu,
 // step a6).  Built by rpim_build_pattern next to the CSR pattern; depends on the supports only.
 //
 //   group g   = the GB = 8 consecutive quadrature points 8g .. 8g+7 (the Gauss points of one background
 //               cell when a cell carries 8 of them: their supports nearly coincide)
-//   U_g       = sorted union of the supports of the group's points (gu_nodes, stride 32 C, padded with -1)
+//   U_g       = sorted union of the supports of the group's points (32 C entries, padded with -1)
 //   gpos      = position of every (point, support node) in U_g                       (one byte each)
-//   gu_mask   = per union entry one byte: bit p set iff U_g[u] is a support node of the group's point p
-//   tile t    = the T consecutive block rows T t .. T t + T-1
+//   gjinv     = per union entry eight bytes: byte p = support position of U_g[u] in the group's point p,
+//               0xFF when that point does not hold the node
+//   tile t    = the T consecutive block rows T t .. T t + T-1 (T even, <= 8)
 //   tdesc     = per tile the ascending list of the groups incident to any of its rows; per (tile, group)
-//               1 + ceil(T/2) words: the group id, then per row 16 bits: position u_r of the row's node in
+//               1 + T/2 words: the group id, then per row 16 bits: position u_r of the row's node in
 //               U_g (low byte) and the mask of the group's points whose support contains that node (high
 //               byte; 0 = the row is not incident to the group)
 //
-// The tiled path runs on request (rpim_set_reduction(ctx, 2)) when the groups fit (max |U_g| <= 192 and
-// two rows' accumulators fit in shared memory); otherwise the row-owner kernel of accumulate.cu runs.
+// The panel path applies when the groups fit (max |U_g| <= 128) and two rows' accumulators fit in shared
+// memory; otherwise the row-owner kernel of accumulate.cu runs.
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace {
 
 constexpr int GB = RPIM_GROUP_POINTS;
 constexpr int GSORT = 1024;     // >= GB * RPIM_MAX_K = 992 ids sorted per group
-constexpr int GU_MAX = 192;     // longest union the reduction handles (6 chunks of 32 lanes)
+constexpr int GU_MAX = 128;     // longest union the reduction handles (4 chunks of 32 lanes)
 constexpr int GW = 4;           // warps per block
+constexpr int TMAX = 8;         // most block rows per tile
 
 // One warp per group.  FILL = false: only |U_g| statistics (max, sum).  FILL = true: U_g, gpos, gu_mask.
 template <bool FILL>
 __global__ void __launch_bounds__(GW * 32)
 group_union_kernel(int64_t Nq, int k, int C, const int32_t* __restrict__ support, int* __restrict__ max_len,
-                   unsigned long long* __restrict__ sum_len, int32_t* __restrict__ gu_nodes,
-                   uint8_t* __restrict__ gpos, uint8_t* __restrict__ gu_mask) {
+                   unsigned long long* __restrict__ sum_len,
+                   uint8_t* __restrict__ gpos, unsigned char* __restrict__ gmeta) {
     __shared__ int buf_s[GW][GSORT];
     __shared__ int ul_s[GW][GU_MAX];
-    __shared__ unsigned um_s[GW][GU_MAX];
+    __shared__ __align__(16) uint8_t ji_s[GW][GU_MAX * GB];
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int* buf = buf_s[wid];
     int* ul = ul_s[wid];
-    unsigned* um = um_s[wid];
+    uint8_t* ji = ji_s[wid];
     const int64_t G = (Nq + GB - 1) / GB;
     const int gcap = 32 * C;
     for (int64_t g = (int64_t)blockIdx.x * GW + wid; g < G; g += (int64_t)gridDim.x * GW) {
@@ -65,8 +69,10 @@ group_union_kernel(int64_t Nq, int k, int C, const int32_t* __restrict__ support
             }
         } else {
             // total <= gcap: the host chose C from the statistics pass
-            for (int u = lane; u < gcap; u += 32) gu_nodes[g * gcap + u] = (u < total) ? ul[u] : -1;
-            for (int u = lane; u < GU_MAX; u += 32) um[u] = 0u;
+            unsigned char* rec = gmeta + g * (int64_t)(gcap * 12 + GB * 8);   // rpim_panel_meta_bytes(C)
+            int* gu_nodes = reinterpret_cast<int*>(rec + gcap * 8);
+            for (int u = lane; u < gcap; u += 32) gu_nodes[u] = (u < total) ? ul[u] : -1;
+            for (int u = lane; u < GU_MAX * GB / 4; u += 32) reinterpret_cast<unsigned*>(ji)[u] = 0xFFFFFFFFu;
             __syncwarp();
             for (int i = lane; i < n; i += 32) {
                 const int node = src[i];
@@ -76,10 +82,12 @@ group_union_kernel(int64_t Nq, int k, int C, const int32_t* __restrict__ support
                     if (ul[mid] < node) lo = mid + 1; else hi = mid;
                 }
                 gpos[q0 * k + i] = (uint8_t)lo;
-                atomicOr(&um[lo], 1u << (i / k));
+                const int p = i / k;
+                ji[lo * GB + p] = (uint8_t)(i - p * k);
             }
             __syncwarp();
-            for (int u = lane; u < gcap; u += 32) gu_mask[g * gcap + u] = (uint8_t)(u < total ? um[u] : 0u);
+            uint4* dst = reinterpret_cast<uint4*>(rec);
+            for (int e = lane; e < gcap * GB / 16; e += 32) dst[e] = reinterpret_cast<const uint4*>(ji)[e];
         }
     }
 }
@@ -93,11 +101,11 @@ tile_desc_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restr
                  unsigned* __restrict__ tdesc) {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= ntiles) return;
-    const int DW = 1 + (T + 1) / 2;
-    int64_t c[4], e[4];
-    int gq[4];   // group of the next entry of row r (INT_MAX: list exhausted)
+    const int DW = 1 + T / 2;
+    int64_t c[TMAX], e[TMAX];
+    int gq[TMAX];   // group of the next entry of row r (INT_MAX: list exhausted)
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
+    for (int r = 0; r < TMAX; ++r) {
         const int64_t I = t * T + r;
         c[r] = e[r] = 0;
         if (r < T && I < N) { c[r] = inc_ptr[I]; e[r] = inc_ptr[I + 1]; }
@@ -106,11 +114,15 @@ tile_desc_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restr
     int n = 0;
     unsigned* dst = FILL ? tdesc + tile_ptr[t] * DW : nullptr;
     while (true) {
-        const int g = min(min(gq[0], gq[1]), min(gq[2], gq[3]));
-        if (g == 0x7FFFFFFF) break;
-        unsigned half[4] = {0u, 0u, 0u, 0u};
+        int g = gq[0];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
+        for (int r = 1; r < TMAX; ++r) g = min(g, gq[r]);
+        if (g == 0x7FFFFFFF) break;
+        unsigned half[TMAX];
+#pragma unroll
+        for (int r = 0; r < TMAX; ++r) half[r] = 0u;
+#pragma unroll
+        for (int r = 0; r < TMAX; ++r) {
             if (gq[r] != g) continue;
             unsigned m = 0u, u = 0u;
             while (true) {
@@ -126,8 +138,9 @@ tile_desc_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restr
         }
         if (FILL) {
             dst[(int64_t)n * DW] = (unsigned)g;
-            dst[(int64_t)n * DW + 1] = half[0] | (half[1] << 16);
-            if (DW > 2) dst[(int64_t)n * DW + 2] = half[2] | (half[3] << 16);
+#pragma unroll
+            for (int w = 0; w < TMAX / 2; ++w)
+                if (1 + w < DW) dst[(int64_t)n * DW + 1 + w] = half[2 * w] | (half[2 * w + 1] << 16);
         }
         ++n;
     }
@@ -136,57 +149,61 @@ tile_desc_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restr
 
 }  // namespace
 
-// After the support search: unions of the point groups; decides whether the tiled reduction applies
-// (ctx->tg_C > 0) and, if so, leaves U_g, gpos and gu_mask in the workspace.
+// After the support search: unions of the point groups; decides whether the panel reduction applies
+// (ctx->tg_C > 0) and, if so, leaves gpos and the group records in the workspace.
 int rpim_stage_groups(rpim_ctx* ctx) {
     cudaStream_t st = ctx->stream;
     ctx->tg_C = 0;
     ctx->have_tiles = false;
-    // Measured on B200 (round 2): the tiled kernel ties with the row-owner kernel at
-    // `stress` (0.93 s vs 0.92 s) and loses at `slope` (15.6 ms vs 10.5 ms), so the automatic choice is the
-    // row-owner kernel; the tiled one runs on request (rpim_set_reduction(ctx, 2)).
-    if (ctx->reduce_mode != 2) return RPIM_OK;
+    if (ctx->reduce_mode == 1 || ctx->reduce_mode == 3) return RPIM_OK;
     const int64_t Nq = ctx->Nq, G = (Nq + GB - 1) / GB;
     const int k = ctx->k;
     int* d_max = (int*)ctx->d_scratch;
     unsigned long long* d_sum = (unsigned long long*)(ctx->d_scratch + 1);
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_scratch, 0, 2 * sizeof(double), st));
     const unsigned nb = (unsigned)std::min<int64_t>((G + GW - 1) / GW, 148 * 16);
-    group_union_kernel<false><<<nb, GW * 32, 0, st>>>(Nq, k, 0, ctx->d_support, d_max, d_sum, nullptr, nullptr, nullptr);
+    group_union_kernel<false><<<nb, GW * 32, 0, st>>>(Nq, k, 0, ctx->d_support, d_max, d_sum, nullptr, nullptr);
     KERNEL_CHECK(ctx);
     int h_max = 0;
     unsigned long long h_sum = 0;
     CUDA_TRY(ctx, cudaMemcpyAsync(&h_max, d_max, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaMemcpyAsync(&h_sum, d_sum, sizeof(h_sum), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaStreamSynchronize(st));
-    const double mean = (double)h_sum / (double)G;
-    (void)mean;   // reported by nothing yet; the density criterion (mean |U_g| <= 1.75 k) is moot while tiles are opt-in
+    ctx->tg_mean_union = (double)h_sum / (double)G;
     if (h_max > GU_MAX) return RPIM_OK;
+    // automatic choice: the panel kernel pays when a group's points share most of their supports
+    if (ctx->reduce_mode == 0 && ctx->tg_mean_union > RPIM_PANEL_MAX_UNION_RATIO * k) return RPIM_OK;
     int C = (h_max + 31) / 32;
-    if (C == 5) C = 6;
     if (C < 2) C = 2;
     int rc;
-    if ((rc = ws_alloc(ctx, &ctx->d_gu_nodes, G * 32 * C))) return rc;
     if ((rc = ws_alloc(ctx, &ctx->d_gpos, Nq * k))) return rc;
-    if ((rc = ws_alloc(ctx, &ctx->d_gu_mask, G * 32 * C))) return rc;
-    group_union_kernel<true><<<nb, GW * 32, 0, st>>>(Nq, k, C, ctx->d_support, nullptr, nullptr, ctx->d_gu_nodes,
-                                                      ctx->d_gpos, ctx->d_gu_mask);
+    if ((rc = ws_alloc(ctx, &ctx->d_gmeta, G * (int64_t)rpim_panel_meta_bytes(C)))) return rc;
+    group_union_kernel<true><<<nb, GW * 32, 0, st>>>(Nq, k, C, ctx->d_support, nullptr, nullptr, ctx->d_gpos, ctx->d_gmeta);
     KERNEL_CHECK(ctx);
     ctx->tg_C = C;
     return RPIM_OK;
 }
 
-// After incidence + block pattern: rows per tile from the shared-memory budget, tile descriptors.
+// After incidence + block pattern: rows per tile and ring depth from the shared-memory budget, tile descriptors.
 int rpim_stage_tiles(rpim_ctx* ctx) {
     cudaStream_t st = ctx->stream;
     ctx->have_tiles = false;
     if (ctx->tg_C == 0) return RPIM_OK;
     const int64_t N = ctx->N;
-    int T = 4;
-    while (T >= 2 && rpim_tiles_smem_bytes(ctx->tg_C, T, ctx->max_blen) > 227 * 1024) T >>= 1;
-    if (T < 2) { ctx->tg_C = 0; return RPIM_OK; }   // rows too long to keep two of them on chip
+    const int Lcap = std::max(ctx->max_blen, 1);
+    // the most rows per tile (8, 6, 4, 2) that leave room for a ring of three stages; then the deepest ring (<= 6)
+    int T = 0, nstage = 0;
+    const unsigned budget = 227u * 1024u;
+    if (Lcap <= 1024)
+        for (int t = TMAX; t >= 2 && T == 0; t -= 2)
+            if (rpim_panel_smem(ctx->tg_C, t, ctx->k, Lcap, 3).total <= budget) T = t;
+    if (const char* e = getenv("RPIM_PANEL_T")) { const int t = atoi(e); if (t >= 2 && t <= TMAX && !(t & 1)) T = t; }
+    if (T == 0) { ctx->tg_C = 0; return RPIM_OK; }   // rows too long to keep two of them on chip
+    for (nstage = 6; nstage > 2 && rpim_panel_smem(ctx->tg_C, T, ctx->k, Lcap, nstage).total > budget; --nstage) {}
+    if (const char* e = getenv("RPIM_PANEL_NSTAGE")) { const int n = atoi(e); if (n >= 2 && n <= 8) nstage = n; }
+    if (rpim_panel_smem(ctx->tg_C, T, ctx->k, Lcap, nstage).total > budget) { ctx->tg_C = 0; return RPIM_OK; }
     const int64_t ntiles = (N + T - 1) / T;
-    const int DW = 1 + (T + 1) / 2;
+    const int DW = 1 + T / 2;
     int rc;
     int* d_cnt = nullptr;
     if ((rc = ws_alloc(ctx, &d_cnt, ntiles))) return rc;
@@ -207,6 +224,7 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
                                                 ctx->d_gpos, nullptr, ctx->d_tile_ptr, ctx->d_tdesc);
     KERNEL_CHECK(ctx);
     ctx->tg_T = T;
+    ctx->tg_nstage = nstage;
     ctx->ntiles = ntiles;
     ctx->have_tiles = true;
     return RPIM_OK;

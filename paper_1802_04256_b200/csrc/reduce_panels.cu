@@ -1,0 +1,369 @@
+// Steps a5 + a6 (R8), PANEL form: w * B^T D B blocks reduced deterministically into the CSR
+// values, for quadrature points that come in groups with overlapping supports (several Gauss points per
+// background cell, or neighbouring cells).  Integer preprocessing: groups.cu.
+//
+// A CTA owns a TILE of T = 2 RP consecutive block rows at a time (tiles strided over a persistent grid).
+// Their accumulators S_IJ (nine doubles per block column, one array per entry: conflict-free for the
+// consecutive slots a warp touches) live in SHARED memory, next to each row's column list and a 16-bit
+// open-addressing table column node -> slot.  The point groups incident to the tile arrive through a ring
+// of NSTAGE shared-memory stages filled by a PRODUCER warp with bulk copies (cp.async.bulk + mbarrier):
+// ONE copy of the staged rows of the group's eight consecutive points and ONE of the group's record (its
+// sorted union of supports U_g, the map (union entry, point) -> support position, the quadrature weights):
+// the bulk-copy engine has a per-request cost, so few large requests, not one per point.  Consumer
+// warp (rp, c) owns rows 2 rp, 2 rp + 1 of the tile and union entries 32 c .. 32 c + 31: a lane sums
+// (w grad phi_I) (x) grad phi_{U_g[u]} over the group's points IN REGISTERS (dense: |U_g| is 1.3 .. 3 k,
+// both rows share the gradient loads), then adds its nine sums per row to the row's accumulator of that
+// column: one table probe and one read-modify-write per (row, group, column) instead of per (row, point,
+// column).  The C warps of a row pair meet at a named barrier between their read-modify-write phases of
+// consecutive groups; nothing else synchronises in the steady state, and the producer runs ahead across
+// tile boundaries.  Every CSR entry is summed in a fixed order (points ascending inside a group, groups
+// ascending) by one lane: no floating-point atomics, bitwise run-to-run reproducible; K is written once,
+// with the isotropic closed form K_IJ = lambda S + mu S^T + mu tr(S) I applied at write-out.
+// The body-force load f_I = b sum_q w phi_I(q) is a separate row-owner pass over the incidence lists.
+#include "bulk_copy.cuh"
+#include "common.cuh"
+
+namespace {
+
+constexpr int GB = RPIM_GROUP_POINTS;
+constexpr unsigned FULLMASK = 0xffffffffu;
+
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void named_bar(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+struct PanelArgs {
+    int64_t N, Nq, ntiles;
+    int k, hlog, nstage;
+    const int64_t* brow_ptr;
+    const int32_t* bcol;
+    const double* stage;
+    const unsigned char* gmeta;
+    const int64_t* tile_ptr;
+    const unsigned* tdesc;
+    double lambda, mu;
+    double* vals;
+    PanelSmem L;
+};
+
+// quadrature weights of every group into the group's record (once per rpim_assemble: the weights are its input)
+__global__ void panel_weights_kernel(int64_t Nq, int64_t G, unsigned meta_bytes, unsigned off_w, const double* __restrict__ qw,
+                                     unsigned char* __restrict__ gmeta) {
+    const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= G * GB) return;
+    reinterpret_cast<double*>(gmeta + (q / GB) * meta_bytes + off_w)[q % GB] = q < Nq ? qw[q] : 0.0;
+}
+
+template <int C, int RP>
+__global__ void __launch_bounds__((RP * C + 1) * 32, 1)
+reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
+    constexpr int T = 2 * RP, NCW = RP * C, NCT = NCW * 32, GCAP = 32 * C, DW = 1 + RP;
+    constexpr unsigned META = GCAP * 12 + GB * 8;   // group record: [jinv: GCAP x 8 bytes][un: GCAP ints][w: GB doubles]
+    constexpr int AWS = 6 * GB;   // doubles of one warp's a-vectors: [p][ax0 ay0 az0 ax1 ay1 az1]
+    extern __shared__ __align__(16) unsigned char panel_smem[];
+    const PanelSmem& L = A.L;
+    double* acc = reinterpret_cast<double*>(panel_smem + L.off_acc);                    // [T][LS][9]
+    int* bcol_s = reinterpret_cast<int*>(panel_smem + L.off_bcol);                      // [T][LS]
+    unsigned short* hash_s = reinterpret_cast<unsigned short*>(panel_smem + L.off_hash);   // [T][HSZ]
+    double* aw_s = reinterpret_cast<double*>(panel_smem + L.off_aw);                    // [NCW][AWS]
+    unsigned char* stages = panel_smem + L.off_stage;
+    const unsigned char* zeros = panel_smem + L.off_zero;                               // 2 k + 2 zero doubles
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(panel_smem + L.off_bar);
+    unsigned long long* empty = full + A.nstage;
+    long long* rowo_s = reinterpret_cast<long long*>(panel_smem + L.off_rowo);          // [T]
+    int* rowL_s = reinterpret_cast<int*>(panel_smem + L.off_rowo + 8 * T);              // [T]
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int k = A.k, LS = L.LS, HSZ = 1 << A.hlog, hshift = 32 - A.hlog, nstage = A.nstage;
+    // stage: [the group's staged rows: GB x 4 x k doubles][group record: META bytes][desc: 8 words]
+    const unsigned gbytes = (unsigned)(GB * 4 * k * 8), off_desc = gbytes + META, stage_bytes = L.stage_bytes;
+    const unsigned k8 = (unsigned)k * 8u;
+
+    if (tid == 0) {
+        for (int s = 0; s < nstage; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NCW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int i = tid; i < 2 * k + 2; i += blockDim.x) reinterpret_cast<double*>(panel_smem + L.off_zero)[i] = 0.0;
+    __syncthreads();
+
+    if (warp == NCW) {
+        // ------------------------------------------------------------------ producer warp
+        int s = 0;
+        unsigned par = 1u;
+        for (int64_t tile = blockIdx.x; tile < A.ntiles; tile += gridDim.x) {
+            const int64_t t0 = A.tile_ptr[tile];
+            const int ng = (int)(A.tile_ptr[tile + 1] - t0);
+            for (int it0 = 0; it0 < ng; it0 += 32) {
+                const int cnt = min(32, ng - it0);
+                unsigned dsc[DW];
+#pragma unroll
+                for (int w = 0; w < DW; ++w) dsc[w] = (lane < cnt) ? A.tdesc[(t0 + it0 + lane) * DW + w] : 0u;
+                for (int i = 0; i < cnt; ++i) {
+                    unsigned mine = 0;   // lane w < DW takes word w of descriptor i
+#pragma unroll
+                    for (int w = 0; w < DW; ++w) {
+                        const unsigned v = __shfl_sync(FULLMASK, dsc[w], i);
+                        if (lane == w) mine = v;
+                    }
+                    const int64_t g = __shfl_sync(FULLMASK, mine, 0);
+                    unsigned char* st = stages + (unsigned)s * stage_bytes;
+                    mbar_wait(&empty[s], par);
+                    if (lane < DW) reinterpret_cast<unsigned*>(st + off_desc)[lane] = mine;
+                    __syncwarp();
+                    if (lane == 0) {
+                        mbar_expect_tx(&full[s], gbytes + META);
+                        bulk_g2s(st, A.stage + g * (GB * 4) * k, gbytes, &full[s]);
+                        bulk_g2s(st + gbytes, A.gmeta + g * META, META, &full[s]);
+                    }
+                    if (++s == nstage) { s = 0; par ^= 1u; }
+                }
+            }
+        }
+        return;
+    }
+
+    // ---------------------------------------------------------------------- consumer warps
+    const int rp = warp / C, c = warp % C;
+    const int r0 = 2 * rp, r1 = r0 + 1;
+    const int u = 32 * c + lane;
+    double* aw = aw_s + warp * AWS;
+    double* acc0 = acc + (size_t)r0 * 9 * LS;
+    double* acc1 = acc + (size_t)r1 * 9 * LS;
+    const unsigned short* hash0 = hash_s + (size_t)r0 * HSZ;
+    const unsigned short* hash1 = hash_s + (size_t)r1 * HSZ;
+    const int* bcol0 = bcol_s + (size_t)r0 * LS;
+    const int* bcol1 = bcol_s + (size_t)r1 * LS;
+    int s = 0;
+    unsigned par = 0u;
+
+    for (int64_t tile = blockIdx.x; tile < A.ntiles; tile += gridDim.x) {
+        named_bar(1, NCT);   // the previous tile's write-out has read its accumulators
+        if (tid < T) {
+            const int64_t I = tile * T + tid;
+            int64_t o = 0;
+            int Lr = 0;
+            if (I < A.N) { o = A.brow_ptr[I]; Lr = (int)(A.brow_ptr[I + 1] - o); }
+            rowo_s[tid] = o;
+            rowL_s[tid] = Lr;
+        }
+        {
+            double2* z = reinterpret_cast<double2*>(acc);
+            const double2 zz = make_double2(0.0, 0.0);
+            for (int i = tid; i < T * 9 * LS / 2; i += NCT) z[i] = zz;
+            unsigned* hz = reinterpret_cast<unsigned*>(hash_s);
+            for (int i = tid; i < T * HSZ / 2; i += NCT) hz[i] = 0xFFFFFFFFu;
+        }
+        named_bar(1, NCT);
+        // column lists and tables: the C warps of a row pair fill the pair's two rows
+#pragma unroll
+        for (int rr = 0; rr < 2; ++rr) {
+            const int r = r0 + rr;
+            const int64_t o_r = rowo_s[r];
+            const int L_r = rowL_s[r];
+            unsigned short* hw = hash_s + (size_t)r * HSZ;
+            int* bc = bcol_s + (size_t)r * LS;
+            for (int sl = c * 32 + lane; sl < L_r; sl += C * 32) {
+                const unsigned J = (unsigned)A.bcol[o_r + sl];
+                bc[sl] = (int)J;
+                unsigned h = (J * 2654435761u) >> hshift;
+                while (atomicCAS(&hw[h], (unsigned short)0xFFFFu, (unsigned short)sl) != (unsigned short)0xFFFFu) h = (h + 1) & (HSZ - 1);
+            }
+        }
+        named_bar(1, NCT);
+        const int ng = (int)(A.tile_ptr[tile + 1] - A.tile_ptr[tile]);
+        for (int it = 0; it < ng; ++it) {
+            const unsigned char* st = stages + (unsigned)s * stage_bytes;
+            mbar_wait(&full[s], par);
+            const unsigned dw = reinterpret_cast<const unsigned*>(st + off_desc)[1 + rp];   // rows 2 rp (low half), 2 rp + 1 (high half)
+            const unsigned u0 = dw & 0xFFu, m0 = (dw >> 8) & 0xFFu, u1 = (dw >> 16) & 0xFFu, m1 = dw >> 24;
+            const unsigned mm = m0 | m1;
+            double s0[9], s1[9];
+            int slot0 = -1, slot1 = -1;
+            bool work = false;
+            if (mm != 0u) {
+                const unsigned long long* jinv = reinterpret_cast<const unsigned long long*>(st + gbytes);
+                const int J = reinterpret_cast<const int*>(st + gbytes + GCAP * 8)[u];
+                work = __ballot_sync(FULLMASK, J >= 0) != 0u;
+                if (work) {
+                    const unsigned long long jv = jinv[u];
+                    // w * grad phi_I of the two rows' nodes at the group's points: lane p + 8 rr (zero when the
+                    // point does not hold the row's node)
+                    if (lane < 2 * GB) {
+                        const int p = lane & (GB - 1), rr = lane >> 3;
+                        const unsigned ur = rr ? u1 : u0, mr = rr ? m1 : m0;
+                        double ax = 0.0, ay = 0.0, az = 0.0;
+                        if ((mr >> p) & 1u) {
+                            const unsigned j = (unsigned)(jinv[ur] >> (8 * p)) & 0xFFu;
+                            const double wq = reinterpret_cast<const double*>(st + gbytes + GCAP * 12)[p];
+                            const double* gp = reinterpret_cast<const double*>(st) + (4 * p + 1) * k + j;
+                            ax = wq * gp[0]; ay = wq * gp[k]; az = wq * gp[2 * k];
+                        }
+                        double* dst = aw + p * 6 + rr * 3;
+                        dst[0] = ax; dst[1] = ay; dst[2] = az;
+                    }
+                    __syncwarp();
+                    const unsigned jlo = (unsigned)jv, jhi = (unsigned)(jv >> 32);
+#pragma unroll
+                    for (int p = 0; p < GB; ++p) {
+                        const unsigned jb = ((p < 4 ? jlo : jhi) >> (8 * (p & 3))) & 0xFFu;
+                        // absent (0xFF): the zero area stands in for the three gradient rows
+                        const unsigned char* gq = (jb != 0xFFu) ? st + (unsigned)(4 * p + 1) * k8 + jb * 8u : zeros;
+                        const double gx = *reinterpret_cast<const double*>(gq);
+                        const double gy = *reinterpret_cast<const double*>(gq + k8);
+                        const double gz = *reinterpret_cast<const double*>(gq + 2 * k8);
+                        const double2 a01 = *reinterpret_cast<const double2*>(aw + p * 6);       // ax0 ay0
+                        const double2 a23 = *reinterpret_cast<const double2*>(aw + p * 6 + 2);   // az0 ax1
+                        const double2 a45 = *reinterpret_cast<const double2*>(aw + p * 6 + 4);   // ay1 az1
+                        if (p == 0) {
+                            s0[0] = a01.x * gx; s0[1] = a01.x * gy; s0[2] = a01.x * gz;
+                            s0[3] = a01.y * gx; s0[4] = a01.y * gy; s0[5] = a01.y * gz;
+                            s0[6] = a23.x * gx; s0[7] = a23.x * gy; s0[8] = a23.x * gz;
+                            s1[0] = a23.y * gx; s1[1] = a23.y * gy; s1[2] = a23.y * gz;
+                            s1[3] = a45.x * gx; s1[4] = a45.x * gy; s1[5] = a45.x * gz;
+                            s1[6] = a45.y * gx; s1[7] = a45.y * gy; s1[8] = a45.y * gz;
+                        } else {
+                            s0[0] = fma(a01.x, gx, s0[0]); s0[1] = fma(a01.x, gy, s0[1]); s0[2] = fma(a01.x, gz, s0[2]);
+                            s0[3] = fma(a01.y, gx, s0[3]); s0[4] = fma(a01.y, gy, s0[4]); s0[5] = fma(a01.y, gz, s0[5]);
+                            s0[6] = fma(a23.x, gx, s0[6]); s0[7] = fma(a23.x, gy, s0[7]); s0[8] = fma(a23.x, gz, s0[8]);
+                            s1[0] = fma(a23.y, gx, s1[0]); s1[1] = fma(a23.y, gy, s1[1]); s1[2] = fma(a23.y, gz, s1[2]);
+                            s1[3] = fma(a45.x, gx, s1[3]); s1[4] = fma(a45.x, gy, s1[4]); s1[5] = fma(a45.x, gz, s1[5]);
+                            s1[6] = fma(a45.y, gx, s1[6]); s1[7] = fma(a45.y, gy, s1[7]); s1[8] = fma(a45.y, gz, s1[8]);
+                        }
+                    }
+                    // column slots: the entry (I, U_g[u]) exists iff some point holds both nodes; a pair without
+                    // an entry has only zero sums and is skipped
+                    if (J >= 0) {
+                        const unsigned h00 = ((unsigned)J * 2654435761u) >> hshift;
+                        if (m0) {
+                            unsigned h = h00;
+                            while (true) {
+                                const unsigned sl = hash0[h];
+                                if (sl == 0xFFFFu) break;
+                                if (bcol0[sl] == J) { slot0 = (int)sl; break; }
+                                h = (h + 1) & (HSZ - 1);
+                            }
+                        }
+                        if (m1) {
+                            unsigned h = h00;
+                            while (true) {
+                                const unsigned sl = hash1[h];
+                                if (sl == 0xFFFFu) break;
+                                if (bcol1[sl] == J) { slot1 = (int)sl; break; }
+                                h = (h + 1) & (HSZ - 1);
+                            }
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);   // the stage (and this warp's a-vectors) are no longer read
+            if (++s == nstage) { s = 0; par ^= 1u; }
+            if (mm != 0u) {
+                // read-modify-write phases of consecutive groups are separated for the C warps of the row pair
+                if (C > 1) named_bar(2 + rp, C * 32);
+                if (work) {
+                    if (slot0 >= 0) {
+                        double* a = acc0 + slot0 * 9;
+#pragma unroll
+                        for (int e = 0; e < 9; ++e) a[e] += s0[e];
+                    }
+                    if (slot1 >= 0) {
+                        double* a = acc1 + slot1 * 9;
+#pragma unroll
+                        for (int e = 0; e < 9; ++e) a[e] += s1[e];
+                    }
+                }
+            }
+        }
+        named_bar(1, NCT);   // every contribution is in the accumulators
+        // ---- K_IJ = lambda S + mu S^T + mu tr(S) I, three scalar rows of 3 L entries per block row
+        for (int r = 0; r < T; ++r) {
+            const int Lr = rowL_s[r];
+            if (Lr == 0) continue;
+            const double* ar = acc + (size_t)r * 9 * LS;
+            double* dst = A.vals + 9 * rowo_s[r];
+            const int L3 = 3 * Lr;
+#pragma unroll
+            for (int row = 0; row < 3; ++row) {
+                for (int col = tid; col < L3; col += NCT) {
+                    const int sl = (int)(((unsigned)col * 43691u) >> 17);   // col / 3 for col < 2^15 (columns <= 3 * 1024)
+                    const int cc = col - 3 * sl;
+                    const double* a = ar + sl * 9;
+                    double v = fma(A.lambda, a[3 * row + cc], A.mu * a[3 * cc + row]);
+                    if (row == cc) v += A.mu * ((a[0] + a[4]) + a[8]);
+                    __stcs(dst + (size_t)row * L3 + col, v);
+                }
+            }
+        }
+    }
+}
+
+// f_I = b * sum over the incident points (ascending) of w phi_I: one warp per block row, lane-strided
+// partial sums combined in a fixed order (bitwise reproducible)
+__global__ void __launch_bounds__(256)
+load_rows_kernel(int64_t N, int k, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
+                 const uint8_t* __restrict__ inc_j, const double* __restrict__ stage, const double* __restrict__ qw,
+                 double bx, double by, double bz, double* __restrict__ f) {
+    const int lane = threadIdx.x & 31;
+    const int64_t I = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (I >= N) return;
+    const int64_t pa = inc_ptr[I], pb = inc_ptr[I + 1];
+    double sum = 0.0;
+    for (int64_t p = pa + lane; p < pb; p += 32) {
+        const int64_t q = inc_q[p];
+        sum += qw[q] * stage[q * 4 * k + inc_j[p]];
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) sum += __shfl_xor_sync(FULLMASK, sum, d);
+    if (lane == 0) { f[3 * I] = sum * bx; f[3 * I + 1] = sum * by; f[3 * I + 2] = sum * bz; }
+}
+
+template <int C, int RP>
+int launch_panels(rpim_ctx* ctx, PanelArgs& A) {
+    auto kern = reduce_panels_kernel<C, RP>;
+    const size_t smem = A.L.total;
+    CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 1, sms = 148;
+    CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, (RP * C + 1) * 32, smem));
+    if (per_sm < 1) RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "panel reduction does not fit on chip (rows of %d block columns)", ctx->max_blen);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
+    const int64_t blocks = std::min<int64_t>(A.ntiles, (int64_t)sms * per_sm);
+    kern<<<(unsigned)blocks, (RP * C + 1) * 32, smem, ctx->stream>>>(A);
+    KERNEL_CHECK(ctx);
+    return RPIM_OK;
+}
+
+}  // namespace
+
+int rpim_stage_accumulate_panels(rpim_ctx* ctx, const double* d_qw, double lambda, double mu, const double body[3],
+                                 double* d_vals, double* d_f) {
+    PanelArgs A;
+    A.N = ctx->N; A.Nq = ctx->Nq; A.ntiles = ctx->ntiles;
+    A.k = ctx->k;
+    A.L = rpim_panel_smem(ctx->tg_C, ctx->tg_T, ctx->k, std::max(ctx->max_blen, 1), ctx->tg_nstage);
+    A.hlog = A.L.hlog; A.nstage = ctx->tg_nstage;
+    A.brow_ptr = ctx->d_brow_ptr; A.bcol = ctx->d_bcol; A.stage = ctx->d_stage;
+    A.gmeta = ctx->d_gmeta;
+    A.tile_ptr = ctx->d_tile_ptr; A.tdesc = ctx->d_tdesc;
+    A.lambda = lambda; A.mu = mu; A.vals = d_vals;
+    const int64_t G = (ctx->Nq + GB - 1) / GB;
+    const unsigned meta = rpim_panel_meta_bytes(ctx->tg_C);
+    panel_weights_kernel<<<(unsigned)((G * GB + 255) / 256), 256, 0, ctx->stream>>>(ctx->Nq, G, meta, 32u * ctx->tg_C * 12u, d_qw, ctx->d_gmeta);
+    KERNEL_CHECK(ctx);
+    {
+        const int wpb = 8;
+        load_rows_kernel<<<(unsigned)((ctx->N + wpb - 1) / wpb), wpb * 32, 0, ctx->stream>>>(
+            ctx->N, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_stage, d_qw, body[0], body[1], body[2], d_f);
+        KERNEL_CHECK(ctx);
+    }
+    const int C = ctx->tg_C, RP = ctx->tg_T / 2;
+#define RPIM_PANELS_CASE(CC, RR) if (C == CC && RP == RR) return launch_panels<CC, RR>(ctx, A)
+    RPIM_PANELS_CASE(2, 1); RPIM_PANELS_CASE(2, 2); RPIM_PANELS_CASE(2, 3); RPIM_PANELS_CASE(2, 4);
+    RPIM_PANELS_CASE(3, 1); RPIM_PANELS_CASE(3, 2); RPIM_PANELS_CASE(3, 3); RPIM_PANELS_CASE(3, 4);
+    RPIM_PANELS_CASE(4, 1); RPIM_PANELS_CASE(4, 2); RPIM_PANELS_CASE(4, 3); RPIM_PANELS_CASE(4, 4);
+#undef RPIM_PANELS_CASE
+    RPIM_FAIL(ctx, RPIM_ERR_STATE, "no panel reduction kernel for C = %d, T = %d", C, ctx->tg_T);
+}

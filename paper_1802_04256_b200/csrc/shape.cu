@@ -311,7 +311,7 @@ shape_generic_kernel(const double* __restrict__ nodes, const double* __restrict_
             const double p0 = Y[4 * u], g1 = Y[4 * u + 1] * SP.inv_dc, g2 = Y[4 * u + 2] * SP.inv_dc,
                          g3 = Y[4 * u + 3] * SP.inv_dc;
             finite = finite && isfinite(p0) && isfinite(g1) && isfinite(g2) && isfinite(g3);
-            out[4 * pu] = p0; out[4 * pu + 1] = g1; out[4 * pu + 2] = g2; out[4 * pu + 3] = g3;
+            out[pu] = p0; out[k + pu] = g1; out[2 * k + pu] = g2; out[3 * k + pu] = g3;   // staged layout [q][phi, d/dx, d/dy, d/dz][k]
         }
         if (__any_sync(0xffffffffu, !finite)) {
             __syncwarp();

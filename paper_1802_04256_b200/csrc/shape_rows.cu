@@ -473,7 +473,7 @@ shape_rows_kernel(const double* __restrict__ nodes, const double* __restrict__ p
             }
         });
 
-        // ---- outputs in support order; derivatives back to physical coordinates
+        // ---- outputs in support order (staged layout [q][phi, d/dx, d/dy, d/dz][K]); derivatives back to physical coordinates
         double* out = stage + q * 4 * (int64_t)K;
         bool finite = true;
 #pragma unroll
@@ -481,13 +481,13 @@ shape_rows_kernel(const double* __restrict__ nodes, const double* __restrict__ p
             const int ir = skipmap(urow[s], bs);
             const double p0 = Y[s][0], g1 = Y[s][1] * inv_dc, g2 = Y[s][2] * inv_dc, g3 = Y[s][3] * inv_dc;
             finite = finite && isfinite(p0) && isfinite(g1) && isfinite(g2) && isfinite(g3);
-            if (live) { st2(out + 4 * ir, p0, g1); st2(out + 4 * ir + 2, g2, g3); }
+            if (live) { out[ir] = p0; out[K + ir] = g1; out[2 * K + ir] = g2; out[3 * K + ir] = g3; }
         }
         if (!hpoly) {
             const int ia = (hm == 0) ? anc[0] : (hm == 1) ? anc[1] : (hm == 2) ? anc[2] : anc[3];
             const double p0 = Y[HS][0], g1 = Y[HS][1] * inv_dc, g2 = Y[HS][2] * inv_dc, g3 = Y[HS][3] * inv_dc;
             finite = finite && isfinite(p0) && isfinite(g1) && isfinite(g2) && isfinite(g3);
-            if (live) { st2(out + 4 * ia, p0, g1); st2(out + 4 * ia + 2, g2, g3); }
+            if (live) { out[ia] = p0; out[K + ia] = g1; out[2 * K + ia] = g2; out[3 * K + ia] = g3; }
         }
         const unsigned gmask = (G == 32) ? FULL : (0xffffu << (16 * grp));
         const bool fail = ((__ballot_sync(FULL, bad || !finite) & gmask) != 0u);

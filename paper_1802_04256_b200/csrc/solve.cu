@@ -231,8 +231,8 @@ stress_kernel(int64_t Nq, int k, const int32_t* __restrict__ support, const doub
         double e[6] = {0, 0, 0, 0, 0, 0};   // exx eyy ezz gxy gyz gzx (engineering shear)
         for (int j = lane; j < k; j += 32) {
             const int64_t J = support[q * k + j];
-            const double* g = stage + (q * k + j) * 4;
-            const double gx = g[1], gy = g[2], gz = g[3];
+            const double* g = stage + q * 4 * k + j;   // staged layout [q][phi, d/dx, d/dy, d/dz][k]
+            const double gx = g[k], gy = g[2 * k], gz = g[3 * k];
             const double ux = u[3 * J], uy = u[3 * J + 1], uz = u[3 * J + 2];
             e[0] = fma(gx, ux, e[0]);
             e[1] = fma(gy, uy, e[1]);

@@ -69,20 +69,21 @@ def test_jittered_blocks_span_tiles_and_ragged_tails(k, dims, jit, gauss):
 
 
 @pytest.mark.parametrize("k,dims,gauss", [
-    (27, (7, 7, 6), 2),            # union of a cell's 8 supports: 2 chunks of 32
+    (27, (7, 7, 6), 2),            # union of a cell's 8 supports: 2 chunks of 32; odd k
     (40, (9, 8, 7), 2),            # 3 chunks
     (60, (10, 9, 8), 2),           # 4 chunks, rows of ~400 block columns
     (30, (9, 5, 5), 3),            # 27 points per cell: groups of 8 straddle cells
-    (124, (9, 8, 8), 2),           # unions near the 192-node limit (beyond it the row-owner kernel takes over)
+    (124, (9, 8, 8), 2),           # unions beyond the 128-node limit: the row-owner kernel takes over
+    (64, (9, 9, 8), 2),
     (12, (6, 6, 5), 1),            # one point per cell: sparse groups, still correct
 ])
-def test_tiled_reduction_matches_the_oracle_and_the_row_owner_kernel(k, dims, gauss):
-    # rpim_set_reduction(ctx, 2): groups of 8 points, tiles of rows, accumulators in shared memory
-    # (reduce_tiles.cu).  Same bars as the default path; run twice for bitwise reproducibility.
+def test_panel_reduction_matches_the_oracle_and_the_row_owner_kernel(k, dims, gauss):
+    # rpim_set_reduction(ctx, 2): groups of 8 points, tiles of rows, accumulators in shared memory, group panels
+    # through a bulk-copy ring (reduce_panels.cu).  Same bars as the default path; run twice for bitwise reproducibility.
     w = workloads.make_block(f"t{k}", *dims, 1.0, gauss, k, 5e9, 0.3, jitter=0.3, seed=300 + k,
                              body=(10.0, -20.0, -2.5e4), bc="bottom+roller")
     g, o = run_cuda(w, reduction=2), run_oracle(w)
-    assert g["reduction_used"] == 2 or (k == 124 and g["reduction_used"] == 1)
+    assert g["reduction_used"] == (1 if k == 124 else 2)
     _compare(w, g, o)
     g2 = run_cuda(w, reduction=2)
     assert np.array_equal(g["vals"], g2["vals"]) and np.array_equal(g["f"], g2["f"])

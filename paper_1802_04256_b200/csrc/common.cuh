@@ -93,6 +93,8 @@ struct rpim_ctx {
     int tg_C = 0;                    // 32-lane chunks per group union (0: panel path not applicable)
     int tg_T = 0;                    // block rows per tile (even)
     int tg_nstage = 0;               // stages of the group ring
+    int tg_CW = 0;                   // consumer warps per row pair
+    int max_ulen = 0;                // most upper block columns (diagonal included) of a row
     double tg_mean_union = 0.0;      // mean |U_g| of the last statistics pass
     int64_t ntiles = 0;
     uint8_t* d_gpos = nullptr;       // Nq x k: position of (point, support node) in its group's union
@@ -239,32 +241,31 @@ int rpim_stage_point_loads(rpim_ctx* ctx, const int32_t* d_support, const double
 int rpim_stage_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* d_bc_mask, const double* d_u_bar,
                        int64_t m, double alpha, int relative, double* d_vals, double* d_f, double* out_alpha);
 
-// Dynamic shared memory of reduce_panels_kernel<C, T / 2> (reduce_panels.cu) for rows of up to Lcap block
-// columns: byte offsets of its areas, identical on host and device.
+// Dynamic shared memory of reduce_panels_kernel<CW, T / 2> (reduce_panels.cu) for rows of up to Ucap upper
+// block columns (diagonal included): byte offsets of its areas, identical on host and device.
 struct PanelSmem {
-    int LS;            // accumulator / column-list stride in block columns (Lcap rounded up to even)
-    int hlog;          // log2 of the per-row table size (power of two >= 2 Lcap)
+    int LS;            // accumulator / column-list stride in block columns (Ucap rounded up to even)
+    int hlog;          // log2 of the per-row table size (power of two >= 2 Ucap)
     unsigned stage_bytes;
-    unsigned off_acc, off_bcol, off_hash, off_aw, off_stage, off_zero, off_bar, off_rowo, total;
+    unsigned off_acc, off_bcol, off_hash, off_aw, off_stage, off_bar, off_rowo, total;
 };
 // bytes of a group's record: [jinv: 32 C x 8][union node ids: 32 C ints][weights: 8 doubles]
 inline unsigned rpim_panel_meta_bytes(int C) { return 32u * C * 12u + RPIM_GROUP_POINTS * 8u; }
-inline PanelSmem rpim_panel_smem(int C, int T, int k, int Lcap, int nstage) {
+inline PanelSmem rpim_panel_smem(int C, int CW, int T, int k, int Ucap, int nstage) {
     PanelSmem L;
-    L.LS = (Lcap + 1) & ~1;
+    L.LS = (Ucap + 1) & ~1;
     L.hlog = 6;
-    while ((1 << L.hlog) < 2 * Lcap) ++L.hlog;
+    while ((1 << L.hlog) < 2 * Ucap) ++L.hlog;
     L.stage_bytes = (unsigned)(RPIM_GROUP_POINTS * 4 * k * 8) + rpim_panel_meta_bytes(C) + 32u;
     auto up16 = [](unsigned v) { return (v + 15u) & ~15u; };
     unsigned o = 0;
     L.off_acc = o; o = up16(o + (unsigned)T * 9u * L.LS * 8u);
     L.off_bcol = o; o = up16(o + (unsigned)T * L.LS * 4u);
     L.off_hash = o; o = up16(o + (unsigned)T * (2u << L.hlog));
-    L.off_aw = o; o = up16(o + (unsigned)(T / 2) * C * RPIM_GROUP_POINTS * 6u * 8u);
+    L.off_aw = o; o = up16(o + (unsigned)(T / 2) * CW * RPIM_GROUP_POINTS * 6u * 8u);
     L.off_stage = o; o = up16(o + (unsigned)nstage * L.stage_bytes);
-    L.off_zero = o; o = up16(o + (unsigned)(2 * k + 2) * 8u);
     L.off_bar = o; o = up16(o + 2u * nstage * 8u);
-    L.off_rowo = o; o = up16(o + (unsigned)T * 12u);
+    L.off_rowo = o; o = up16(o + (unsigned)T * 16u);
     L.total = o;
     return L;
 }

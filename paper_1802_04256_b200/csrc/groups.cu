@@ -184,24 +184,45 @@ int rpim_stage_groups(rpim_ctx* ctx) {
     return RPIM_OK;
 }
 
+namespace {
+// most upper block columns (diagonal included) of a block row
+__global__ void max_ulen_kernel(int64_t N, const int* __restrict__ blen, const int* __restrict__ bdiag, int* __restrict__ out) {
+    int m = 0;
+    for (int64_t I = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; I < N; I += (int64_t)gridDim.x * blockDim.x)
+        if (blen[I] > 0) m = max(m, blen[I] - bdiag[I]);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, d));
+    if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
+}
+}  // namespace
+
 // After incidence + block pattern: rows per tile and ring depth from the shared-memory budget, tile descriptors.
 int rpim_stage_tiles(rpim_ctx* ctx) {
     cudaStream_t st = ctx->stream;
     ctx->have_tiles = false;
     if (ctx->tg_C == 0) return RPIM_OK;
     const int64_t N = ctx->N;
-    const int Lcap = std::max(ctx->max_blen, 1);
-    // the most rows per tile (8, 6, 4, 2) that leave room for a ring of three stages; then the deepest ring (<= 6)
+    int* d_max = (int*)ctx->d_scratch;
+    CUDA_TRY(ctx, cudaMemsetAsync(d_max, 0, sizeof(int), st));
+    max_ulen_kernel<<<(unsigned)std::min<int64_t>((N + 255) / 256, 1024), 256, 0, st>>>(N, ctx->d_blen, ctx->d_bdiag, d_max);
+    KERNEL_CHECK(ctx);
+    CUDA_TRY(ctx, cudaMemcpyAsync(&ctx->max_ulen, d_max, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    const int Ucap = std::max(ctx->max_ulen, 1);
+    // consumer warps per row pair; the most rows per tile (8, 6, 4, 2) that leave room for a ring of three
+    // stages; then the deepest ring (<= 6)
+    int CW = std::min(2, ctx->tg_C);
+    if (const char* e = getenv("RPIM_PANEL_CW")) { const int c = atoi(e); if (c >= 1 && c <= 3) CW = c; }
     int T = 0, nstage = 0;
     const unsigned budget = 227u * 1024u;
-    if (Lcap <= 1024)
+    if (Ucap <= 1024)
         for (int t = TMAX; t >= 2 && T == 0; t -= 2)
-            if (rpim_panel_smem(ctx->tg_C, t, ctx->k, Lcap, 3).total <= budget) T = t;
+            if (rpim_panel_smem(ctx->tg_C, CW, t, ctx->k, Ucap, 3).total <= budget) T = t;
     if (const char* e = getenv("RPIM_PANEL_T")) { const int t = atoi(e); if (t >= 2 && t <= TMAX && !(t & 1)) T = t; }
     if (T == 0) { ctx->tg_C = 0; return RPIM_OK; }   // rows too long to keep two of them on chip
-    for (nstage = 6; nstage > 2 && rpim_panel_smem(ctx->tg_C, T, ctx->k, Lcap, nstage).total > budget; --nstage) {}
+    for (nstage = 6; nstage > 2 && rpim_panel_smem(ctx->tg_C, CW, T, ctx->k, Ucap, nstage).total > budget; --nstage) {}
     if (const char* e = getenv("RPIM_PANEL_NSTAGE")) { const int n = atoi(e); if (n >= 2 && n <= 8) nstage = n; }
-    if (rpim_panel_smem(ctx->tg_C, T, ctx->k, Lcap, nstage).total > budget) { ctx->tg_C = 0; return RPIM_OK; }
+    if (rpim_panel_smem(ctx->tg_C, CW, T, ctx->k, Ucap, nstage).total > budget) { ctx->tg_C = 0; return RPIM_OK; }
     const int64_t ntiles = (N + T - 1) / T;
     const int DW = 1 + T / 2;
     int rc;
@@ -224,6 +245,7 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
                                                 ctx->d_gpos, nullptr, ctx->d_tile_ptr, ctx->d_tdesc);
     KERNEL_CHECK(ctx);
     ctx->tg_T = T;
+    ctx->tg_CW = CW;
     ctx->tg_nstage = nstage;
     ctx->ntiles = ntiles;
     ctx->have_tiles = true;

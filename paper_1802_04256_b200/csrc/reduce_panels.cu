@@ -2,23 +2,28 @@
 // values, for quadrature points that come in groups with overlapping supports (several Gauss points per
 // background cell, or neighbouring cells).  Integer preprocessing: groups.cu.
 //
+// K is symmetric block-wise (K_JI = K_IJ^T, R8: one support per point), so only the UPPER blocks
+// (column node J >= row node I) are accumulated; mirror_lower_kernel then fills the lower blocks with the
+// transposes.  Half the arithmetic, half the on-chip accumulators (twice the rows per tile).
+//
 // A CTA owns a TILE of T = 2 RP consecutive block rows at a time (tiles strided over a persistent grid).
-// Their accumulators S_IJ (nine doubles per block column, one array per entry: conflict-free for the
-// consecutive slots a warp touches) live in SHARED memory, next to each row's column list and a 16-bit
-// open-addressing table column node -> slot.  The point groups incident to the tile arrive through a ring
-// of NSTAGE shared-memory stages filled by a PRODUCER warp with bulk copies (cp.async.bulk + mbarrier):
-// ONE copy of the staged rows of the group's eight consecutive points and ONE of the group's record (its
-// sorted union of supports U_g, the map (union entry, point) -> support position, the quadrature weights):
-// the bulk-copy engine has a per-request cost, so few large requests, not one per point.  Consumer
-// warp (rp, c) owns rows 2 rp, 2 rp + 1 of the tile and union entries 32 c .. 32 c + 31: a lane sums
-// (w grad phi_I) (x) grad phi_{U_g[u]} over the group's points IN REGISTERS (dense: |U_g| is 1.3 .. 3 k,
-// both rows share the gradient loads), then adds its nine sums per row to the row's accumulator of that
-// column: one table probe and one read-modify-write per (row, group, column) instead of per (row, point,
-// column).  The C warps of a row pair meet at a named barrier between their read-modify-write phases of
-// consecutive groups; nothing else synchronises in the steady state, and the producer runs ahead across
-// tile boundaries.  Every CSR entry is summed in a fixed order (points ascending inside a group, groups
-// ascending) by one lane: no floating-point atomics, bitwise run-to-run reproducible; K is written once,
-// with the isotropic closed form K_IJ = lambda S + mu S^T + mu tr(S) I applied at write-out.
+// The accumulators S_IJ of their upper blocks (nine doubles per block column) live in SHARED memory, next to
+// each row's upper column list and a 16-bit open-addressing table column node -> slot.  The point groups
+// incident to the tile arrive through a ring of NSTAGE shared-memory stages filled by a PRODUCER warp with
+// bulk copies (cp.async.bulk + mbarrier): ONE copy of the staged rows of the group's eight consecutive
+// points and ONE of the group's record (its sorted union of supports U_g, the map (union entry, point) ->
+// support position, the quadrature weights): the bulk-copy engine has a per-request cost, so few large
+// requests, not one per point.  Row pair rp (rows 2 rp, 2 rp + 1) has CW consumer warps; the chunks of 32
+// union entries from the one that holds the rows' own nodes upwards (U_g is ascending: everything below
+// is a lower block) are dealt to them round-robin.  In a chunk a lane owns one union entry and sums
+// (w grad phi_I) (x) grad phi_{U_g[u]} over the group's points IN REGISTERS (dense: |U_g| is 1.3 .. 3 k, both
+// rows share the gradient loads), then adds its nine sums per row to the row's accumulator of that column:
+// one table probe and one read-modify-write per (row, group, column) instead of per (row, point, column).
+// The CW warps of a row pair meet at a named barrier between their read-modify-write phases of consecutive
+// groups; nothing else synchronises in the steady state, and the producer runs ahead across tile
+// boundaries.  Every CSR entry is summed in a fixed order (points ascending inside a group, groups
+// ascending) by one lane: no floating-point atomics, bitwise run-to-run reproducible; every entry of K is
+// written once, with the isotropic closed form K_IJ = lambda S + mu S^T + mu tr(S) I applied at write-out.
 // The body-force load f_I = b sum_q w phi_I(q) is a separate row-owner pass over the incidence lists.
 #include "bulk_copy.cuh"
 #include "common.cuh"
@@ -37,9 +42,10 @@ __device__ __forceinline__ void named_bar(int id, int nthreads) {
 
 struct PanelArgs {
     int64_t N, Nq, ntiles;
-    int k, hlog, nstage;
+    int k, C, hlog, nstage;
     const int64_t* brow_ptr;
     const int32_t* bcol;
+    const int* bdiag;
     const double* stage;
     const unsigned char* gmeta;
     const int64_t* tile_ptr;
@@ -57,11 +63,10 @@ __global__ void panel_weights_kernel(int64_t Nq, int64_t G, unsigned meta_bytes,
     reinterpret_cast<double*>(gmeta + (q / GB) * meta_bytes + off_w)[q % GB] = q < Nq ? qw[q] : 0.0;
 }
 
-template <int C, int RP>
-__global__ void __launch_bounds__((RP * C + 1) * 32, 1)
+template <int CW, int RP>
+__global__ void __launch_bounds__((RP * CW + 1) * 32, 1)
 reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
-    constexpr int T = 2 * RP, NCW = RP * C, NCT = NCW * 32, GCAP = 32 * C, DW = 1 + RP;
-    constexpr unsigned META = GCAP * 12 + GB * 8;   // group record: [jinv: GCAP x 8 bytes][un: GCAP ints][w: GB doubles]
+    constexpr int T = 2 * RP, NCW = RP * CW, NCT = NCW * 32, DW = 1 + RP;
     constexpr int AWS = 6 * GB;   // doubles of one warp's a-vectors: [p][ax0 ay0 az0 ax1 ay1 az1]
     extern __shared__ __align__(16) unsigned char panel_smem[];
     const PanelSmem& L = A.L;
@@ -70,23 +75,23 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
     unsigned short* hash_s = reinterpret_cast<unsigned short*>(panel_smem + L.off_hash);   // [T][HSZ]
     double* aw_s = reinterpret_cast<double*>(panel_smem + L.off_aw);                    // [NCW][AWS]
     unsigned char* stages = panel_smem + L.off_stage;
-    const unsigned char* zeros = panel_smem + L.off_zero;                               // 2 k + 2 zero doubles
     unsigned long long* full = reinterpret_cast<unsigned long long*>(panel_smem + L.off_bar);
     unsigned long long* empty = full + A.nstage;
-    long long* rowo_s = reinterpret_cast<long long*>(panel_smem + L.off_rowo);          // [T]
-    int* rowL_s = reinterpret_cast<int*>(panel_smem + L.off_rowo + 8 * T);              // [T]
+    long long* rowo_s = reinterpret_cast<long long*>(panel_smem + L.off_rowo);          // [T] first block of the row
+    int* rowL_s = reinterpret_cast<int*>(panel_smem + L.off_rowo + 8 * T);              // [T] block columns of the row
+    int* rowd_s = rowL_s + T;                                                           // [T] slot of the diagonal block
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int k = A.k, LS = L.LS, HSZ = 1 << A.hlog, hshift = 32 - A.hlog, nstage = A.nstage;
-    // stage: [the group's staged rows: GB x 4 x k doubles][group record: META bytes][desc: 8 words]
-    const unsigned gbytes = (unsigned)(GB * 4 * k * 8), off_desc = gbytes + META, stage_bytes = L.stage_bytes;
+    const int k = A.k, C = A.C, LS = L.LS, HSZ = 1 << A.hlog, hshift = 32 - A.hlog, nstage = A.nstage;
+    // stage: [the group's staged rows: GB x 4 x k doubles][group record: jinv, union ids, weights][desc: 8 words]
+    const unsigned gcap = 32u * C, meta = gcap * 12u + GB * 8u;
+    const unsigned gbytes = (unsigned)(GB * 4 * k * 8), off_desc = gbytes + meta, stage_bytes = L.stage_bytes;
     const unsigned k8 = (unsigned)k * 8u;
 
     if (tid == 0) {
         for (int s = 0; s < nstage; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NCW); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int i = tid; i < 2 * k + 2; i += blockDim.x) reinterpret_cast<double*>(panel_smem + L.off_zero)[i] = 0.0;
     __syncthreads();
 
     if (warp == NCW) {
@@ -114,9 +119,9 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
                     if (lane < DW) reinterpret_cast<unsigned*>(st + off_desc)[lane] = mine;
                     __syncwarp();
                     if (lane == 0) {
-                        mbar_expect_tx(&full[s], gbytes + META);
+                        mbar_expect_tx(&full[s], gbytes + meta);
                         bulk_g2s(st, A.stage + g * (GB * 4) * k, gbytes, &full[s]);
-                        bulk_g2s(st + gbytes, A.gmeta + g * META, META, &full[s]);
+                        bulk_g2s(st + gbytes, A.gmeta + g * meta, meta, &full[s]);
                     }
                     if (++s == nstage) { s = 0; par ^= 1u; }
                 }
@@ -126,9 +131,8 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
     }
 
     // ---------------------------------------------------------------------- consumer warps
-    const int rp = warp / C, c = warp % C;
+    const int rp = warp / CW, w = warp % CW;
     const int r0 = 2 * rp, r1 = r0 + 1;
-    const int u = 32 * c + lane;
     double* aw = aw_s + warp * AWS;
     double* acc0 = acc + (size_t)r0 * 9 * LS;
     double* acc1 = acc + (size_t)r1 * 9 * LS;
@@ -144,10 +148,11 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
         if (tid < T) {
             const int64_t I = tile * T + tid;
             int64_t o = 0;
-            int Lr = 0;
-            if (I < A.N) { o = A.brow_ptr[I]; Lr = (int)(A.brow_ptr[I + 1] - o); }
+            int Lr = 0, d = 0;
+            if (I < A.N) { o = A.brow_ptr[I]; Lr = (int)(A.brow_ptr[I + 1] - o); d = Lr ? A.bdiag[I] : 0; }
             rowo_s[tid] = o;
             rowL_s[tid] = Lr;
+            rowd_s[tid] = d;
         }
         {
             double2* z = reinterpret_cast<double2*>(acc);
@@ -157,15 +162,15 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
             for (int i = tid; i < T * HSZ / 2; i += NCT) hz[i] = 0xFFFFFFFFu;
         }
         named_bar(1, NCT);
-        // column lists and tables: the C warps of a row pair fill the pair's two rows
+        // upper column lists (from the diagonal on) and tables: the CW warps of a row pair fill the pair's two rows
 #pragma unroll
         for (int rr = 0; rr < 2; ++rr) {
             const int r = r0 + rr;
-            const int64_t o_r = rowo_s[r];
-            const int L_r = rowL_s[r];
+            const int64_t o_r = rowo_s[r] + rowd_s[r];
+            const int Lu = rowL_s[r] - rowd_s[r];
             unsigned short* hw = hash_s + (size_t)r * HSZ;
             int* bc = bcol_s + (size_t)r * LS;
-            for (int sl = c * 32 + lane; sl < L_r; sl += C * 32) {
+            for (int sl = w * 32 + lane; sl < Lu; sl += CW * 32) {
                 const unsigned J = (unsigned)A.bcol[o_r + sl];
                 bc[sl] = (int)J;
                 unsigned h = (J * 2654435761u) >> hshift;
@@ -173,6 +178,7 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
             }
         }
         named_bar(1, NCT);
+        const int I0 = (int)(tile * T) + r0, I1 = I0 + 1;
         const int ng = (int)(A.tile_ptr[tile + 1] - A.tile_ptr[tile]);
         for (int it = 0; it < ng; ++it) {
             const unsigned char* st = stages + (unsigned)s * stage_bytes;
@@ -180,40 +186,45 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
             const unsigned dw = reinterpret_cast<const unsigned*>(st + off_desc)[1 + rp];   // rows 2 rp (low half), 2 rp + 1 (high half)
             const unsigned u0 = dw & 0xFFu, m0 = (dw >> 8) & 0xFFu, u1 = (dw >> 16) & 0xFFu, m1 = dw >> 24;
             const unsigned mm = m0 | m1;
-            double s0[9], s1[9];
-            int slot0 = -1, slot1 = -1;
-            bool work = false;
             if (mm != 0u) {
                 const unsigned long long* jinv = reinterpret_cast<const unsigned long long*>(st + gbytes);
-                const int J = reinterpret_cast<const int*>(st + gbytes + GCAP * 8)[u];
-                work = __ballot_sync(FULLMASK, J >= 0) != 0u;
-                if (work) {
-                    const unsigned long long jv = jinv[u];
-                    // w * grad phi_I of the two rows' nodes at the group's points: lane p + 8 rr (zero when the
-                    // point does not hold the row's node)
-                    if (lane < 2 * GB) {
-                        const int p = lane & (GB - 1), rr = lane >> 3;
-                        const unsigned ur = rr ? u1 : u0, mr = rr ? m1 : m0;
-                        double ax = 0.0, ay = 0.0, az = 0.0;
-                        if ((mr >> p) & 1u) {
-                            const unsigned j = (unsigned)(jinv[ur] >> (8 * p)) & 0xFFu;
-                            const double wq = reinterpret_cast<const double*>(st + gbytes + GCAP * 12)[p];
-                            const double* gp = reinterpret_cast<const double*>(st) + (4 * p + 1) * k + j;
-                            ax = wq * gp[0]; ay = wq * gp[k]; az = wq * gp[2 * k];
-                        }
-                        double* dst = aw + p * 6 + rr * 3;
-                        dst[0] = ax; dst[1] = ay; dst[2] = az;
+                const int* un = reinterpret_cast<const int*>(st + gbytes + gcap * 8u);
+                // w * grad phi_I of the two rows' nodes at the group's points: lane p + 8 rr (zero when the
+                // point does not hold the row's node)
+                if (lane < 2 * GB) {
+                    const int p = lane & (GB - 1), rr = lane >> 3;
+                    const unsigned ur = rr ? u1 : u0, mr = rr ? m1 : m0;
+                    double ax = 0.0, ay = 0.0, az = 0.0;
+                    if ((mr >> p) & 1u) {
+                        const unsigned j = (unsigned)(jinv[ur] >> (8 * p)) & 0xFFu;
+                        const double wq = reinterpret_cast<const double*>(st + gbytes + gcap * 12u)[p];
+                        const double* gp = reinterpret_cast<const double*>(st) + (4 * p + 1) * k + j;
+                        ax = wq * gp[0]; ay = wq * gp[k]; az = wq * gp[2 * k];
                     }
-                    __syncwarp();
+                    double* dst = aw + p * 6 + rr * 3;
+                    dst[0] = ax; dst[1] = ay; dst[2] = az;
+                }
+                __syncwarp();
+                // U_g ascends: the upper blocks start in the chunk that holds the rows' own nodes
+                const int Ilow = m0 ? I0 : I1;
+                bool met = false;
+                for (int cc = (int)((m0 ? u0 : u1) >> 5) + w; cc < C; cc += CW) {
+                    const int u = 32 * cc + lane;
+                    const int J = un[u];
+                    if (__ballot_sync(FULLMASK, J >= Ilow) == 0u) break;   // (padding: -1)
+                    const unsigned long long jv = jinv[u];
                     const unsigned jlo = (unsigned)jv, jhi = (unsigned)(jv >> 32);
+                    double s0[9], s1[9];
 #pragma unroll
                     for (int p = 0; p < GB; ++p) {
                         const unsigned jb = ((p < 4 ? jlo : jhi) >> (8 * (p & 3))) & 0xFFu;
-                        // absent (0xFF): the zero area stands in for the three gradient rows
-                        const unsigned char* gq = (jb != 0xFFu) ? st + (unsigned)(4 * p + 1) * k8 + jb * 8u : zeros;
-                        const double gx = *reinterpret_cast<const double*>(gq);
-                        const double gy = *reinterpret_cast<const double*>(gq + k8);
-                        const double gz = *reinterpret_cast<const double*>(gq + 2 * k8);
+                        double gx = 0.0, gy = 0.0, gz = 0.0;   // a union entry the point does not hold (0xFF) contributes zeros
+                        if (jb != 0xFFu) {
+                            const unsigned char* gq = st + (unsigned)(4 * p + 1) * k8 + jb * 8u;
+                            gx = *reinterpret_cast<const double*>(gq);
+                            gy = *reinterpret_cast<const double*>(gq + k8);
+                            gz = *reinterpret_cast<const double*>(gq + 2 * k8);
+                        }
                         const double2 a01 = *reinterpret_cast<const double2*>(aw + p * 6);       // ax0 ay0
                         const double2 a23 = *reinterpret_cast<const double2*>(aw + p * 6 + 2);   // az0 ax1
                         const double2 a45 = *reinterpret_cast<const double2*>(aw + p * 6 + 4);   // ay1 az1
@@ -235,36 +246,28 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
                     }
                     // column slots: the entry (I, U_g[u]) exists iff some point holds both nodes; a pair without
                     // an entry has only zero sums and is skipped
-                    if (J >= 0) {
-                        const unsigned h00 = ((unsigned)J * 2654435761u) >> hshift;
-                        if (m0) {
-                            unsigned h = h00;
-                            while (true) {
-                                const unsigned sl = hash0[h];
-                                if (sl == 0xFFFFu) break;
-                                if (bcol0[sl] == J) { slot0 = (int)sl; break; }
-                                h = (h + 1) & (HSZ - 1);
-                            }
-                        }
-                        if (m1) {
-                            unsigned h = h00;
-                            while (true) {
-                                const unsigned sl = hash1[h];
-                                if (sl == 0xFFFFu) break;
-                                if (bcol1[sl] == J) { slot1 = (int)sl; break; }
-                                h = (h + 1) & (HSZ - 1);
-                            }
+                    int slot0 = -1, slot1 = -1;
+                    const unsigned h00 = ((unsigned)J * 2654435761u) >> hshift;
+                    if (m0 && J >= I0) {
+                        unsigned h = h00;
+                        while (true) {
+                            const unsigned sl = hash0[h];
+                            if (sl == 0xFFFFu) break;
+                            if (bcol0[sl] == J) { slot0 = (int)sl; break; }
+                            h = (h + 1) & (HSZ - 1);
                         }
                     }
-                }
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[s]);   // the stage (and this warp's a-vectors) are no longer read
-            if (++s == nstage) { s = 0; par ^= 1u; }
-            if (mm != 0u) {
-                // read-modify-write phases of consecutive groups are separated for the C warps of the row pair
-                if (C > 1) named_bar(2 + rp, C * 32);
-                if (work) {
+                    if (m1 && J >= I1) {
+                        unsigned h = h00;
+                        while (true) {
+                            const unsigned sl = hash1[h];
+                            if (sl == 0xFFFFu) break;
+                            if (bcol1[sl] == J) { slot1 = (int)sl; break; }
+                            h = (h + 1) & (HSZ - 1);
+                        }
+                    }
+                    // read-modify-write phases of consecutive groups are separated for the CW warps of the row pair
+                    if (CW > 1 && !met) { named_bar(2 + rp, CW * 32); met = true; }
                     if (slot0 >= 0) {
                         double* a = acc0 + slot0 * 9;
 #pragma unroll
@@ -276,28 +279,63 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
                         for (int e = 0; e < 9; ++e) a[e] += s1[e];
                     }
                 }
+                if (CW > 1 && !met) named_bar(2 + rp, CW * 32);
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);   // the stage (and this warp's a-vectors) are no longer read
+            if (++s == nstage) { s = 0; par ^= 1u; }
         }
         named_bar(1, NCT);   // every contribution is in the accumulators
-        // ---- K_IJ = lambda S + mu S^T + mu tr(S) I, three scalar rows of 3 L entries per block row
+        // ---- upper blocks K_IJ = lambda S + mu S^T + mu tr(S) I: per block row three contiguous pieces
         for (int r = 0; r < T; ++r) {
             const int Lr = rowL_s[r];
             if (Lr == 0) continue;
+            const int d = rowd_s[r];
             const double* ar = acc + (size_t)r * 9 * LS;
-            double* dst = A.vals + 9 * rowo_s[r];
-            const int L3 = 3 * Lr;
+            double* dst = A.vals + 9 * rowo_s[r] + 3 * d;
+            const int L3 = 3 * Lr, U3 = 3 * (Lr - d);
 #pragma unroll
             for (int row = 0; row < 3; ++row) {
-                for (int col = tid; col < L3; col += NCT) {
+                for (int col = tid; col < U3; col += NCT) {
                     const int sl = (int)(((unsigned)col * 43691u) >> 17);   // col / 3 for col < 2^15 (columns <= 3 * 1024)
                     const int cc = col - 3 * sl;
                     const double* a = ar + sl * 9;
                     double v = fma(A.lambda, a[3 * row + cc], A.mu * a[3 * cc + row]);
                     if (row == cc) v += A.mu * ((a[0] + a[4]) + a[8]);
-                    __stcs(dst + (size_t)row * L3 + col, v);
+                    dst[(size_t)row * L3 + col] = v;
                 }
             }
         }
+    }
+}
+
+// Lower blocks: K_IJ = K_JI^T for J < I.  One warp per block row; a lane takes a lower slot, finds the slot of I
+// in row J by bisection of that row's ascending column list and copies the transposed block.
+__global__ void __launch_bounds__(256)
+mirror_lower_kernel(int64_t N, const int64_t* __restrict__ brow_ptr, const int32_t* __restrict__ bcol,
+                    const int* __restrict__ bdiag, double* __restrict__ vals) {
+    const int lane = threadIdx.x & 31;
+    const int64_t I = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (I >= N) return;
+    const int64_t o = brow_ptr[I];
+    const int L = (int)(brow_ptr[I + 1] - o);
+    if (L == 0) return;
+    const int d = bdiag[I];
+    for (int s = lane; s < d; s += 32) {
+        const int64_t J = bcol[o + s];
+        const int64_t oj = brow_ptr[J];
+        const int Lj = (int)(brow_ptr[J + 1] - oj);
+        int lo = bdiag[J] + 1, hi = Lj - 1;   // I > J sits right of row J's diagonal
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (bcol[oj + mid] < (int)I) lo = mid + 1; else hi = mid;
+        }
+        const double* src = vals + 9 * oj + 3 * lo;
+        double* dst = vals + 9 * o + 3 * s;
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) dst[(size_t)r * 3 * L + c] = src[(size_t)c * 3 * Lj + r];
     }
 }
 
@@ -321,17 +359,17 @@ load_rows_kernel(int64_t N, int k, const int64_t* __restrict__ inc_ptr, const in
     if (lane == 0) { f[3 * I] = sum * bx; f[3 * I + 1] = sum * by; f[3 * I + 2] = sum * bz; }
 }
 
-template <int C, int RP>
+template <int CW, int RP>
 int launch_panels(rpim_ctx* ctx, PanelArgs& A) {
-    auto kern = reduce_panels_kernel<C, RP>;
+    auto kern = reduce_panels_kernel<CW, RP>;
     const size_t smem = A.L.total;
     CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 1, sms = 148;
-    CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, (RP * C + 1) * 32, smem));
-    if (per_sm < 1) RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "panel reduction does not fit on chip (rows of %d block columns)", ctx->max_blen);
+    CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, (RP * CW + 1) * 32, smem));
+    if (per_sm < 1) RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "panel reduction does not fit on chip (rows of %d upper block columns)", ctx->max_ulen);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
     const int64_t blocks = std::min<int64_t>(A.ntiles, (int64_t)sms * per_sm);
-    kern<<<(unsigned)blocks, (RP * C + 1) * 32, smem, ctx->stream>>>(A);
+    kern<<<(unsigned)blocks, (RP * CW + 1) * 32, smem, ctx->stream>>>(A);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
 }
@@ -342,10 +380,10 @@ int rpim_stage_accumulate_panels(rpim_ctx* ctx, const double* d_qw, double lambd
                                  double* d_vals, double* d_f) {
     PanelArgs A;
     A.N = ctx->N; A.Nq = ctx->Nq; A.ntiles = ctx->ntiles;
-    A.k = ctx->k;
-    A.L = rpim_panel_smem(ctx->tg_C, ctx->tg_T, ctx->k, std::max(ctx->max_blen, 1), ctx->tg_nstage);
+    A.k = ctx->k; A.C = ctx->tg_C;
+    A.L = rpim_panel_smem(ctx->tg_C, ctx->tg_CW, ctx->tg_T, ctx->k, std::max(ctx->max_ulen, 1), ctx->tg_nstage);
     A.hlog = A.L.hlog; A.nstage = ctx->tg_nstage;
-    A.brow_ptr = ctx->d_brow_ptr; A.bcol = ctx->d_bcol; A.stage = ctx->d_stage;
+    A.brow_ptr = ctx->d_brow_ptr; A.bcol = ctx->d_bcol; A.bdiag = ctx->d_bdiag; A.stage = ctx->d_stage;
     A.gmeta = ctx->d_gmeta;
     A.tile_ptr = ctx->d_tile_ptr; A.tdesc = ctx->d_tdesc;
     A.lambda = lambda; A.mu = mu; A.vals = d_vals;
@@ -353,17 +391,21 @@ int rpim_stage_accumulate_panels(rpim_ctx* ctx, const double* d_qw, double lambd
     const unsigned meta = rpim_panel_meta_bytes(ctx->tg_C);
     panel_weights_kernel<<<(unsigned)((G * GB + 255) / 256), 256, 0, ctx->stream>>>(ctx->Nq, G, meta, 32u * ctx->tg_C * 12u, d_qw, ctx->d_gmeta);
     KERNEL_CHECK(ctx);
-    {
-        const int wpb = 8;
-        load_rows_kernel<<<(unsigned)((ctx->N + wpb - 1) / wpb), wpb * 32, 0, ctx->stream>>>(
-            ctx->N, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_stage, d_qw, body[0], body[1], body[2], d_f);
-        KERNEL_CHECK(ctx);
-    }
-    const int C = ctx->tg_C, RP = ctx->tg_T / 2;
-#define RPIM_PANELS_CASE(CC, RR) if (C == CC && RP == RR) return launch_panels<CC, RR>(ctx, A)
+    const int wpb = 8;
+    load_rows_kernel<<<(unsigned)((ctx->N + wpb - 1) / wpb), wpb * 32, 0, ctx->stream>>>(
+        ctx->N, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_stage, d_qw, body[0], body[1], body[2], d_f);
+    KERNEL_CHECK(ctx);
+    const int CW = ctx->tg_CW, RP = ctx->tg_T / 2;
+    int rc = RPIM_ERR_STATE;
+#define RPIM_PANELS_CASE(CC, RR) if (CW == CC && RP == RR) rc = launch_panels<CC, RR>(ctx, A)
+    RPIM_PANELS_CASE(1, 1); RPIM_PANELS_CASE(1, 2); RPIM_PANELS_CASE(1, 3); RPIM_PANELS_CASE(1, 4);
     RPIM_PANELS_CASE(2, 1); RPIM_PANELS_CASE(2, 2); RPIM_PANELS_CASE(2, 3); RPIM_PANELS_CASE(2, 4);
     RPIM_PANELS_CASE(3, 1); RPIM_PANELS_CASE(3, 2); RPIM_PANELS_CASE(3, 3); RPIM_PANELS_CASE(3, 4);
-    RPIM_PANELS_CASE(4, 1); RPIM_PANELS_CASE(4, 2); RPIM_PANELS_CASE(4, 3); RPIM_PANELS_CASE(4, 4);
 #undef RPIM_PANELS_CASE
-    RPIM_FAIL(ctx, RPIM_ERR_STATE, "no panel reduction kernel for C = %d, T = %d", C, ctx->tg_T);
+    if (rc == RPIM_ERR_STATE) RPIM_FAIL(ctx, RPIM_ERR_STATE, "no panel reduction kernel for CW = %d, T = %d", CW, ctx->tg_T);
+    if (rc) return rc;
+    mirror_lower_kernel<<<(unsigned)((ctx->N + wpb - 1) / wpb), wpb * 32, 0, ctx->stream>>>(ctx->N, ctx->d_brow_ptr, ctx->d_bcol,
+                                                                                              ctx->d_bdiag, d_vals);
+    KERNEL_CHECK(ctx);
+    return RPIM_OK;
 }

@@ -211,8 +211,8 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
     const int Ucap = std::max(ctx->max_ulen, 1);
     // consumer warps per row pair; the most rows per tile (8, 6, 4, 2) that leave room for a ring of three
     // stages; then the deepest ring (<= 6)
-    int CW = std::min(2, ctx->tg_C);
-    if (const char* e = getenv("RPIM_PANEL_CW")) { const int c = atoi(e); if (c >= 1 && c <= 3) CW = c; }
+    int CW = std::min(3, ctx->tg_C);
+    if (const char* e = getenv("RPIM_PANEL_CW")) { const int c = atoi(e); if (c >= 1 && c <= 4) CW = c; }
     int T = 0, nstage = 0;
     const unsigned budget = 227u * 1024u;
     if (Ucap <= 1024)

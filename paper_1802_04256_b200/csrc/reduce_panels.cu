@@ -401,6 +401,7 @@ int rpim_stage_accumulate_panels(rpim_ctx* ctx, const double* d_qw, double lambd
     RPIM_PANELS_CASE(1, 1); RPIM_PANELS_CASE(1, 2); RPIM_PANELS_CASE(1, 3); RPIM_PANELS_CASE(1, 4);
     RPIM_PANELS_CASE(2, 1); RPIM_PANELS_CASE(2, 2); RPIM_PANELS_CASE(2, 3); RPIM_PANELS_CASE(2, 4);
     RPIM_PANELS_CASE(3, 1); RPIM_PANELS_CASE(3, 2); RPIM_PANELS_CASE(3, 3); RPIM_PANELS_CASE(3, 4);
+    RPIM_PANELS_CASE(4, 1); RPIM_PANELS_CASE(4, 2); RPIM_PANELS_CASE(4, 3); RPIM_PANELS_CASE(4, 4);
 #undef RPIM_PANELS_CASE
     if (rc == RPIM_ERR_STATE) RPIM_FAIL(ctx, RPIM_ERR_STATE, "no panel reduction kernel for CW = %d, T = %d", CW, ctx->tg_T);
     if (rc) return rc;

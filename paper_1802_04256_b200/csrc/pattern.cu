@@ -147,14 +147,15 @@ __device__ __forceinline__ void table_to_sorted_list(const int* table, int* list
 constexpr int B1W = 320;      // level-1 words per warp: windows of up to 320 * 32 * 32 = 327,680 node ids
 constexpr int B2CAP = 512;    // touched 32-id blocks per row
 constexpr int BM_WARPS = 8;
-constexpr int BM_PER_WARP = B1W + B1W / 2 + B2CAP + B2CAP / 2 + 32;   // 32-bit words of shared memory
+constexpr int BM_GCAP = 256;  // (group, point mask) pairs of a row kept on chip for the group sweeps
+constexpr int BM_PER_WARP = B1W + B1W / 2 + B2CAP + B2CAP / 2 + 32 + 2 * BM_GCAP;   // 32-bit words of shared memory
 
 template <int PSTRIDE>
 __global__ void __launch_bounds__(BM_WARPS * 32)
 brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
                    const int32_t* __restrict__ support, int k, int* __restrict__ blen, int32_t* __restrict__ pool,
                    int* __restrict__ bdiag, int32_t* __restrict__ ovf_rows, unsigned* __restrict__ masks,
-                   long long* __restrict__ flags) {
+                   const unsigned char* __restrict__ gmeta, int gC, long long* __restrict__ flags) {
     constexpr int NWS = PSTRIDE / 32;   // mask words per (row, incident point)
     constexpr int NPASS = PSTRIDE / 256; // passes of 32 lanes over a support (8 k <= PSTRIDE)
     constexpr unsigned FULLW = 0xffffffffu;
@@ -166,6 +167,9 @@ brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t
     unsigned short* p1 = reinterpret_cast<unsigned short*>(l1 + B1W);                 // [B1W] touched blocks before word
     unsigned short* p2 = reinterpret_cast<unsigned short*>(l1 + B1W + B1W / 2);       // [B2CAP] columns before block
     unsigned* mw = l1 + B1W + B1W / 2 + B2CAP / 2;                                    // [32] mask words of one point
+    int* gl = reinterpret_cast<int*>(mw + 32);                                        // [BM_GCAP] groups incident to the row
+    unsigned* gm = reinterpret_cast<unsigned*>(gl + BM_GCAP);                         // [BM_GCAP] their points that hold the row's node
+    const unsigned gcap = 32u * (unsigned)gC, gmeta_bytes = gcap * 12u + RPIM_GROUP_POINTS * 8u;
     for (int64_t I = (int64_t)blockIdx.x * BM_WARPS + wid; I < N; I += (int64_t)gridDim.x * BM_WARPS) {
         const int64_t pa = inc_ptr[I], pb = inc_ptr[I + 1];
         const int np = (int)(pb - pa);
@@ -215,6 +219,68 @@ brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t
             }
         };
         auto nop = [](int) {};
+        // With point groups (groups.cu: the panel reduction's preprocessing) the same union is reached through
+        // the groups' sorted unions U_g: a node J of U_g is a column of the row iff one of the group's points
+        // holds both J and the row's node.  One visit per (row, group) with |U_g| ~ 1.3 k entries instead of
+        // one per (row, point) with k entries.  The (group, point mask) pairs of the row go to shared memory
+        // first (runs of equal q / 8 in the ascending incidence list; a run cut by a 32-entry boundary gives
+        // two pairs, which is harmless for a union).
+        int ngl = -1;   // -1: no group sweep for this row
+        if (gC > 0) {
+            ngl = 0;
+            for (int t0 = 0; t0 < np; t0 += 32) {
+                const int t = t0 + lane;
+                const int q = t < np ? inc_q[pa + t] : -1;
+                const int g = q >= 0 ? q / RPIM_GROUP_POINTS : -1;
+                const unsigned bit = q >= 0 ? 1u << (q % RPIM_GROUP_POINTS) : 0u;
+                const int gp = __shfl_up_sync(FULLW, g, 1);
+                const bool head = q >= 0 && (lane == 0 || g != gp);
+                unsigned m = bit;
+#pragma unroll
+                for (int d = 1; d < RPIM_GROUP_POINTS; ++d) {
+                    const int gd = __shfl_down_sync(FULLW, g, d);
+                    const unsigned bd = __shfl_down_sync(FULLW, bit, d);
+                    if (lane + d < 32 && gd == g) m |= bd;
+                }
+                const unsigned heads = __ballot_sync(FULLW, head);
+                const int pos = ngl + __popc(heads & ((1u << lane) - 1u));
+                if (head && pos < BM_GCAP) { gl[pos] = g; gm[pos] = m; }
+                ngl += __popc(heads);
+            }
+            if (ngl > BM_GCAP) ngl = -1;   // (never with the configs' densities) back to the point sweep
+            __syncwarp();
+        }
+        auto sweep_groups = [&](auto&& body) {
+            // lane u of pass ps holds union entry 32 ps + u of the group: its node and the points that hold it
+            auto fetch = [&](int i, int (&J)[4], unsigned (&pm)[4]) {
+                const unsigned char* rec = gmeta + (int64_t)gl[i] * gmeta_bytes;
+#pragma unroll
+                for (int ps = 0; ps < 4; ++ps) {
+                    J[ps] = -1;
+                    pm[ps] = 0u;
+                    if (ps < gC) {
+                        const int u = 32 * ps + lane;
+                        J[ps] = reinterpret_cast<const int*>(rec + gcap * 8u)[u];
+                        const uint2 jv = reinterpret_cast<const uint2*>(rec)[u];
+                        // bit p = byte p of jinv is not 0xFF
+                        const unsigned a = __vcmpne4(jv.x, 0xFFFFFFFFu) & 0x01010101u, b = __vcmpne4(jv.y, 0xFFFFFFFFu) & 0x01010101u;
+                        pm[ps] = ((a * 0x01020408u) >> 24) | (((b * 0x01020408u) >> 24) << 4);
+                    }
+                }
+            };
+            int J_c[4], J_n[4];
+            unsigned pm_c[4], pm_n[4];
+            fetch(0, J_c, pm_c);
+            for (int i = 0; i < ngl; ++i) {
+                if (i + 1 < ngl) fetch(i + 1, J_n, pm_n);
+                const unsigned m = gm[i];
+#pragma unroll
+                for (int ps = 0; ps < 4; ++ps)
+                    if (J_c[ps] >= 0 && (pm_c[ps] & m)) body(J_c[ps]);
+#pragma unroll
+                for (int ps = 0; ps < 4; ++ps) { J_c[ps] = J_n[ps]; pm_c[ps] = pm_n[ps]; }
+            }
+        };
         // exclusive prefix of a per-lane count over the warp; returns (prefix, total)
         auto warp_excl = [&](int cnt, int& total) {
             int incl = cnt;
@@ -231,10 +297,11 @@ brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t
             for (int w = lane; w < n1; w += 32) l1[w] = 0u;
             __syncwarp();
             // ---- sweep A: touched blocks
-            sweep(nop, [&](int J) {
+            auto markA = [&](int J) {
                 const int b = (J - base) >> 5;
                 atomicOr(&l1[b >> 5], 1u << (b & 31));
-            }, nop);
+            };
+            if (ngl > 0) sweep_groups(markA); else sweep(nop, markA, nop);
             __syncwarp();
             const int C1 = (n1 + 31) >> 5;   // level-1 words per lane: lane owns [lane C1, lane C1 + C1)
             {
@@ -254,11 +321,12 @@ brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t
                 for (int r = lane; r < nb2; r += 32) l2[r] = 0u;
                 __syncwarp();
                 // ---- sweep B: ids inside the touched blocks
-                sweep(nop, [&](int J) {
+                auto markB = [&](int J) {
                     const int d = J - base, b = d >> 5;
                     const int r = p1[b >> 5] + __popc(l1[b >> 5] & ((1u << (b & 31)) - 1u));
                     atomicOr(&l2[r], 1u << (d & 31));
-                }, nop);
+                };
+                if (ngl > 0) sweep_groups(markB); else sweep(nop, markB, nop);
                 __syncwarp();
                 const int C2 = (nb2 + 31) >> 5;
                 {
@@ -488,8 +556,10 @@ int launch_brow_bitmap(rpim_ctx* ctx, int32_t* d_pool, int32_t* d_ovf_rows, unsi
     const size_t smem = (size_t)BM_WARPS * BM_PER_WARP * sizeof(unsigned);
     CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const unsigned nb = (unsigned)std::min<int64_t>((N + BM_WARPS - 1) / BM_WARPS, 148 * 16);
+    // (point groups exist: the sweeps go through their unions; they never coexist with the slot masks)
+    const int gC = (ctx->tg_C > 0 && ctx->d_gmeta && !d_masks) ? ctx->tg_C : 0;
     kern<<<nb, BM_WARPS * 32, smem, ctx->stream>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->k, ctx->d_blen,
-                                                   d_pool, ctx->d_bdiag, d_ovf_rows, d_masks, ctx->d_flags);
+                                                   d_pool, ctx->d_bdiag, d_ovf_rows, d_masks, ctx->d_gmeta, gC, ctx->d_flags);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
 }
@@ -545,7 +615,7 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
             size_t free_b = 0, total_b = 0;
             if (!reuse && ctx->tg_C == 0) CUDA_TRY(ctx, cudaMemGetInfo(&free_b, &total_b));   // a driver call: only when it matters
             if (ctx->tg_C > 0) {
-                // the tiled reduction (reduce_tiles.cu) needs no slot masks
+                // the panel reduction (reduce_panels.cu) needs no slot masks
             } else if (reuse || (uint64_t)bytes <= free_b / 4) {
                 if (ws_alloc(ctx, &ctx->d_masks, words) == RPIM_OK) d_masks = ctx->d_masks;
                 else ctx->err.clear();

@@ -74,9 +74,10 @@ def survey_flops_per_point(k: int) -> float:
     return 70.0 * k * (k + 1) / 2 + 76.0 * k + (2.0 / 3.0) * n ** 3 - n * n / 2.0 + 8.0 * n * n + 51.0 * k * k
 
 
-def flops_per_point(k: int):
+def flops_per_point(k: int, symmetric: bool = False):
     """Algorithmic fp64 flops per quadrature point of THIS implementation,
-    fma = 2.  Returns (shape_flops, reduce_flops)."""
+    fma = 2.  Returns (shape_flops, reduce_flops).  symmetric: the panel reduction accumulates the
+    upper blocks only (k (k + 1) / 2 block pairs per point instead of k^2)."""
     n = k + 4
     pairs = k * (k + 1) // 2
     build = pairs * (7 + 2 * 10 + 3 + 1) + k * (6 + 2 * 10 + 3 + 5)   # t, pow (1+9 fma, 2 mul), t*P; rhs
@@ -88,7 +89,7 @@ def flops_per_point(k: int):
     factor += sum(2 * (j * (j + 1) // 2) + j + 8 * j for j in range(m))      # 1x1 pivots (+ 4 rhs)
     back = 8 * (n * (n - 1) // 2) + 8 * n
     shape = build + factor + back
-    reduce_ = k * k * 18 + k * 3                                              # S += (w g_I) x g_J : 9 fma
+    reduce_ = (k * (k + 1) // 2 if symmetric else k * k) * 18 + k * 3      # S += (w g_I) x g_J : 9 fma per block pair
     return shape, reduce_
 
 
@@ -307,14 +308,15 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
                  "knn": phase_ms[0] / n_pat, "incidence": phase_ms[1] / n_pat, "block_pattern": phase_ms[2] / n_pat}
     kernel_ms = {kk: max_over_ranks(v, world, dev) for kk, v in kernel_ms.items()}
     shape_ms, reduce_ms = kernel_ms["shape_functions"], kernel_ms["reduce_into_csr"]
-    fl_shape, fl_reduce = flops_per_point(w.k)
+    used = {1: "rows", 2: "panels"}.get(ctx.reduction_used(), "?")
+    red_params = ctx.reduction_params()
+    fl_shape, fl_reduce = flops_per_point(w.k, symmetric=(used == "panels"))
     fl_survey = survey_flops_per_point(w.k)
     peak_tflops = N_SM * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
     # SURVEY.md section 8(d) minimum traffic of assemble + penalty: K written once, supports, points, nodes, f
     hbm_min = nnz * 8 + w.Nq * w.k * 4 + w.Nq * 32 + w.N * 24 + 3 * w.N * 8
     staged_reread = 37 * w.Nq * w.k            # this implementation's staged gradients + incidence, read once
     traffic = read_traffic(w.name)
-    used = {1: "rows", 2: "panels"}.get(ctx.reduction_used(), "?")
     reduce_name = "reduce_rows_kernel" if used == "rows" else "reduce_panels_kernel"
     t_red_alu = fl_reduce * w.Nq / (peak_tflops * 1e12) * 1e3          # ms at the FP64 peak
     t_red_hbm = hbm_min / (hbm_gbs * 1e9) * 1e3                        # ms at the HBM peak
@@ -453,6 +455,7 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
 
     out = {
         "w": w, "value": value, "ms_per_step": ms_step, "nnz": nnz, "bits": bits, "reduction": used,
+        "reduction_params": red_params,
         "assemble_penalty": {"value": world * w.Nq / (ms_asm * 1e-3), "unit": UNIT, "ms_per_step": ms_asm,
                              "gdof_entries_per_s": 9.0 * w.k * w.k * w.Nq * world / (ms_asm * 1e-3) / 1e9},
         "clocks": clocks, "e2e": e2e, "launches": int(launches), "roofline": roofline, "solve": solve,
@@ -471,6 +474,7 @@ def config_block(w, world, r):
     return {"workload": f"{w.name} (BASELINE.json configs[{workloads.CONFIG_NAMES.index(w.name)}])",
             "N": w.N, "Nq": w.Nq, "k": w.k, "nnz": r["nnz"], "index_bits": r["bits"],
             "step": "build_pattern + get_pattern + assemble + apply_penalty", "reduction": r["reduction"],
+            "reduction_params": r["reduction_params"],
             "l2": "inputs and outputs larger than L2 (no flush needed)" if r["nnz"] * 8 > 2.5e8 else
                   "working set may fit L2; no flush",
             "parallelism": (f"{world} independent replicas of the workload, one per GPU (own jitter stream, no halo, "

@@ -58,16 +58,25 @@ const char* rpim_last_error(const rpim_ctx* ctx);
 /* Bytes of device workspace currently owned by the context. */
 int64_t rpim_workspace_bytes(const rpim_ctx* ctx);
 
-/* Which kernel reduces the element matrices into the CSR values (step a6; both are deterministic and
- * give results within rounding of each other): 0 = automatic (default; currently the row-owner kernel),
- * 1 = row-owner kernel, 2 = tiled kernel whenever its preprocessing fits (groups of 8 consecutive points
- * whose supports' union has at most 192 nodes; it pays when a background cell carries several Gauss points),
- * 3 = the long-row kernel that rows of more than 1024 block columns take automatically (accumulators in
- * shared memory, binary search of the column; for tests).
+/* Which kernel reduces the element matrices into the CSR values (step a6; all are deterministic and give
+ * results within rounding of each other):
+ *   0 = automatic (default): the panel kernel when the quadrature points come in groups of 8 consecutive
+ *       points that share most of their supports (mean size of a group's union of supports <= 2 k and no
+ *       union above 128 nodes: several Gauss points per background cell), else the row-owner kernel;
+ *   1 = row-owner kernel (accumulators in registers, one lane per column slot);
+ *   2 = panel kernel whenever its preprocessing fits (no union above 128 nodes);
+ *   3 = the long-row kernel that rows of more than 1024 block columns take automatically (accumulators in
+ *       shared memory, binary search of the column; for tests).
+ * The panel kernel accumulates the upper blocks (column node >= row node) and fills the lower ones with the
+ * transposes (K is symmetric block-wise, R8), so its K is bitwise symmetric.
  * Takes effect at the next rpim_build_pattern.  rpim_reduction_used: 1 or 2 for the current pattern
- * (0 before rpim_build_pattern). */
+ * (0 before rpim_build_pattern).  rpim_reduction_params (host array of 8 ints; a report for benchmarks):
+ * [0] kernel as rpim_reduction_used, [1] chunks of 32 entries per group union, [2] block rows per tile,
+ * [3] consumer warps per row pair, [4] ring stages, [5] most upper block columns of a row, [6] longest block
+ * row, [7] 100 x mean size of a group's union of supports (0 when no statistics were taken). */
 int rpim_set_reduction(rpim_ctx* ctx, int mode);
 int rpim_reduction_used(const rpim_ctx* ctx);
+int rpim_reduction_params(const rpim_ctx* ctx, int out[8]);
 
 /* Stage 0 (R1, R2; hot-path steps a1, a2): exact k-nearest-neighbour supports on a
  * uniform cell grid and the CSR pattern of the 3N x 3N stiffness matrix.

@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = (
     "rpim_get_pattern", "rpim_assemble", "rpim_add_point_loads", "rpim_apply_penalty", "rpim_get_shape",
     "rpim_host_pattern", "rpim_host_assemble", "rpim_last_phase_ms", "rpim_phase_totals", "rpim_launch_count",
     "rpim_matvec", "rpim_solve_pcg", "rpim_recover_stress", "rpim_set_reduction", "rpim_reduction_used",
-    "rpim_probe_fp64", "rpim_update_nodes",
+    "rpim_probe_fp64", "rpim_update_nodes", "rpim_reduction_params",
 )
 
 
@@ -71,6 +71,7 @@ def _load():
     lib.rpim_probe_fp64.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]
     lib.rpim_set_reduction.argtypes = [vp, C.c_int]
     lib.rpim_reduction_used.argtypes = [vp]
+    lib.rpim_reduction_params.argtypes = [vp, C.POINTER(C.c_int)]
     _lib = lib
     return lib
 
@@ -151,6 +152,16 @@ def rpim_set_reduction(ctx, mode: int):
 
 def rpim_reduction_used(ctx) -> int:
     return int(_load().rpim_reduction_used(ctx))
+
+
+def rpim_reduction_params(ctx) -> dict:
+    out = (C.c_int * 8)()
+    rc = _load().rpim_reduction_params(ctx, out)
+    if rc != 0:
+        raise RpimError(rc, "rpim_reduction_params failed")
+    keys = ("kernel", "union_chunks", "rows_per_tile", "warps_per_row_pair", "ring_stages", "max_upper_columns",
+            "max_block_row", "mean_union_x100")
+    return dict(zip(keys, [int(v) for v in out]))
 
 
 def rpim_workspace_bytes(ctx) -> int:
@@ -331,6 +342,9 @@ class Context:
 
     def reduction_used(self):
         return rpim_reduction_used(self.ctx)
+
+    def reduction_params(self):
+        return rpim_reduction_params(self.ctx)
 
     def launch_count(self):
         return rpim_launch_count(self.ctx)

@@ -90,12 +90,26 @@ int64_t rpim_launch_count(const rpim_ctx* ctx) { return ctx ? ctx->launches : 0;
 
 int rpim_set_reduction(rpim_ctx* ctx, int mode) {
     if (!ctx) return RPIM_ERR_INVALID_ARG;
-    if (mode < 0 || mode > 3) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "reduction mode must be 0 (auto), 1 (rows), 2 (tiles) or 3 (long rows)");
+    if (mode < 0 || mode > 3) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "reduction mode must be 0 (auto), 1 (rows), 2 (panels) or 3 (long rows)");
     ctx->reduce_mode = mode;
     return RPIM_OK;
 }
 
 int rpim_reduction_used(const rpim_ctx* ctx) { return ctx && ctx->have_pattern ? (ctx->have_tiles ? 2 : 1) : 0; }
+
+int rpim_reduction_params(const rpim_ctx* ctx, int out[8]) {
+    if (!ctx || !out) return RPIM_ERR_INVALID_ARG;
+    const bool t = ctx->have_pattern && ctx->have_tiles;
+    out[0] = rpim_reduction_used(ctx);
+    out[1] = t ? ctx->tg_C : 0;
+    out[2] = t ? ctx->tg_T : 0;
+    out[3] = t ? ctx->tg_CW : 0;
+    out[4] = t ? ctx->tg_nstage : 0;
+    out[5] = t ? ctx->max_ulen : 0;
+    out[6] = ctx->have_pattern ? ctx->max_blen : 0;
+    out[7] = (int)(100.0 * ctx->tg_mean_union + 0.5);
+    return RPIM_OK;
+}
 
 int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const double* d_qpts, int64_t Nq, int k,
                        int index_bits, int64_t* out_nnz, int* out_index_bits) {

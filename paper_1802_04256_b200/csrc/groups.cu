@@ -30,7 +30,7 @@ constexpr int TMAX = 8;         // most block rows per tile
 // One warp per group.  FILL = false: only |U_g| statistics (max, sum).  FILL = true: U_g, gpos, gu_mask.
 template <bool FILL>
 __global__ void __launch_bounds__(GW * 32)
-group_union_kernel(int64_t Nq, int k, int C, const int32_t* __restrict__ support, int* __restrict__ max_len,
+group_union_kernel(int64_t Nq, int k, int C, int64_t gstep, const int32_t* __restrict__ support, int* __restrict__ max_len,
                    unsigned long long* __restrict__ sum_len,
                    uint8_t* __restrict__ gpos, unsigned char* __restrict__ gmeta) {
     __shared__ int buf_s[GW][GSORT];
@@ -42,7 +42,9 @@ group_union_kernel(int64_t Nq, int k, int C, const int32_t* __restrict__ support
     uint8_t* ji = ji_s[wid];
     const int64_t G = (Nq + GB - 1) / GB;
     const int gcap = 32 * C;
-    for (int64_t g = (int64_t)blockIdx.x * GW + wid; g < G; g += (int64_t)gridDim.x * GW) {
+    // gstep > 1: a sample (every gstep-th group), statistics only
+    for (int64_t gs = (int64_t)blockIdx.x * GW + wid; gs * gstep < G; gs += (int64_t)gridDim.x * GW) {
+        const int64_t g = gs * gstep;
         const int64_t q0 = g * GB;
         const int nb = (int)min((int64_t)GB, Nq - q0);
         const int n = nb * k;
@@ -155,6 +157,7 @@ int rpim_stage_groups(rpim_ctx* ctx) {
     cudaStream_t st = ctx->stream;
     ctx->tg_C = 0;
     ctx->have_tiles = false;
+    ctx->tg_mean_union = 0.0;
     if (ctx->reduce_mode == 1 || ctx->reduce_mode == 3) return RPIM_OK;
     const int64_t Nq = ctx->Nq, G = (Nq + GB - 1) / GB;
     const int k = ctx->k;
@@ -162,10 +165,24 @@ int rpim_stage_groups(rpim_ctx* ctx) {
     unsigned long long* d_sum = (unsigned long long*)(ctx->d_scratch + 1);
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_scratch, 0, 2 * sizeof(double), st));
     const unsigned nb = (unsigned)std::min<int64_t>((G + GW - 1) / GW, 148 * 16);
-    group_union_kernel<false><<<nb, GW * 32, 0, st>>>(Nq, k, 0, ctx->d_support, d_max, d_sum, nullptr, nullptr);
-    KERNEL_CHECK(ctx);
     int h_max = 0;
     unsigned long long h_sum = 0;
+    if (ctx->reduce_mode == 0 && G > 16384) {
+        // automatic choice on a large problem: a sample of about 4096 groups first; unions far over the bar
+        // (one point per cell: mean |U_g| ~ 3 k) settle it without the full pass
+        const int64_t gstep = G / 4096, Gs = (G + gstep - 1) / gstep;
+        group_union_kernel<false><<<(unsigned)((Gs + GW - 1) / GW), GW * 32, 0, st>>>(Nq, k, 0, gstep, ctx->d_support, d_max, d_sum,
+                                                                                   nullptr, nullptr);
+        KERNEL_CHECK(ctx);
+        CUDA_TRY(ctx, cudaMemcpyAsync(&h_sum, d_sum, sizeof(h_sum), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(ctx, cudaStreamSynchronize(st));
+        ctx->tg_mean_union = (double)h_sum / (double)Gs;
+        if (ctx->tg_mean_union > 1.25 * RPIM_PANEL_MAX_UNION_RATIO * k) return RPIM_OK;
+        CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_scratch, 0, 2 * sizeof(double), st));
+        h_sum = 0;
+    }
+    group_union_kernel<false><<<nb, GW * 32, 0, st>>>(Nq, k, 0, 1, ctx->d_support, d_max, d_sum, nullptr, nullptr);
+    KERNEL_CHECK(ctx);
     CUDA_TRY(ctx, cudaMemcpyAsync(&h_max, d_max, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaMemcpyAsync(&h_sum, d_sum, sizeof(h_sum), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaStreamSynchronize(st));
@@ -178,7 +195,7 @@ int rpim_stage_groups(rpim_ctx* ctx) {
     int rc;
     if ((rc = ws_alloc(ctx, &ctx->d_gpos, Nq * k))) return rc;
     if ((rc = ws_alloc(ctx, &ctx->d_gmeta, G * (int64_t)rpim_panel_meta_bytes(C)))) return rc;
-    group_union_kernel<true><<<nb, GW * 32, 0, st>>>(Nq, k, C, ctx->d_support, nullptr, nullptr, ctx->d_gpos, ctx->d_gmeta);
+    group_union_kernel<true><<<nb, GW * 32, 0, st>>>(Nq, k, C, 1, ctx->d_support, nullptr, nullptr, ctx->d_gpos, ctx->d_gmeta);
     KERNEL_CHECK(ctx);
     ctx->tg_C = C;
     return RPIM_OK;

@@ -16,7 +16,7 @@
 // requests, not one per point.  Row pair rp (rows 2 rp, 2 rp + 1) has CW consumer warps; the chunks of 32
 // union entries from the one that holds the rows' own nodes upwards (U_g is ascending: everything below
 // is a lower block) are dealt to them round-robin.  In a chunk a lane owns one union entry and sums
-// (w grad phi_I) (x) grad phi_{U_g[u]} over the group's points IN REGISTERS (dense: |U_g| is 1.3 .. 3 k, both
+// (w grad phi_I) (x) grad phi_{U_g[u]} over the group's points IN REGISTERS (dense: |U_g| is 1.3 .. 1.6 k, both
 // rows share the gradient loads), then adds its nine sums per row to the row's accumulator of that column:
 // one table probe and one read-modify-write per (row, group, column) instead of per (row, point, column).
 // The CW warps of a row pair meet at a named barrier between their read-modify-write phases of consecutive

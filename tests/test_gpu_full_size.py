@@ -69,6 +69,7 @@ def test_full_size_every_block_row(name):
     w = workloads.config(name)
     r = run_full_config(w, whole=True, slabs=_cover(w.N, 16 if name == "slope" else 20), want_shape=True)
     assert r["bits"] == (64 if name == "large" else 32)
+    assert r["reduction_used"] == (1 if name == "large" else 2)      # the automatic choice
     _check_common(w, r)
     assert sum(s["hi"] - s["lo"] for s in r["slabs"]) == w.N                         # all rows, once
     assert r["phi_equal"] and r["dphi_equal"] and r["oracle_nsing"] == 0             # a3 + a4 bitwise, all points
@@ -77,11 +78,13 @@ def test_full_size_every_block_row(name):
     assert r["f_untouched"]
 
 
-def test_slope_full_size_tiled_reduction():
-    """The opt-in tiled reduction (rpim_set_reduction(ctx, 2)) at full size: every block row of `slope`."""
+def test_slope_full_size_row_owner_reduction():
+    """`slope` and `stress` take the panel reduction automatically (8 Gauss points per cell), `large` the
+    row-owner kernel; this runs the row-owner kernel (rpim_set_reduction(ctx, 1)) on every block row of `slope`
+    too, so that both kernels are compared at full size on the same matrix."""
     w = workloads.config("slope")
-    r = run_full_config(w, whole=True, slabs=_cover(w.N, 16), want_shape=False, reduction=2)
-    assert r["reduction_used"] == 2
+    r = run_full_config(w, whole=True, slabs=_cover(w.N, 16), want_shape=False, reduction=1)
+    assert r["reduction_used"] == 1
     _check_common(w, r)
     assert sum(s["hi"] - s["lo"] for s in r["slabs"]) == w.N
 

@@ -278,3 +278,23 @@ def test_point_loads_report_singular_load_points():
         pts_ok = torch.tensor([[2.5, 2.5, 5.0]], dtype=torch.float64, device=dev)    # between the planes: regular
         ctx.add_point_loads(pts_ok, one, t, f)                                       # the flags were cleared
         assert abs(float((f - f0).view(-1, 3).sum(0)[2]) + 1.0) < 1e-12
+
+
+@pytest.mark.parametrize("idx", range(4))
+@pytest.mark.parametrize("reduction", [1, 2])
+def test_cuda_K_against_the_plain_definition(idx, reduction):
+    """The CUDA K and f against the DEFINITION (oracle.assemble_dense_ref: plain moment matrix in global
+    coordinates, powl, partial-pivoting LU, literal B and D, long double throughout), not the operation-level
+    recipe both sides transcribe: configs 1 and 2 and jittered k = 40 / k = 60 blocks, both reduction kernels.
+    Bar: the definition-level tolerance of tests/test_oracle_definition.py (about 10x the measured error, under
+    the a-priori bound 2 cond(G) eps of the moment systems)."""
+    from test_oracle_definition import DEF_TOL, definition_K, definition_cases
+    w = definition_cases()[idx]
+    s, rp, ci, vr, fr, km = definition_K(w)
+    g = run_cuda(w, penalty=False, loads=False, reduction=reduction)
+    assert np.array_equal(g["support"], s)
+    assert np.array_equal(g["row_ptr"].astype(np.int64), rp) and np.array_equal(g["col_idx"].astype(np.int64), ci)
+    err = np.abs(g["vals0"] - vr).max() / km
+    ferr = np.abs(g["f0"] - fr).max() / max(np.abs(fr).max(), 1e-300)
+    print(f"{w.name}: k={w.k} reduction={g['reduction_used']} CUDA vs definition: max|dK|/max|K_ii| = {err:.3e}, f {ferr:.3e}")
+    assert err <= DEF_TOL[w.k] and (ferr <= DEF_TOL[w.k] or np.abs(fr).max() == 0.0)

@@ -93,7 +93,8 @@ struct rpim_ctx {
     int tg_C = 0;                    // 32-lane chunks per group union (0: panel path not applicable)
     int tg_T = 0;                    // block rows per tile (even)
     int tg_nstage = 0;               // stages of the group ring
-    int tg_CW = 0;                   // consumer warps per row pair
+    int tg_CW = 0;                   // consumer warps per row group
+    int tg_R = 2;                    // block rows per row group (2: a pair shares the gradient loads; 1: twice the warps)
     int max_ulen = 0;                // most upper block columns (diagonal included) of a row
     double tg_mean_union = 0.0;      // mean |U_g| of the last statistics pass
     int64_t ntiles = 0;
@@ -251,7 +252,7 @@ struct PanelSmem {
 };
 // bytes of a group's record: [jinv: 32 C x 8][union node ids: 32 C ints][weights: 8 doubles]
 inline unsigned rpim_panel_meta_bytes(int C) { return 32u * C * 12u + RPIM_GROUP_POINTS * 8u; }
-inline PanelSmem rpim_panel_smem(int C, int CW, int T, int k, int Ucap, int nstage) {
+inline PanelSmem rpim_panel_smem(int C, int CW, int R, int T, int k, int Ucap, int nstage) {
     PanelSmem L;
     L.LS = (Ucap + 1) & ~1;
     L.hlog = 6;
@@ -262,7 +263,7 @@ inline PanelSmem rpim_panel_smem(int C, int CW, int T, int k, int Ucap, int nsta
     L.off_acc = o; o = up16(o + (unsigned)T * 9u * L.LS * 8u);
     L.off_bcol = o; o = up16(o + (unsigned)T * L.LS * 4u);
     L.off_hash = o; o = up16(o + (unsigned)T * (2u << L.hlog));
-    L.off_aw = o; o = up16(o + (unsigned)(T / 2) * CW * RPIM_GROUP_POINTS * 6u * 8u);
+    L.off_aw = o; o = up16(o + (unsigned)(T / R) * CW * RPIM_GROUP_POINTS * 6u * 8u);
     L.off_stage = o; o = up16(o + (unsigned)nstage * L.stage_bytes);
     L.off_bar = o; o = up16(o + 2u * nstage * 8u);
     L.off_rowo = o; o = up16(o + (unsigned)T * 16u);

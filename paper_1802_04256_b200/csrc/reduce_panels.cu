@@ -63,10 +63,11 @@ __global__ void panel_weights_kernel(int64_t Nq, int64_t G, unsigned meta_bytes,
     reinterpret_cast<double*>(gmeta + (q / GB) * meta_bytes + off_w)[q % GB] = q < Nq ? qw[q] : 0.0;
 }
 
-template <int CW, int RP>
+// R = block rows per consumer warp (2: a row pair shares the gradient loads; 1: twice the warps), RP = row groups
+template <int CW, int RP, int R>
 __global__ void __launch_bounds__((RP * CW + 1) * 32, 1)
 reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
-    constexpr int T = 2 * RP, NCW = RP * CW, NCT = NCW * 32, DW = 1 + RP;
+    constexpr int T = R * RP, NCW = RP * CW, NCT = NCW * 32, DW = 1 + T / 2;
     constexpr int AWS = 6 * GB;   // doubles of one warp's a-vectors: [p][ax0 ay0 az0 ax1 ay1 az1]
     extern __shared__ __align__(16) unsigned char panel_smem[];
     const PanelSmem& L = A.L;
@@ -132,7 +133,7 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
 
     // ---------------------------------------------------------------------- consumer warps
     const int rp = warp / CW, w = warp % CW;
-    const int r0 = 2 * rp, r1 = r0 + 1;
+    const int r0 = R * rp, r1 = r0 + (R - 1);   // (R = 1: the second row is the first; its half of the code is compiled out)
     double* aw = aw_s + warp * AWS;
     double* acc0 = acc + (size_t)r0 * 9 * LS;
     double* acc1 = acc + (size_t)r1 * 9 * LS;
@@ -164,7 +165,7 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
         named_bar(1, NCT);
         // upper column lists (from the diagonal on) and tables: the CW warps of a row pair fill the pair's two rows
 #pragma unroll
-        for (int rr = 0; rr < 2; ++rr) {
+        for (int rr = 0; rr < R; ++rr) {
             const int r = r0 + rr;
             const int64_t o_r = rowo_s[r] + rowd_s[r];
             const int Lu = rowL_s[r] - rowd_s[r];
@@ -183,15 +184,17 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
         for (int it = 0; it < ng; ++it) {
             const unsigned char* st = stages + (unsigned)s * stage_bytes;
             mbar_wait(&full[s], par);
-            const unsigned dw = reinterpret_cast<const unsigned*>(st + off_desc)[1 + rp];   // rows 2 rp (low half), 2 rp + 1 (high half)
-            const unsigned u0 = dw & 0xFFu, m0 = (dw >> 8) & 0xFFu, u1 = (dw >> 16) & 0xFFu, m1 = dw >> 24;
+            // descriptor word 1 + r / 2 holds rows r (low half, r even) and r + 1 (high half)
+            unsigned dw = reinterpret_cast<const unsigned*>(st + off_desc)[1 + (r0 >> 1)];
+            if (R == 1 && (r0 & 1)) dw >>= 16;
+            const unsigned u0 = dw & 0xFFu, m0 = (dw >> 8) & 0xFFu, u1 = (R == 2) ? (dw >> 16) & 0xFFu : 0u, m1 = (R == 2) ? dw >> 24 : 0u;
             const unsigned mm = m0 | m1;
             if (mm != 0u) {
                 const unsigned long long* jinv = reinterpret_cast<const unsigned long long*>(st + gbytes);
                 const int* un = reinterpret_cast<const int*>(st + gbytes + gcap * 8u);
                 // w * grad phi_I of the two rows' nodes at the group's points: lane p + 8 rr (zero when the
                 // point does not hold the row's node)
-                if (lane < 2 * GB) {
+                if (lane < R * GB) {
                     const int p = lane & (GB - 1), rr = lane >> 3;
                     const unsigned ur = rr ? u1 : u0, mr = rr ? m1 : m0;
                     double ax = 0.0, ay = 0.0, az = 0.0;
@@ -227,21 +230,26 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
                         }
                         const double2 a01 = *reinterpret_cast<const double2*>(aw + p * 6);       // ax0 ay0
                         const double2 a23 = *reinterpret_cast<const double2*>(aw + p * 6 + 2);   // az0 ax1
-                        const double2 a45 = *reinterpret_cast<const double2*>(aw + p * 6 + 4);   // ay1 az1
+                        double2 a45 = make_double2(0.0, 0.0);
+                        if constexpr (R == 2) a45 = *reinterpret_cast<const double2*>(aw + p * 6 + 4);   // ay1 az1
                         if (p == 0) {
                             s0[0] = a01.x * gx; s0[1] = a01.x * gy; s0[2] = a01.x * gz;
                             s0[3] = a01.y * gx; s0[4] = a01.y * gy; s0[5] = a01.y * gz;
                             s0[6] = a23.x * gx; s0[7] = a23.x * gy; s0[8] = a23.x * gz;
-                            s1[0] = a23.y * gx; s1[1] = a23.y * gy; s1[2] = a23.y * gz;
-                            s1[3] = a45.x * gx; s1[4] = a45.x * gy; s1[5] = a45.x * gz;
-                            s1[6] = a45.y * gx; s1[7] = a45.y * gy; s1[8] = a45.y * gz;
+                            if constexpr (R == 2) {
+                                s1[0] = a23.y * gx; s1[1] = a23.y * gy; s1[2] = a23.y * gz;
+                                s1[3] = a45.x * gx; s1[4] = a45.x * gy; s1[5] = a45.x * gz;
+                                s1[6] = a45.y * gx; s1[7] = a45.y * gy; s1[8] = a45.y * gz;
+                            }
                         } else {
                             s0[0] = fma(a01.x, gx, s0[0]); s0[1] = fma(a01.x, gy, s0[1]); s0[2] = fma(a01.x, gz, s0[2]);
                             s0[3] = fma(a01.y, gx, s0[3]); s0[4] = fma(a01.y, gy, s0[4]); s0[5] = fma(a01.y, gz, s0[5]);
                             s0[6] = fma(a23.x, gx, s0[6]); s0[7] = fma(a23.x, gy, s0[7]); s0[8] = fma(a23.x, gz, s0[8]);
-                            s1[0] = fma(a23.y, gx, s1[0]); s1[1] = fma(a23.y, gy, s1[1]); s1[2] = fma(a23.y, gz, s1[2]);
-                            s1[3] = fma(a45.x, gx, s1[3]); s1[4] = fma(a45.x, gy, s1[4]); s1[5] = fma(a45.x, gz, s1[5]);
-                            s1[6] = fma(a45.y, gx, s1[6]); s1[7] = fma(a45.y, gy, s1[7]); s1[8] = fma(a45.y, gz, s1[8]);
+                            if constexpr (R == 2) {
+                                s1[0] = fma(a23.y, gx, s1[0]); s1[1] = fma(a23.y, gy, s1[1]); s1[2] = fma(a23.y, gz, s1[2]);
+                                s1[3] = fma(a45.x, gx, s1[3]); s1[4] = fma(a45.x, gy, s1[4]); s1[5] = fma(a45.x, gz, s1[5]);
+                                s1[6] = fma(a45.y, gx, s1[6]); s1[7] = fma(a45.y, gy, s1[7]); s1[8] = fma(a45.y, gz, s1[8]);
+                            }
                         }
                     }
                     // column slots: the entry (I, U_g[u]) exists iff some point holds both nodes; a pair without
@@ -257,7 +265,7 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
                             h = (h + 1) & (HSZ - 1);
                         }
                     }
-                    if (m1 && J >= I1) {
+                    if (R == 2 && m1 && J >= I1) {
                         unsigned h = h00;
                         while (true) {
                             const unsigned sl = hash1[h];
@@ -273,7 +281,7 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
 #pragma unroll
                         for (int e = 0; e < 9; ++e) a[e] += s0[e];
                     }
-                    if (slot1 >= 0) {
+                    if (R == 2 && slot1 >= 0) {
                         double* a = acc1 + slot1 * 9;
 #pragma unroll
                         for (int e = 0; e < 9; ++e) a[e] += s1[e];
@@ -302,7 +310,7 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
                     const double* a = ar + sl * 9;
                     double v = fma(A.lambda, a[3 * row + cc], A.mu * a[3 * cc + row]);
                     if (row == cc) v += A.mu * ((a[0] + a[4]) + a[8]);
-                    dst[(size_t)row * L3 + col] = v;
+                    __stcs(dst + (size_t)row * L3 + col, v);   // streaming: K is not read again by this kernel, the groups' staged rows are
                 }
             }
         }
@@ -359,9 +367,9 @@ load_rows_kernel(int64_t N, int k, const int64_t* __restrict__ inc_ptr, const in
     if (lane == 0) { f[3 * I] = sum * bx; f[3 * I + 1] = sum * by; f[3 * I + 2] = sum * bz; }
 }
 
-template <int CW, int RP>
+template <int CW, int RP, int R>
 int launch_panels(rpim_ctx* ctx, PanelArgs& A) {
-    auto kern = reduce_panels_kernel<CW, RP>;
+    auto kern = reduce_panels_kernel<CW, RP, R>;
     const size_t smem = A.L.total;
     CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 1, sms = 148;
@@ -381,7 +389,7 @@ int rpim_stage_accumulate_panels(rpim_ctx* ctx, const double* d_qw, double lambd
     PanelArgs A;
     A.N = ctx->N; A.Nq = ctx->Nq; A.ntiles = ctx->ntiles;
     A.k = ctx->k; A.C = ctx->tg_C;
-    A.L = rpim_panel_smem(ctx->tg_C, ctx->tg_CW, ctx->tg_T, ctx->k, std::max(ctx->max_ulen, 1), ctx->tg_nstage);
+    A.L = rpim_panel_smem(ctx->tg_C, ctx->tg_CW, ctx->tg_R, ctx->tg_T, ctx->k, std::max(ctx->max_ulen, 1), ctx->tg_nstage);
     A.hlog = A.L.hlog; A.nstage = ctx->tg_nstage;
     A.brow_ptr = ctx->d_brow_ptr; A.bcol = ctx->d_bcol; A.bdiag = ctx->d_bdiag; A.stage = ctx->d_stage;
     A.gmeta = ctx->d_gmeta;
@@ -395,15 +403,20 @@ int rpim_stage_accumulate_panels(rpim_ctx* ctx, const double* d_qw, double lambd
     load_rows_kernel<<<(unsigned)((ctx->N + wpb - 1) / wpb), wpb * 32, 0, ctx->stream>>>(
         ctx->N, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_stage, d_qw, body[0], body[1], body[2], d_f);
     KERNEL_CHECK(ctx);
-    const int CW = ctx->tg_CW, RP = ctx->tg_T / 2;
+    const int CW = ctx->tg_CW, R = ctx->tg_R, RP = ctx->tg_T / R;
     int rc = RPIM_ERR_STATE;
-#define RPIM_PANELS_CASE(CC, RR) if (CW == CC && RP == RR) rc = launch_panels<CC, RR>(ctx, A)
+#define RPIM_PANELS_CASE(CC, RR) if (R == 2 && CW == CC && RP == RR) rc = launch_panels<CC, RR, 2>(ctx, A)
     RPIM_PANELS_CASE(1, 1); RPIM_PANELS_CASE(1, 2); RPIM_PANELS_CASE(1, 3); RPIM_PANELS_CASE(1, 4);
     RPIM_PANELS_CASE(2, 1); RPIM_PANELS_CASE(2, 2); RPIM_PANELS_CASE(2, 3); RPIM_PANELS_CASE(2, 4);
     RPIM_PANELS_CASE(3, 1); RPIM_PANELS_CASE(3, 2); RPIM_PANELS_CASE(3, 3); RPIM_PANELS_CASE(3, 4);
     RPIM_PANELS_CASE(4, 1); RPIM_PANELS_CASE(4, 2); RPIM_PANELS_CASE(4, 3); RPIM_PANELS_CASE(4, 4);
 #undef RPIM_PANELS_CASE
-    if (rc == RPIM_ERR_STATE) RPIM_FAIL(ctx, RPIM_ERR_STATE, "no panel reduction kernel for CW = %d, T = %d", CW, ctx->tg_T);
+#define RPIM_PANELS_CASE1(CC, RR) if (R == 1 && CW == CC && RP == RR) rc = launch_panels<CC, RR, 1>(ctx, A)
+    RPIM_PANELS_CASE1(1, 2); RPIM_PANELS_CASE1(1, 4); RPIM_PANELS_CASE1(1, 6); RPIM_PANELS_CASE1(1, 8);
+    RPIM_PANELS_CASE1(2, 2); RPIM_PANELS_CASE1(2, 4); RPIM_PANELS_CASE1(2, 6); RPIM_PANELS_CASE1(2, 8);
+    RPIM_PANELS_CASE1(3, 2); RPIM_PANELS_CASE1(3, 4); RPIM_PANELS_CASE1(3, 6); RPIM_PANELS_CASE1(3, 8);
+#undef RPIM_PANELS_CASE1
+    if (rc == RPIM_ERR_STATE) RPIM_FAIL(ctx, RPIM_ERR_STATE, "no panel reduction kernel for CW = %d, R = %d, T = %d", CW, R, ctx->tg_T);
     if (rc) return rc;
     mirror_lower_kernel<<<(unsigned)((ctx->N + wpb - 1) / wpb), wpb * 32, 0, ctx->stream>>>(ctx->N, ctx->d_brow_ptr, ctx->d_bcol,
                                                                                               ctx->d_bdiag, d_vals);

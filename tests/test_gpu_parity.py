@@ -298,3 +298,24 @@ def test_cuda_K_against_the_plain_definition(idx, reduction):
     ferr = np.abs(g["f0"] - fr).max() / max(np.abs(fr).max(), 1e-300)
     print(f"{w.name}: k={w.k} reduction={g['reduction_used']} CUDA vs definition: max|dK|/max|K_ii| = {err:.3e}, f {ferr:.3e}")
     assert err <= DEF_TOL[w.k] and (ferr <= DEF_TOL[w.k] or np.abs(fr).max() == 0.0)
+
+
+@pytest.mark.parametrize("env", [
+    {"RPIM_PANEL_R": "2", "RPIM_PANEL_CW": "3"},                        # row pairs sharing the gradient loads
+    {"RPIM_PANEL_R": "2", "RPIM_PANEL_CW": "1", "RPIM_PANEL_T": "2"},   # one warp takes all chunks of its pair
+    {"RPIM_PANEL_R": "1", "RPIM_PANEL_CW": "1", "RPIM_PANEL_NSTAGE": "2"},
+    {"RPIM_PANEL_R": "1", "RPIM_PANEL_CW": "3", "RPIM_PANEL_T": "4"},
+])
+def test_panel_reduction_launch_shapes(env, monkeypatch):
+    """The other launch shapes of reduce_panels_kernel (rows per warp group, warps per group, rows per tile, ring
+    depth; rpim_build_pattern reads the RPIM_PANEL_* overrides): same bars, and bitwise the same K as the default
+    shape (the order of summation per entry does not depend on the launch shape)."""
+    w = workloads.make_block("shape60", 10, 9, 8, 1.0, 2, 60, 5e9, 0.3, jitter=0.3, seed=360,
+                             body=(10.0, -20.0, -2.5e4), bc="bottom+roller")
+    g0, o = run_cuda(w, reduction=2), run_oracle(w)
+    for kk, v in env.items():
+        monkeypatch.setenv(kk, v)
+    g = run_cuda(w, reduction=2)
+    assert g["reduction_used"] == 2
+    _compare(w, g, o)
+    assert np.array_equal(g["vals"], g0["vals"]) and np.array_equal(g["f"], g0["f"])

@@ -70,13 +70,14 @@ int64_t rpim_workspace_bytes(const rpim_ctx* ctx);
  * The panel kernel accumulates the upper blocks (column node >= row node) and fills the lower ones with the
  * transposes (K is symmetric block-wise, R8), so its K is bitwise symmetric.
  * Takes effect at the next rpim_build_pattern.  rpim_reduction_used: 1 or 2 for the current pattern
- * (0 before rpim_build_pattern).  rpim_reduction_params (host array of 8 ints; a report for benchmarks):
+ * (0 before rpim_build_pattern).  rpim_reduction_params (host array of 10 ints; a report for benchmarks):
  * [0] kernel as rpim_reduction_used, [1] chunks of 32 entries per group union, [2] block rows per tile,
- * [3] consumer warps per row pair, [4] ring stages, [5] most upper block columns of a row, [6] longest block
- * row, [7] 100 x mean size of a group's union of supports (0 when no statistics were taken). */
+ * [3] consumer warps per row group, [4] ring stages, [5] most upper block columns of a row, [6] longest block
+ * row, [7] 100 x mean size of a group's union of supports (0 when no statistics were taken), [8] block rows per
+ * consumer warp group, [9] 1 when the groups' staged rows travel as a 2-D tensor copy of the gradient rows only. */
 int rpim_set_reduction(rpim_ctx* ctx, int mode);
 int rpim_reduction_used(const rpim_ctx* ctx);
-int rpim_reduction_params(const rpim_ctx* ctx, int out[8]);
+int rpim_reduction_params(const rpim_ctx* ctx, int out[10]);
 
 /* Stage 0 (R1, R2; hot-path steps a1, a2): exact k-nearest-neighbour supports on a
  * uniform cell grid and the CSR pattern of the 3N x 3N stiffness matrix.

@@ -155,12 +155,12 @@ def rpim_reduction_used(ctx) -> int:
 
 
 def rpim_reduction_params(ctx) -> dict:
-    out = (C.c_int * 8)()
+    out = (C.c_int * 10)()
     rc = _load().rpim_reduction_params(ctx, out)
     if rc != 0:
         raise RpimError(rc, "rpim_reduction_params failed")
-    keys = ("kernel", "union_chunks", "rows_per_tile", "warps_per_row_pair", "ring_stages", "max_upper_columns",
-            "max_block_row", "mean_union_x100")
+    keys = ("kernel", "union_chunks", "rows_per_tile", "warps_per_row_group", "ring_stages", "max_upper_columns",
+            "max_block_row", "mean_union_x100", "rows_per_warp_group", "tensor_copy_staging")
     return dict(zip(keys, [int(v) for v in out]))
 
 

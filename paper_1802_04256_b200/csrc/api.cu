@@ -97,7 +97,7 @@ int rpim_set_reduction(rpim_ctx* ctx, int mode) {
 
 int rpim_reduction_used(const rpim_ctx* ctx) { return ctx && ctx->have_pattern ? (ctx->have_tiles ? 2 : 1) : 0; }
 
-int rpim_reduction_params(const rpim_ctx* ctx, int out[8]) {
+int rpim_reduction_params(const rpim_ctx* ctx, int out[10]) {
     if (!ctx || !out) return RPIM_ERR_INVALID_ARG;
     const bool t = ctx->have_pattern && ctx->have_tiles;
     out[0] = rpim_reduction_used(ctx);
@@ -108,6 +108,8 @@ int rpim_reduction_params(const rpim_ctx* ctx, int out[8]) {
     out[5] = t ? ctx->max_ulen : 0;
     out[6] = ctx->have_pattern ? ctx->max_blen : 0;
     out[7] = (int)(100.0 * ctx->tg_mean_union + 0.5);
+    out[8] = t ? ctx->tg_R : 0;
+    out[9] = t && ctx->tg_grad_only ? 1 : 0;
     return RPIM_OK;
 }
 

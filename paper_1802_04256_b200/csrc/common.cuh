@@ -94,6 +94,7 @@ struct rpim_ctx {
     int tg_T = 0;                    // block rows per tile (even)
     int tg_nstage = 0;               // stages of the group ring
     int tg_CW = 0;                   // consumer warps per row group
+    bool tg_grad_only = false;       // the groups' staged rows travel as a 2-D tensor copy of the gradient rows only
     int tg_R = 2;                    // block rows per row group (2: a pair shares the gradient loads; 1: twice the warps)
     int max_ulen = 0;                // most upper block columns (diagonal included) of a row
     double tg_mean_union = 0.0;      // mean |U_g| of the last statistics pass
@@ -252,19 +253,23 @@ struct PanelSmem {
 };
 // bytes of a group's record: [jinv: 32 C x 8][union node ids: 32 C ints][weights: 8 doubles]
 inline unsigned rpim_panel_meta_bytes(int C) { return 32u * C * 12u + RPIM_GROUP_POINTS * 8u; }
-inline PanelSmem rpim_panel_smem(int C, int CW, int R, int T, int k, int Ucap, int nstage) {
+// the group's staged rows travel as a 2-D tensor copy of the three gradient rows per point when their 24 k bytes
+// are a 16-byte multiple and fit a copy box (else as one plain bulk copy of the whole rows, phi included)
+inline bool rpim_panel_grad_only(int k) { return (k & 1) == 0 && 3 * k <= 256; }
+inline PanelSmem rpim_panel_smem(int C, int CW, int R, int T, int k, int Ucap, int nstage, bool grad_only) {
     PanelSmem L;
     L.LS = (Ucap + 1) & ~1;
     L.hlog = 6;
     while ((1 << L.hlog) < 2 * Ucap) ++L.hlog;
-    L.stage_bytes = (unsigned)(RPIM_GROUP_POINTS * 4 * k * 8) + rpim_panel_meta_bytes(C) + 32u;
     auto up16 = [](unsigned v) { return (v + 15u) & ~15u; };
+    auto up128 = [](unsigned v) { return (v + 127u) & ~127u; };
+    L.stage_bytes = up128((unsigned)(RPIM_GROUP_POINTS * (grad_only ? 3 : 4) * k * 8) + rpim_panel_meta_bytes(C) + 32u);
     unsigned o = 0;
     L.off_acc = o; o = up16(o + (unsigned)T * 9u * L.LS * 8u);
     L.off_bcol = o; o = up16(o + (unsigned)T * L.LS * 4u);
     L.off_hash = o; o = up16(o + (unsigned)T * (2u << L.hlog));
     L.off_aw = o; o = up16(o + (unsigned)(T / R) * CW * RPIM_GROUP_POINTS * 6u * 8u);
-    L.off_stage = o; o = up16(o + (unsigned)nstage * L.stage_bytes);
+    L.off_stage = up128(o); o = up16(L.off_stage + (unsigned)nstage * L.stage_bytes);
     L.off_bar = o; o = up16(o + 2u * nstage * 8u);
     L.off_rowo = o; o = up16(o + (unsigned)T * 16u);
     L.total = o;

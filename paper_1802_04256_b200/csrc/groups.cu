@@ -228,23 +228,45 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
     const int Ucap = std::max(ctx->max_ulen, 1);
     // Launch shape of reduce_panels_kernel.  Measured on B200: one block row per consumer
     // warp group and two warps per group (13 warps at T = 6) beat row pairs with three warps (10 warps) by 7 % at
-    // `stress`; the most rows per tile (8, 6, 4, 2) that leave room for a ring of three stages, then the deepest
-    // ring (<= 6).  RPIM_PANEL_R / _CW / _T / _NSTAGE override (tuning and tests).
+    // `stress`; the most rows per tile (8, 6, 4, 2) that leave room for a ring of five stages (else four, three),
+    // then the deepest ring (<= 6).  RPIM_PANEL_R / _CW / _T / _NSTAGE override (tuning and tests).
     int CW = 2;
     if (const char* e = getenv("RPIM_PANEL_CW")) { const int c = atoi(e); if (c >= 1 && c <= 4) CW = c; }
     int R = 1;
     if (const char* e = getenv("RPIM_PANEL_R")) { const int r = atoi(e); if (r == 1 || r == 2) R = r; }
     if (R == 1 && CW > 3) CW = 3;
-    int T = 0, nstage = 0;
     const unsigned budget = 227u * 1024u;
-    if (Ucap <= 1024)
-        for (int t = TMAX; t >= 2 && T == 0; t -= 2)
-            if (rpim_panel_smem(ctx->tg_C, CW, R, t, ctx->k, Ucap, 3).total <= budget) T = t;
-    if (const char* e = getenv("RPIM_PANEL_T")) { const int t = atoi(e); if (t >= 2 && t <= TMAX && !(t & 1)) T = t; }
+    // rows per tile and ring depth for one way of staging the groups' rows
+    auto choose = [&](bool grad_only, int& T, int& nstage) {
+        T = 0;
+        nstage = 0;
+        // (a deep ring decouples the consumer warps: at `stress` 6 rows with 6 stages beat 8 rows with 3 by 36 %)
+        if (Ucap <= 1024)
+            for (int need = 5; need >= 3 && T == 0; --need)
+                for (int t = TMAX; t >= 2 && T == 0; t -= 2)
+                    if (rpim_panel_smem(ctx->tg_C, CW, R, t, ctx->k, Ucap, need, grad_only).total <= budget) T = t;
+        if (const char* e = getenv("RPIM_PANEL_T")) { const int t = atoi(e); if (t >= 2 && t <= TMAX && !(t & 1)) T = t; }
+        if (T == 0) return;
+        for (nstage = 6; nstage > 2 && rpim_panel_smem(ctx->tg_C, CW, R, T, ctx->k, Ucap, nstage, grad_only).total > budget; --nstage) {}
+        if (const char* e = getenv("RPIM_PANEL_NSTAGE")) { const int n = atoi(e); if (n >= 2 && n <= 8) nstage = n; }
+        if (rpim_panel_smem(ctx->tg_C, CW, R, T, ctx->k, Ucap, nstage, grad_only).total > budget) T = 0;
+    };
+    // Whole staged rows by one plain bulk copy, or the gradient rows only by a 2-D tensor copy (three quarters of
+    // the bytes, but eight row transfers inside the request: slower at `slope`, where the plain ring is already
+    // six deep).  The tensor copy is taken when it buys rows per tile or ring depth.
+    int T = 0, nstage = 0;
+    bool grad_only = false;
+    choose(false, T, nstage);
+    if (rpim_panel_grad_only(ctx->k)) {
+        int Tg = 0, ng = 0;
+        choose(true, Tg, ng);
+        if (Tg > T || (Tg == T && ng > nstage)) { T = Tg; nstage = ng; grad_only = true; }
+    }
+    if (const char* e = getenv("RPIM_PANEL_GRAD_ONLY")) {
+        const bool want = atoi(e) != 0;
+        if (want != grad_only && (!want || rpim_panel_grad_only(ctx->k))) { grad_only = want; choose(grad_only, T, nstage); }
+    }
     if (T == 0) { ctx->tg_C = 0; return RPIM_OK; }   // rows too long to keep two of them on chip
-    for (nstage = 6; nstage > 2 && rpim_panel_smem(ctx->tg_C, CW, R, T, ctx->k, Ucap, nstage).total > budget; --nstage) {}
-    if (const char* e = getenv("RPIM_PANEL_NSTAGE")) { const int n = atoi(e); if (n >= 2 && n <= 8) nstage = n; }
-    if (rpim_panel_smem(ctx->tg_C, CW, R, T, ctx->k, Ucap, nstage).total > budget) { ctx->tg_C = 0; return RPIM_OK; }
     const int64_t ntiles = (N + T - 1) / T;
     const int DW = 1 + T / 2;
     int rc;
@@ -269,6 +291,7 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
     ctx->tg_T = T;
     ctx->tg_CW = CW;
     ctx->tg_R = R;
+    ctx->tg_grad_only = grad_only;
     ctx->tg_nstage = nstage;
     ctx->ntiles = ntiles;
     ctx->have_tiles = true;

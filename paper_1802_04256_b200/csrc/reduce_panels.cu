@@ -10,8 +10,9 @@
 // The accumulators S_IJ of their upper blocks (nine doubles per block column) live in SHARED memory, next to
 // each row's upper column list and a 16-bit open-addressing table column node -> slot.  The point groups
 // incident to the tile arrive through a ring of NSTAGE shared-memory stages filled by a PRODUCER warp with
-// bulk copies (cp.async.bulk + mbarrier): ONE copy of the staged rows of the group's eight consecutive
-// points and ONE of the group's record (its sorted union of supports U_g, the map (union entry, point) ->
+// TWO copies (cp.async.bulk + mbarrier): a 2-D tensor copy (TMA) of the gradient rows of the group's eight
+// consecutive points (a plain bulk copy of their whole staged rows when 24 k bytes is no 16-byte multiple)
+// and ONE plain bulk copy of the group's record (its sorted union of supports U_g, the map (union entry, point) ->
 // support position, the quadrature weights): the bulk-copy engine has a per-request cost, so few large
 // requests, not one per point.  Row pair rp (rows 2 rp, 2 rp + 1) has CW consumer warps; the chunks of 32
 // union entries from the one that holds the rows' own nodes upwards (U_g is ascending: everything below
@@ -25,6 +26,8 @@
 // ascending) by one lane: no floating-point atomics, bitwise run-to-run reproducible; every entry of K is
 // written once, with the isotropic closed form K_IJ = lambda S + mu S^T + mu tr(S) I applied at write-out.
 // The body-force load f_I = b sum_q w phi_I(q) is a separate row-owner pass over the incidence lists.
+#include <cuda.h>
+
 #include "bulk_copy.cuh"
 #include "common.cuh"
 
@@ -35,6 +38,12 @@ constexpr unsigned FULLMASK = 0xffffffffu;
 
 __device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// predicated shared-memory load: 0.0 when `on` is false (no branch, no access)
+__device__ __forceinline__ double lds_f64_if(unsigned addr, bool on) {
+    double v = 0.0;
+    asm("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %2, 0;\n\t@q ld.shared.f64 %0, [%1];\n\t}" : "+d"(v) : "r"(addr), "r"((int)on));
+    return v;
 }
 __device__ __forceinline__ void named_bar(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -53,7 +62,15 @@ struct PanelArgs {
     double lambda, mu;
     double* vals;
     PanelSmem L;
+    int grad_only;               // 1: the staged rows travel through `tmap` (gradient rows only), 0: plain bulk copy of whole rows
+    alignas(64) CUtensorMap tmap;   // staged array as [point][4 k] doubles, box = 8 points x 3 k doubles
 };
+
+// 2-D tensor copy (TMA) global -> shared, completion on an mbarrier
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(smem_u32(dst)), "l"(reinterpret_cast<unsigned long long>(map)), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
+}
 
 // quadrature weights of every group into the group's record (once per rpim_assemble: the weights are its input)
 __global__ void panel_weights_kernel(int64_t Nq, int64_t G, unsigned meta_bytes, unsigned off_w, const double* __restrict__ qw,
@@ -69,7 +86,7 @@ __global__ void __launch_bounds__((RP * CW + 1) * 32, 1)
 reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
     constexpr int T = R * RP, NCW = RP * CW, NCT = NCW * 32, DW = 1 + T / 2;
     constexpr int AWS = 6 * GB;   // doubles of one warp's a-vectors: [p][ax0 ay0 az0 ax1 ay1 az1]
-    extern __shared__ __align__(16) unsigned char panel_smem[];
+    extern __shared__ __align__(128) unsigned char panel_smem[];
     const PanelSmem& L = A.L;
     double* acc = reinterpret_cast<double*>(panel_smem + L.off_acc);                    // [T][LS][9]
     int* bcol_s = reinterpret_cast<int*>(panel_smem + L.off_bcol);                      // [T][LS]
@@ -86,7 +103,9 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
     const int k = A.k, C = A.C, LS = L.LS, HSZ = 1 << A.hlog, hshift = 32 - A.hlog, nstage = A.nstage;
     // stage: [the group's staged rows: GB x 4 x k doubles][group record: jinv, union ids, weights][desc: 8 words]
     const unsigned gcap = 32u * C, meta = gcap * 12u + GB * 8u;
-    const unsigned gbytes = (unsigned)(GB * 4 * k * 8), off_desc = gbytes + meta, stage_bytes = L.stage_bytes;
+    const unsigned prow8 = (unsigned)(A.grad_only ? 3 : 4) * (unsigned)k * 8u;   // bytes of a point's rows inside a stage
+    const unsigned goff8 = A.grad_only ? 0u : (unsigned)k * 8u;                    // its d/dx row starts here
+    const unsigned gbytes = GB * prow8, off_desc = gbytes + meta, stage_bytes = L.stage_bytes;
     const unsigned k8 = (unsigned)k * 8u;
 
     if (tid == 0) {
@@ -121,7 +140,8 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
                     __syncwarp();
                     if (lane == 0) {
                         mbar_expect_tx(&full[s], gbytes + meta);
-                        bulk_g2s(st, A.stage + g * (GB * 4) * k, gbytes, &full[s]);
+                        if (A.grad_only) tma_load_2d(st, &A.tmap, k, (int)(g * GB), &full[s]);
+                        else bulk_g2s(st, A.stage + g * (GB * 4) * k, gbytes, &full[s]);
                         bulk_g2s(st + gbytes, A.gmeta + g * meta, meta, &full[s]);
                     }
                     if (++s == nstage) { s = 0; par ^= 1u; }
@@ -201,7 +221,7 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
                     if ((mr >> p) & 1u) {
                         const unsigned j = (unsigned)(jinv[ur] >> (8 * p)) & 0xFFu;
                         const double wq = reinterpret_cast<const double*>(st + gbytes + gcap * 12u)[p];
-                        const double* gp = reinterpret_cast<const double*>(st) + (4 * p + 1) * k + j;
+                        const double* gp = reinterpret_cast<const double*>(st + (unsigned)p * prow8 + goff8) + j;
                         ax = wq * gp[0]; ay = wq * gp[k]; az = wq * gp[2 * k];
                     }
                     double* dst = aw + p * 6 + rr * 3;
@@ -217,17 +237,15 @@ reduce_panels_kernel(const __grid_constant__ PanelArgs A) {
                     if (__ballot_sync(FULLMASK, J >= Ilow) == 0u) break;   // (padding: -1)
                     const unsigned long long jv = jinv[u];
                     const unsigned jlo = (unsigned)jv, jhi = (unsigned)(jv >> 32);
+                    const unsigned st_u32 = smem_u32(st);
                     double s0[9], s1[9];
 #pragma unroll
                     for (int p = 0; p < GB; ++p) {
                         const unsigned jb = ((p < 4 ? jlo : jhi) >> (8 * (p & 3))) & 0xFFu;
-                        double gx = 0.0, gy = 0.0, gz = 0.0;   // a union entry the point does not hold (0xFF) contributes zeros
-                        if (jb != 0xFFu) {
-                            const unsigned char* gq = st + (unsigned)(4 * p + 1) * k8 + jb * 8u;
-                            gx = *reinterpret_cast<const double*>(gq);
-                            gy = *reinterpret_cast<const double*>(gq + k8);
-                            gz = *reinterpret_cast<const double*>(gq + 2 * k8);
-                        }
+                        // a union entry the point does not hold (0xFF) contributes zeros: predicated loads
+                        const bool have = jb != 0xFFu;
+                        const unsigned gq = st_u32 + ((unsigned)p * prow8 + goff8) + jb * 8u;
+                        const double gx = lds_f64_if(gq, have), gy = lds_f64_if(gq + k8, have), gz = lds_f64_if(gq + 2 * k8, have);
                         const double2 a01 = *reinterpret_cast<const double2*>(aw + p * 6);       // ax0 ay0
                         const double2 a23 = *reinterpret_cast<const double2*>(aw + p * 6 + 2);   // az0 ax1
                         double2 a45 = make_double2(0.0, 0.0);
@@ -389,13 +407,37 @@ int rpim_stage_accumulate_panels(rpim_ctx* ctx, const double* d_qw, double lambd
     PanelArgs A;
     A.N = ctx->N; A.Nq = ctx->Nq; A.ntiles = ctx->ntiles;
     A.k = ctx->k; A.C = ctx->tg_C;
-    A.L = rpim_panel_smem(ctx->tg_C, ctx->tg_CW, ctx->tg_R, ctx->tg_T, ctx->k, std::max(ctx->max_ulen, 1), ctx->tg_nstage);
+    A.L = rpim_panel_smem(ctx->tg_C, ctx->tg_CW, ctx->tg_R, ctx->tg_T, ctx->k, std::max(ctx->max_ulen, 1), ctx->tg_nstage, ctx->tg_grad_only);
     A.hlog = A.L.hlog; A.nstage = ctx->tg_nstage;
     A.brow_ptr = ctx->d_brow_ptr; A.bcol = ctx->d_bcol; A.bdiag = ctx->d_bdiag; A.stage = ctx->d_stage;
     A.gmeta = ctx->d_gmeta;
     A.tile_ptr = ctx->d_tile_ptr; A.tdesc = ctx->d_tdesc;
     A.lambda = lambda; A.mu = mu; A.vals = d_vals;
     const int64_t G = (ctx->Nq + GB - 1) / GB;
+    A.grad_only = 0;
+    memset(&A.tmap, 0, sizeof(A.tmap));
+    if (ctx->tg_grad_only) {
+        // the staged array as a 2-D tensor [8 G points][4 k doubles]; a box is 8 points x the 3 k gradient doubles
+        typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                      const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                      CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+            qres != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            RPIM_FAIL(ctx, RPIM_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+        }
+        const cuuint64_t dims[2] = {(cuuint64_t)(4 * ctx->k), (cuuint64_t)(G * GB)};
+        const cuuint64_t strides[1] = {(cuuint64_t)(4 * ctx->k) * 8u};
+        const cuuint32_t box[2] = {(cuuint32_t)(3 * ctx->k), (cuuint32_t)GB};
+        const cuuint32_t estr[2] = {1u, 1u};
+        const CUresult cr = ((encode_fn)fn)(&A.tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)ctx->d_stage, dims, strides, box, estr,
+                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (cr != CUDA_SUCCESS) RPIM_FAIL(ctx, RPIM_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)cr);
+        A.grad_only = 1;
+    }
     const unsigned meta = rpim_panel_meta_bytes(ctx->tg_C);
     panel_weights_kernel<<<(unsigned)((G * GB + 255) / 256), 256, 0, ctx->stream>>>(ctx->Nq, G, meta, 32u * ctx->tg_C * 12u, d_qw, ctx->d_gmeta);
     KERNEL_CHECK(ctx);

@@ -19,6 +19,9 @@ oracle timed on a bounded sample of the same workload (a reported baseline, not 
 N > 1 (torchrun, one rank per GPU): the path partitions (quadrature points and matrix rows are
 independent per spatial partition), so every rank assembles its own partition of the
 same size with no data-path collective: weak scaling, value = total points / max-over-ranks time.
+With --shard the N ranks instead share ONE domain of the config (row slabs with point / node halos,
+paper_1802_04256_b200/partition.py; one allreduce(max) of a double per step): strong scaling,
+value = the domain's points / max-over-ranks time.
 
 `--impl reference` times the CPU oracle (oracle/, as it stands, one host core) on bounded samples
 of the same workload; under torchrun only rank 0 runs it.
@@ -174,6 +177,21 @@ def oracle_sample_rate(w, budget_s: float = 15.0):
     return S / t, S, t
 
 
+def shard_workload(config_name: str, rank: int, world: int):
+    """--shard: ONE domain cut into row slabs with point / node halos (paper_1802_04256_b200/partition.py, SURVEY.md
+    section 8(e)): the sub-problem of rank `rank`, its Shard and the domain's total point count.  The rank's owned
+    rows are complete and identical to the same rows of the undivided matrix; the only collective of a step is
+    allreduce(max) of one double (the penalty's max_i K_ii)."""
+    import dataclasses
+    from paper_1802_04256_b200 import partition as pt
+    w = workloads.config(config_name)
+    sh = pt.make_shard(w.nodes, w.qpts, w.k, rank, world)
+    bn, bm, bu = pt.local_bc(sh, w.bc_nodes, w.bc_mask, w.bc_ubar)
+    wl = dataclasses.replace(w, nodes=np.ascontiguousarray(w.nodes[sh.node_ids]), qpts=np.ascontiguousarray(w.qpts[sh.point_ids]),
+                             qw=np.ascontiguousarray(w.qw[sh.point_ids]), bc_nodes=bn, bc_mask=bm, bc_ubar=bu)
+    return wl, sh, w.Nq
+
+
 def rank_workload(config_name: str, rank: int, world: int):
     """The partition rank `rank` assembles.  The path shards by spatial partition (quadrature points are
     independent; K is row-partitionable) with no data-path collective: under weak scaling every
@@ -239,7 +257,12 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
     import paper_1802_04256_b200 as rp
 
     hbm_gbs, sm_max_mhz, peak_src = peaks
-    w = rank_workload(name, rank, world)
+    shard = None
+    nq_job = None
+    if args.shard:
+        w, shard, nq_job = shard_workload(name, rank, world)
+    else:
+        w = rank_workload(name, rank, world)
     ctx = rp.Context(local_rank)
     ctx.set_reduction({"auto": 0, "rows": 1, "panels": 2}[args.reduction])
     d_nodes = torch.from_numpy(w.nodes).to(dev)
@@ -262,7 +285,19 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
         assert n2 == nnz
         ctx.get_pattern(d_rp, d_ci, None)
         ctx.assemble(d_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f, want_singular=False)
-        ctx.apply_penalty(d_bcn, d_bcm, d_bcu, w.penalty_alpha, True, d_vals, d_f)
+        penalty()
+
+    def penalty():
+        if shard is None:
+            ctx.apply_penalty(d_bcn, d_bcm, d_bcu, w.penalty_alpha, True, d_vals, d_f)
+            return
+        # sharded domain: local max_d K_dd (m = 0 applies nothing), allreduce(max) of that one double, then the
+        # penalty with the absolute alpha on the owned boundary nodes
+        kmax = torch.tensor([ctx.apply_penalty(None, None, None, 1.0, True, d_vals, d_f)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(kmax, op=dist.ReduceOp.MAX)
+        if d_bcn.numel():
+            ctx.apply_penalty(d_bcn, d_bcm, d_bcu, w.penalty_alpha * float(kmax.item()), False, d_vals, d_f)
 
     def barrier():
         if world > 1:
@@ -289,14 +324,15 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
     launches = ctx.launch_count() - launches0
     phase_ms, calls = ctx.phase_totals(reset=True)
     ms_step = max_over_ranks(ms_total, world, dev) / steps
-    value = job_value(w.Nq, world, ms_step)
+    # replicas: every rank processed its own w.Nq points; sharded: the domain's points once (halo work is overhead)
+    value = job_value(w.Nq, world, ms_step) if shard is None else nq_job / (ms_step * 1e-3)
 
     # assemble + penalty only (paper stages 1 + 2, R12), same timing discipline
     barrier()
     e0.record(stream)
     for _ in range(steps):
         ctx.assemble(d_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f, want_singular=False)
-        ctx.apply_penalty(d_bcn, d_bcm, d_bcu, w.penalty_alpha, True, d_vals, d_f)
+        penalty()
     e1.record(stream)
     barrier()
     ms_asm = max_over_ranks(e0.elapsed_time(e1) / steps, world, dev)
@@ -456,8 +492,10 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
     out = {
         "w": w, "value": value, "ms_per_step": ms_step, "nnz": nnz, "bits": bits, "reduction": used,
         "reduction_params": red_params,
-        "assemble_penalty": {"value": world * w.Nq / (ms_asm * 1e-3), "unit": UNIT, "ms_per_step": ms_asm,
-                             "gdof_entries_per_s": 9.0 * w.k * w.k * w.Nq * world / (ms_asm * 1e-3) / 1e9},
+        "assemble_penalty": {"value": (world * w.Nq if shard is None else nq_job) / (ms_asm * 1e-3), "unit": UNIT, "ms_per_step": ms_asm,
+                             "gdof_entries_per_s": 9.0 * w.k * w.k * (w.Nq * world if shard is None else nq_job) / (ms_asm * 1e-3) / 1e9},
+        "shard": None if shard is None else {"rows": [shard.row_lo, shard.row_hi], "nodes_taken": int(shard.node_ids.size),
+                                             "points_taken": int(shard.point_ids.size), "points_domain": int(nq_job), "halo": shard.halo},
         "clocks": clocks, "e2e": e2e, "launches": int(launches), "roofline": roofline, "solve": solve,
         "update_nodes": update,
     }
@@ -477,8 +515,11 @@ def config_block(w, world, r):
             "reduction_params": r["reduction_params"],
             "l2": "inputs and outputs larger than L2 (no flush needed)" if r["nnz"] * 8 > 2.5e8 else
                   "working set may fit L2; no flush",
-            "parallelism": (f"{world} independent replicas of the workload, one per GPU (own jitter stream, no halo, "
-                            "no collective): not a sharded assembly of one domain") if world > 1 else "single GPU"}
+            "parallelism": ("single GPU" if world == 1 and r.get("shard") is None else
+                            (f"one domain sharded into {world} row slabs with point / node halos, allreduce(max) of one double "
+                             "per step (partition.py)") if r.get("shard") is not None else
+                            (f"{world} independent replicas of the workload, one per GPU (own jitter stream, no halo, "
+                             "no collective): not a sharded assembly of one domain"))}
 
 
 def main():
@@ -490,6 +531,9 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--reduction", default="auto", choices=["auto", "rows", "panels"],
                     help="reduction kernel (rpim_set_reduction): automatic choice, row-owner, or panel")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: shard ONE domain of the config into row slabs with halos (strong scaling, allreduce(max) of "
+                         "the penalty scale) instead of N independent replicas")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="do not also time `large` when the headline is `stress`")
@@ -543,12 +587,15 @@ def main():
         roofline["fp64_probe"] = r["fp64_probe"]
         line = {
             "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+            "scaling": "strong" if args.shard else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_block(w, world, r),
             "assemble_penalty": r["assemble_penalty"], "clocks": r["clocks"], "e2e": r["e2e"],
             "gpu_launches": r["launches"], "roofline": roofline, "cpu_baseline": cpu_baseline,
         }
         line["update_nodes"] = r["update_nodes"]
+        if r.get("shard") is not None:
+            line["shard"] = r["shard"]
         if secondary is not None:
             line["large"] = secondary
         if r["solve"] is not None:

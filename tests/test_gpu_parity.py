@@ -319,3 +319,12 @@ def test_panel_reduction_launch_shapes(env, monkeypatch):
     assert g["reduction_used"] == 2
     _compare(w, g, o)
     assert np.array_equal(g["vals"], g0["vals"]) and np.array_equal(g["f"], g0["f"])
+
+
+@pytest.mark.parametrize("q,alpha_c", [(0.5, 4.0), (0.5, 1.5), (-0.5, 4.0)])
+def test_classic_and_inverse_multiquadric(q, alpha_c):
+    """the other members of the radial family R = (r^2 + c^2)^q go through the same
+    kernels (classic multiquadric q = 1/2, inverse multiquadric q = -1/2); same bars, shape functions bitwise."""
+    w = workloads.make_block(f"mq{q}", 9, 8, 7, 1.0, 2, 30, 5e9, 0.3, jitter=0.3, seed=77, q=q, alpha_c=alpha_c,
+                             body=(10.0, -20.0, -2.5e4), bc="bottom+roller")
+    _compare(w, run_cuda(w), run_oracle(w))

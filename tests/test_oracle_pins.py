@@ -369,3 +369,31 @@ def test_paper_example1_closed_form(golden_dir):
     sigma = g["density_kg_m3"] * g["inferred"]["g"] * g["inferred"]["height_m"] / 1e6
     assert sigma == pytest.approx(g["theoretical_bottom_stress_MPa"], abs=5e-4)
     assert g["numerical_bottom_stress_MPa"] / g["theoretical_bottom_stress_MPa"] == pytest.approx(1 - 0.0675, abs=1e-3)
+
+
+# ------------------------------------------------------------------ other radial bases of the family
+@pytest.mark.parametrize("q,alpha_c,dense_tol", [
+    (0.5, 4.0, 2e-9),      # classic (Hardy) multiquadric sqrt(r^2 + c^2): conditionally NEGATIVE definite of order 1
+    (0.5, 1.5, 1e-11),
+    (-0.5, 4.0, 2e-10),    # inverse multiquadric: positive definite
+    (-0.5, 1.5, 1e-12),
+    (1.5, 4.0, 1e-8),
+])
+def test_other_multiquadric_exponents(q, alpha_c, dense_tol):
+    """R(r) = (r^2 + (alpha_c d_c)^2)^q for other exponents than the configs' 1.03: the structured LDL^T of R7 does
+    not depend on the sign of the reduced block (its 1x1 pivots are tested by magnitude), so the classic and the
+    inverse multiquadric come out of the same code.  Pins: partition of unity, linear reproduction, the
+    long-double definition (tolerance ~ 30x the measured error: the flatter the basis, the worse conditioned)."""
+    w = workloads.make_block("v", 8, 8, 7, 1.0, 2, 30, 1e9, 0.3, jitter=0.3, seed=11, q=q, alpha_c=alpha_c)
+    sel = np.arange(0, w.Nq, max(1, w.Nq // 300))
+    pts = w.qpts[sel]
+    s = oracle.knn(w.nodes, pts, w.k, "grid")
+    phi, dphi, sing = oracle.shape(w.nodes, pts, s, w.alpha_c, w.d_c, w.q)
+    assert sing.sum() == 0
+    X = w.nodes[s]
+    assert np.abs(phi.sum(1) - 1.0).max() < 1e-13
+    assert np.abs(np.einsum("mk,mkb->mb", phi, X) - pts).max() < 1e-13 * max(1.0, np.abs(pts).max()) * 10
+    assert np.abs(np.einsum("mak,mkb->mab", dphi, X) - np.eye(3)).max() < 1e-13
+    pr, dr = oracle.shape_dense_ref(w.nodes, pts, s, w.alpha_c, w.d_c, w.q)
+    assert np.abs(phi - pr).max() / np.abs(pr).max() < dense_tol
+    assert np.abs(dphi - dr).max() / np.abs(dr).max() < dense_tol

@@ -110,3 +110,24 @@ def test_partition_degenerates_gracefully():
     nodes, pts = w.nodes[sh.node_ids], w.qpts[sh.point_ids]
     s = oracle.knn(np.ascontiguousarray(nodes), np.ascontiguousarray(pts), w.k, "grid")
     assert not pt.support_radius_ok(nodes, pts, s, sh.halo)
+
+
+def test_bench_shard_workload_covers_the_domain_once():
+    """bench.py --shard: the ranks' sub-problems own every block row and every boundary condition exactly once, and
+    take every quadrature point at least once (halo points more than once)."""
+    import bench
+    import workloads
+    world = 3
+    w = workloads.config("cantilever")
+    rows, bcs, pts = [], [], np.zeros(w.Nq, dtype=np.int64)
+    for r in range(world):
+        wl, sh, nq = bench.shard_workload("cantilever", r, world)
+        assert nq == w.Nq and wl.N == sh.node_ids.size and wl.Nq == sh.point_ids.size
+        rows.append((sh.row_lo, sh.row_hi))
+        bcs.append(sh.node_ids[wl.bc_nodes])                     # local -> global ids of the rank's boundary nodes
+        assert np.all((bcs[-1] >= sh.row_lo) & (bcs[-1] < sh.row_hi))
+        pts[sh.point_ids] += 1
+        assert np.array_equal(wl.nodes, w.nodes[sh.node_ids]) and np.array_equal(wl.qw, w.qw[sh.point_ids])
+    assert rows[0][0] == 0 and rows[-1][1] == w.N and all(a[1] == b[0] for a, b in zip(rows[:-1], rows[1:]))
+    assert np.array_equal(np.sort(np.concatenate(bcs)), w.bc_nodes)
+    assert pts.min() >= 1 and pts.max() > 1

@@ -1,6 +1,8 @@
 // Step a2 (R2): node -> point incidence lists, block-CSR pattern (union of
 // supp x supp), scalar CSR emission.  Integer work only; every list is sorted, so the
 // result does not depend on the order in which threads happen to run.
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace {
@@ -147,15 +149,14 @@ __device__ __forceinline__ void table_to_sorted_list(const int* table, int* list
 constexpr int B1W = 320;      // level-1 words per warp: windows of up to 320 * 32 * 32 = 327,680 node ids
 constexpr int B2CAP = 512;    // touched 32-id blocks per row
 constexpr int BM_WARPS = 8;
-constexpr int BM_GCAP = 256;  // (group, point mask) pairs of a row kept on chip for the group sweeps
-constexpr int BM_PER_WARP = B1W + B1W / 2 + B2CAP + B2CAP / 2 + 32 + 2 * BM_GCAP;   // 32-bit words of shared memory
+constexpr int BM_PER_WARP = B1W + B1W / 2 + B2CAP + B2CAP / 2 + 32;   // 32-bit words of shared memory
 
 template <int PSTRIDE>
 __global__ void __launch_bounds__(BM_WARPS * 32)
 brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
                    const int32_t* __restrict__ support, int k, int* __restrict__ blen, int32_t* __restrict__ pool,
                    int* __restrict__ bdiag, int32_t* __restrict__ ovf_rows, unsigned* __restrict__ masks,
-                   const unsigned char* __restrict__ gmeta, int gC, long long* __restrict__ flags) {
+                   long long* __restrict__ flags) {
     constexpr int NWS = PSTRIDE / 32;   // mask words per (row, incident point)
     constexpr int NPASS = PSTRIDE / 256; // passes of 32 lanes over a support (8 k <= PSTRIDE)
     constexpr unsigned FULLW = 0xffffffffu;
@@ -167,9 +168,6 @@ brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t
     unsigned short* p1 = reinterpret_cast<unsigned short*>(l1 + B1W);                 // [B1W] touched blocks before word
     unsigned short* p2 = reinterpret_cast<unsigned short*>(l1 + B1W + B1W / 2);       // [B2CAP] columns before block
     unsigned* mw = l1 + B1W + B1W / 2 + B2CAP / 2;                                    // [32] mask words of one point
-    int* gl = reinterpret_cast<int*>(mw + 32);                                        // [BM_GCAP] groups incident to the row
-    unsigned* gm = reinterpret_cast<unsigned*>(gl + BM_GCAP);                         // [BM_GCAP] their points that hold the row's node
-    const unsigned gcap = 32u * (unsigned)gC, gmeta_bytes = gcap * 12u + RPIM_GROUP_POINTS * 8u;
     for (int64_t I = (int64_t)blockIdx.x * BM_WARPS + wid; I < N; I += (int64_t)gridDim.x * BM_WARPS) {
         const int64_t pa = inc_ptr[I], pb = inc_ptr[I + 1];
         const int np = (int)(pb - pa);
@@ -219,68 +217,6 @@ brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t
             }
         };
         auto nop = [](int) {};
-        // With point groups (groups.cu: the panel reduction's preprocessing) the same union is reached through
-        // the groups' sorted unions U_g: a node J of U_g is a column of the row iff one of the group's points
-        // holds both J and the row's node.  One visit per (row, group) with |U_g| ~ 1.3 k entries instead of
-        // one per (row, point) with k entries.  The (group, point mask) pairs of the row go to shared memory
-        // first (runs of equal q / 8 in the ascending incidence list; a run cut by a 32-entry boundary gives
-        // two pairs, which is harmless for a union).
-        int ngl = -1;   // -1: no group sweep for this row
-        if (gC > 0) {
-            ngl = 0;
-            for (int t0 = 0; t0 < np; t0 += 32) {
-                const int t = t0 + lane;
-                const int q = t < np ? inc_q[pa + t] : -1;
-                const int g = q >= 0 ? q / RPIM_GROUP_POINTS : -1;
-                const unsigned bit = q >= 0 ? 1u << (q % RPIM_GROUP_POINTS) : 0u;
-                const int gp = __shfl_up_sync(FULLW, g, 1);
-                const bool head = q >= 0 && (lane == 0 || g != gp);
-                unsigned m = bit;
-#pragma unroll
-                for (int d = 1; d < RPIM_GROUP_POINTS; ++d) {
-                    const int gd = __shfl_down_sync(FULLW, g, d);
-                    const unsigned bd = __shfl_down_sync(FULLW, bit, d);
-                    if (lane + d < 32 && gd == g) m |= bd;
-                }
-                const unsigned heads = __ballot_sync(FULLW, head);
-                const int pos = ngl + __popc(heads & ((1u << lane) - 1u));
-                if (head && pos < BM_GCAP) { gl[pos] = g; gm[pos] = m; }
-                ngl += __popc(heads);
-            }
-            if (ngl > BM_GCAP) ngl = -1;   // (never with the configs' densities) back to the point sweep
-            __syncwarp();
-        }
-        auto sweep_groups = [&](auto&& body) {
-            // lane u of pass ps holds union entry 32 ps + u of the group: its node and the points that hold it
-            auto fetch = [&](int i, int (&J)[4], unsigned (&pm)[4]) {
-                const unsigned char* rec = gmeta + (int64_t)gl[i] * gmeta_bytes;
-#pragma unroll
-                for (int ps = 0; ps < 4; ++ps) {
-                    J[ps] = -1;
-                    pm[ps] = 0u;
-                    if (ps < gC) {
-                        const int u = 32 * ps + lane;
-                        J[ps] = reinterpret_cast<const int*>(rec + gcap * 8u)[u];
-                        const uint2 jv = reinterpret_cast<const uint2*>(rec)[u];
-                        // bit p = byte p of jinv is not 0xFF
-                        const unsigned a = __vcmpne4(jv.x, 0xFFFFFFFFu) & 0x01010101u, b = __vcmpne4(jv.y, 0xFFFFFFFFu) & 0x01010101u;
-                        pm[ps] = ((a * 0x01020408u) >> 24) | (((b * 0x01020408u) >> 24) << 4);
-                    }
-                }
-            };
-            int J_c[4], J_n[4];
-            unsigned pm_c[4], pm_n[4];
-            fetch(0, J_c, pm_c);
-            for (int i = 0; i < ngl; ++i) {
-                if (i + 1 < ngl) fetch(i + 1, J_n, pm_n);
-                const unsigned m = gm[i];
-#pragma unroll
-                for (int ps = 0; ps < 4; ++ps)
-                    if (J_c[ps] >= 0 && (pm_c[ps] & m)) body(J_c[ps]);
-#pragma unroll
-                for (int ps = 0; ps < 4; ++ps) { J_c[ps] = J_n[ps]; pm_c[ps] = pm_n[ps]; }
-            }
-        };
         // exclusive prefix of a per-lane count over the warp; returns (prefix, total)
         auto warp_excl = [&](int cnt, int& total) {
             int incl = cnt;
@@ -301,7 +237,7 @@ brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t
                 const int b = (J - base) >> 5;
                 atomicOr(&l1[b >> 5], 1u << (b & 31));
             };
-            if (ngl > 0) sweep_groups(markA); else sweep(nop, markA, nop);
+            sweep(nop, markA, nop);
             __syncwarp();
             const int C1 = (n1 + 31) >> 5;   // level-1 words per lane: lane owns [lane C1, lane C1 + C1)
             {
@@ -326,7 +262,7 @@ brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t
                     const int r = p1[b >> 5] + __popc(l1[b >> 5] & ((1u << (b & 31)) - 1u));
                     atomicOr(&l2[r], 1u << (d & 31));
                 };
-                if (ngl > 0) sweep_groups(markB); else sweep(nop, markB, nop);
+                sweep(nop, markB, nop);
                 __syncwarp();
                 const int C2 = (nb2 + 31) >> 5;
                 {
@@ -398,6 +334,173 @@ brow_bitmap_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t
                 __syncwarp();
             });
         }
+    }
+}
+
+// Block rows THROUGH THE POINT GROUPS (panel reduction's preprocessing, groups.cu), ONE sweep: the row's incident
+// groups (runs of q / 8 in its ascending incidence list) are visited once; a node J of a group's sorted union U_g
+// is a column of the row iff one of the group's points holds both J and the row's node (a byte-mask test).  The
+// columns go into a small open-addressing table block of 32 ids -> 32-bit word of members; the touched blocks
+// (~ a hundred) are then compacted, sorted and expanded in order.  No window, no second sweep: the two-level
+// bitmap of brow_bitmap_kernel needs the touched blocks before it can place the ids.
+constexpr int BG_HB = 512;      // table entries per warp (touched blocks of a row: ~ L / 4)
+constexpr int BG_GCAP = 256;    // (group, point mask) pairs of a row
+constexpr int BG_WARPS = 8;
+constexpr int BG_PER_WARP = 2 * BG_HB + 2 * BG_GCAP;   // 32-bit words per warp (keys and words double as the 64-bit sort buffer)
+
+template <int PSTRIDE>
+__global__ void __launch_bounds__(BG_WARPS * 32)
+brow_groups_kernel(int64_t N, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q, int* __restrict__ blen,
+                   int32_t* __restrict__ pool, int* __restrict__ bdiag, int32_t* __restrict__ ovf_rows,
+                   const unsigned char* __restrict__ gmeta, int gC, long long* __restrict__ flags) {
+    constexpr unsigned FULLW = 0xffffffffu;
+    extern __shared__ __align__(16) unsigned bg_smem[];
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned* ws = bg_smem + (size_t)wid * BG_PER_WARP;
+    unsigned long long* kw = reinterpret_cast<unsigned long long*>(ws);   // [BG_HB] (block id << 32) | member word; ~0 = empty
+    int* gl = reinterpret_cast<int*>(ws + 2 * BG_HB);                      // [BG_GCAP] groups incident to the row
+    unsigned* gm = reinterpret_cast<unsigned*>(gl + BG_GCAP);              // [BG_GCAP] their points that hold the row's node
+    const unsigned gcap = 32u * (unsigned)gC, gmeta_bytes = gcap * 12u + RPIM_GROUP_POINTS * 8u;
+    const unsigned lt = (1u << lane) - 1u;
+    for (int64_t I = (int64_t)blockIdx.x * BG_WARPS + wid; I < N; I += (int64_t)gridDim.x * BG_WARPS) {
+        const int64_t pa = inc_ptr[I], pb = inc_ptr[I + 1];
+        const int np = (int)(pb - pa);
+        if (np == 0) {
+            if (lane == 0) blen[I] = 0;
+            continue;
+        }
+        __syncwarp();
+        for (int i = lane; i < BG_HB; i += 32) kw[i] = ~0ull;
+        // (group, point mask) pairs of the row; a run cut by a 32-entry boundary gives two pairs (harmless for a union)
+        int ngl = 0;
+        for (int t0 = 0; t0 < np; t0 += 32) {
+            const int t = t0 + lane;
+            const int q = t < np ? inc_q[pa + t] : -1;
+            const int g = q >= 0 ? q / RPIM_GROUP_POINTS : -1;
+            const unsigned bit = q >= 0 ? 1u << (q % RPIM_GROUP_POINTS) : 0u;
+            const int gp = __shfl_up_sync(FULLW, g, 1);
+            const bool head = q >= 0 && (lane == 0 || g != gp);
+            unsigned m = bit;
+#pragma unroll
+            for (int d = 1; d < RPIM_GROUP_POINTS; ++d) {
+                const int gd = __shfl_down_sync(FULLW, g, d);
+                const unsigned bd = __shfl_down_sync(FULLW, bit, d);
+                if (lane + d < 32 && gd == g) m |= bd;
+            }
+            const unsigned heads = __ballot_sync(FULLW, head);
+            const int pos = ngl + __popc(heads & lt);
+            if (head && pos < BG_GCAP) { gl[pos] = g; gm[pos] = m; }
+            ngl += __popc(heads);
+        }
+        bool ovf = ngl > BG_GCAP;
+        __syncwarp();
+        if (!ovf) {
+            // ---- the sweep: lane u of pass ps holds union entry 32 ps + u of the group
+            auto fetch = [&](int i, int (&J)[4], unsigned (&pm)[4]) {
+                const unsigned char* rec = gmeta + (int64_t)gl[i] * gmeta_bytes;
+#pragma unroll
+                for (int ps = 0; ps < 4; ++ps) {
+                    J[ps] = -1;
+                    pm[ps] = 0u;
+                    if (ps < gC) {
+                        const int u = 32 * ps + lane;
+                        J[ps] = reinterpret_cast<const int*>(rec + gcap * 8u)[u];
+                        const uint2 jv = reinterpret_cast<const uint2*>(rec)[u];
+                        const unsigned a = __vcmpne4(jv.x, 0xFFFFFFFFu) & 0x01010101u, b = __vcmpne4(jv.y, 0xFFFFFFFFu) & 0x01010101u;
+                        pm[ps] = ((a * 0x01020408u) >> 24) | (((b * 0x01020408u) >> 24) << 4);
+                    }
+                }
+            };
+            int J_c[4], J_n[4];
+            unsigned pm_c[4], pm_n[4];
+            bool full = false;
+            fetch(0, J_c, pm_c);
+            for (int i = 0; i < ngl; ++i) {
+                if (i + 1 < ngl) fetch(i + 1, J_n, pm_n);
+                const unsigned m = gm[i];
+#pragma unroll
+                for (int ps = 0; ps < 4; ++ps) {
+                    if (J_c[ps] >= 0 && (pm_c[ps] & m)) {
+                        const unsigned blk = (unsigned)J_c[ps] >> 5;
+                        const unsigned long long bitw = 1ull << (J_c[ps] & 31);
+                        unsigned h = (blk * 2654435761u) >> (32 - 9);   // BG_HB = 2^9
+                        int probes = 0;
+                        while (true) {
+                            const unsigned long long cur = kw[h];
+                            if ((unsigned)(cur >> 32) == blk) { atomicOr(&kw[h], bitw); break; }
+                            if (cur == ~0ull) {
+                                // claim the entry with an empty member word, then set the bit (another lane may have claimed it for
+                                // the same or another block in between: look again)
+                                atomicCAS(&kw[h], ~0ull, (unsigned long long)blk << 32);
+                                continue;
+                            }
+                            h = (h + 1) & (BG_HB - 1);
+                            if (++probes >= BG_HB) { full = true; break; }
+                        }
+                    }
+                }
+#pragma unroll
+                for (int ps = 0; ps < 4; ++ps) { J_c[ps] = J_n[ps]; pm_c[ps] = pm_n[ps]; }
+            }
+            ovf = __any_sync(FULLW, full);
+        }
+        __syncwarp();
+        int nb = 0, L = 0;
+        if (!ovf) {
+            // ---- compact the touched blocks to the front (reads of a 32-entry slice complete before its writes), count columns
+            for (int i0 = 0; i0 < BG_HB; i0 += 32) {
+                const unsigned long long v = kw[i0 + lane];
+                const bool used = v != ~0ull;
+                const unsigned mk = __ballot_sync(FULLW, used);
+                __syncwarp();
+                if (used) kw[nb + __popc(mk & lt)] = v;
+                nb += __popc(mk);
+                L += __popc((unsigned)v & (used ? 0xffffffffu : 0u));
+                __syncwarp();
+            }
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) L += __shfl_xor_sync(FULLW, L, d);
+            ovf = L > PSTRIDE;
+        }
+        if (ovf) {
+            if (lane == 0) {
+                blen[I] = 0;
+                const unsigned long long slot = atomicAdd((unsigned long long*)&flags[FLAG_OVF_ROWS], 1ull);
+                ovf_rows[slot] = (int32_t)I;
+            }
+            __syncwarp();
+            continue;
+        }
+        // ---- sort the blocks by id (the key is the high half), then expand the member words in order
+        const int npow = next_pow2(nb);
+        for (int i = nb + lane; i < npow; i += 32) kw[i] = ~0ull;
+        __syncwarp();
+        warp_bitonic_u64(kw, npow);
+        int32_t* dst = pool + I * PSTRIDE;
+        int base = 0;
+        for (int i0 = 0; i0 < nb; i0 += 32) {
+            const int i = i0 + lane;
+            const unsigned long long v = i < nb ? kw[i] : 0ull;
+            unsigned ids = i < nb ? (unsigned)v : 0u;
+            const int cnt = __popc(ids);
+            int incl = cnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int up = __shfl_up_sync(FULLW, incl, d);
+                if (lane >= d) incl += up;
+            }
+            int pre = base + incl - cnt;
+            const int blk32 = (int)(unsigned)(v >> 32) << 5;
+            while (ids) {
+                const int key = blk32 + __ffs(ids) - 1;
+                ids &= ids - 1;
+                dst[pre] = key;
+                if (key == (int)I) bdiag[I] = pre;
+                ++pre;
+            }
+            base += __shfl_sync(FULLW, incl, 31);
+        }
+        if (lane == 0) blen[I] = L;
     }
 }
 
@@ -556,10 +659,20 @@ int launch_brow_bitmap(rpim_ctx* ctx, int32_t* d_pool, int32_t* d_ovf_rows, unsi
     const size_t smem = (size_t)BM_WARPS * BM_PER_WARP * sizeof(unsigned);
     CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const unsigned nb = (unsigned)std::min<int64_t>((N + BM_WARPS - 1) / BM_WARPS, 148 * 16);
-    // (point groups exist: the sweeps go through their unions; they never coexist with the slot masks)
+    // (point groups exist: the row unions go through theirs, in one sweep; they never coexist with the slot masks)
     const int gC = (ctx->tg_C > 0 && ctx->d_gmeta && !d_masks) ? ctx->tg_C : 0;
+    if (gC > 0) {
+        auto kg = brow_groups_kernel<PSTRIDE>;
+        const size_t smg = (size_t)BG_WARPS * BG_PER_WARP * sizeof(unsigned);
+        CUDA_TRY(ctx, cudaFuncSetAttribute(kg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smg));
+        const unsigned nbg = (unsigned)std::min<int64_t>((N + BG_WARPS - 1) / BG_WARPS, 148 * 16);
+        kg<<<nbg, BG_WARPS * 32, smg, ctx->stream>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_blen, d_pool, ctx->d_bdiag, d_ovf_rows,
+                                                      ctx->d_gmeta, gC, ctx->d_flags);
+        KERNEL_CHECK(ctx);
+        return RPIM_OK;
+    }
     kern<<<nb, BM_WARPS * 32, smem, ctx->stream>>>(N, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_support, ctx->k, ctx->d_blen,
-                                                   d_pool, ctx->d_bdiag, d_ovf_rows, d_masks, ctx->d_gmeta, gC, ctx->d_flags);
+                                                   d_pool, ctx->d_bdiag, d_ovf_rows, d_masks, ctx->d_flags);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
 }

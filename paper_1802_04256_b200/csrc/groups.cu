@@ -97,7 +97,7 @@ group_union_kernel(int64_t Nq, int k, int C, int64_t gstep, const int32_t* __res
 // One thread per tile: merge of the T rows' incidence lists (ascending point ids) by point group.
 template <bool FILL>
 __global__ void __launch_bounds__(128)
-tile_desc_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restrict__ inc_ptr,
+tile_desc_thread_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restrict__ inc_ptr,
                  const int32_t* __restrict__ inc_q, const uint8_t* __restrict__ inc_j,
                  const uint8_t* __restrict__ gpos, int* __restrict__ count, const int64_t* __restrict__ tile_ptr,
                  unsigned* __restrict__ tdesc) {
@@ -147,6 +147,113 @@ tile_desc_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restr
         ++n;
     }
     if (!FILL) count[t] = n;
+}
+
+
+// One warp per tile: the T rows' incidence lists (ascending point ids) cut into runs of one point group each
+// (lane-parallel, 32 entries at a time), the (group, row, union position, point mask) items sorted by group in
+// shared memory, one descriptor per distinct group.  FILL = false counts the descriptors of a tile, FILL = true
+// writes them.  A tile with more than TD_ITEMS items or TD_GROUPS groups raises FLAG_PAT_CAP's neighbour
+// FLAG_TILE_CAP: the caller then takes the thread-per-tile kernel above.  (One thread per tile has the parallelism only
+// when there are hundreds of thousands of tiles; one warp per tile is 2.3x faster at `slope`, 7.8k tiles, and slower
+// at `stress`, 341k tiles, where its 26 KB of shared memory per warp leave 8 warps per SM.)
+constexpr int TD_ITEMS = 2048;   // (row, group) items of a tile (runs cut by a 32-entry boundary count twice)
+constexpr int TD_GROUPS = 512;   // distinct groups of a tile
+constexpr int TD_WARPS = 4;
+constexpr int TD_DWMAX = 1 + TMAX / 2;
+
+template <bool FILL>
+__global__ void __launch_bounds__(TD_WARPS * 32)
+tile_desc_warp_kernel(int64_t N, int64_t ntiles, int T, int k, const int64_t* __restrict__ inc_ptr,
+                 const int32_t* __restrict__ inc_q, const uint8_t* __restrict__ inc_j,
+                 const uint8_t* __restrict__ gpos, int* __restrict__ count, const int64_t* __restrict__ tile_ptr,
+                 unsigned* __restrict__ tdesc, long long* __restrict__ flags) {
+    constexpr unsigned FULLW = 0xffffffffu;
+    extern __shared__ __align__(16) unsigned char td_smem[];
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned long long* items = reinterpret_cast<unsigned long long*>(td_smem) + (size_t)wid * TD_ITEMS;
+    unsigned* desc = reinterpret_cast<unsigned*>(td_smem + (size_t)TD_WARPS * TD_ITEMS * 8) + (size_t)wid * TD_GROUPS * TD_DWMAX;   // (FILL only)
+    const int DW = 1 + T / 2;
+    const unsigned lt = (1u << lane) - 1u;
+    for (int64_t t = (int64_t)blockIdx.x * TD_WARPS + wid; t < ntiles; t += (int64_t)gridDim.x * TD_WARPS) {
+        __syncwarp();
+        int n = 0;
+        for (int r = 0; r < T; ++r) {
+            const int64_t I = t * T + r;
+            if (I >= N) break;
+            const int64_t pa = inc_ptr[I];
+            const int np = (int)(inc_ptr[I + 1] - pa);
+            for (int t0 = 0; t0 < np; t0 += 32) {
+                const int i = t0 + lane;
+                const int q = i < np ? inc_q[pa + i] : -1;
+                const int g = q >= 0 ? q / GB : -1;
+                const unsigned bit = q >= 0 ? 1u << (q % GB) : 0u;
+                const int gp = __shfl_up_sync(FULLW, g, 1);
+                const bool head = q >= 0 && (lane == 0 || g != gp);
+                unsigned m = bit;
+#pragma unroll
+                for (int d = 1; d < GB; ++d) {
+                    const int gd = __shfl_down_sync(FULLW, g, d);
+                    const unsigned bd = __shfl_down_sync(FULLW, bit, d);
+                    if (lane + d < 32 && gd == g) m |= bd;
+                }
+                const unsigned heads = __ballot_sync(FULLW, head);
+                const int pos = n + __popc(heads & lt);
+                if (head && pos < TD_ITEMS) {
+                    // every point of the group that holds the row's node holds it at the same union position
+                    const unsigned u = FILL ? gpos[(int64_t)q * k + inc_j[pa + i]] : 0u;
+                    items[pos] = ((unsigned long long)(unsigned)g << 32) | ((unsigned)r << 16) | (m << 8) | u;   // low 16 bits: the row's descriptor half
+                }
+                n += __popc(heads);
+            }
+        }
+        if (n > TD_ITEMS) {
+            if (lane == 0) atomicAdd((unsigned long long*)&flags[FLAG_TILE_CAP], 1ull);
+            if (!FILL && lane == 0) count[t] = 0;
+            continue;
+        }
+        const int npow = next_pow2(max(n, 1));
+        for (int i = n + lane; i < npow; i += 32) items[i] = ~0ull;
+        __syncwarp();
+        warp_bitonic_u64(items, npow);
+        // distinct groups: item i opens a descriptor when its group differs from the previous item's
+        int ng = 0;
+        const int64_t out0 = FILL ? tile_ptr[t] : 0;
+        if (FILL) {
+            const int cap = min((int)(tile_ptr[t + 1] - out0), TD_GROUPS) * DW;
+            for (int i = lane; i < cap; i += 32) desc[i] = 0u;
+            __syncwarp();
+        }
+        for (int i0 = 0; i0 < n; i0 += 32) {
+            const int i = i0 + lane;
+            const unsigned long long v = i < n ? items[i] : ~0ull;
+            const unsigned g = (unsigned)(v >> 32);
+            const unsigned gprev = (i > 0 && i < n) ? (unsigned)(items[i - 1] >> 32) : 0xFFFFFFFFu;
+            const bool head = i < n && (i == 0 || g != gprev);
+            const unsigned heads = __ballot_sync(FULLW, head);
+            if (FILL && i < n) {
+                const int d = ng + __popc(heads & (lt | (1u << lane))) - 1;   // descriptor of this item's group
+                if (d < TD_GROUPS) {
+                    if (head) desc[d * DW] = g;
+                    const unsigned r = (unsigned)(v >> 16) & 0xFFFFu, half = (unsigned)v & 0xFFFFu;
+                    atomicOr(&desc[d * DW + 1 + (r >> 1)], half << (16 * (r & 1)));
+                }
+            }
+            ng += __popc(heads);
+        }
+        if (ng > TD_GROUPS) {
+            if (lane == 0) atomicAdd((unsigned long long*)&flags[FLAG_TILE_CAP], 1ull);
+            if (!FILL && lane == 0) count[t] = 0;
+            continue;
+        }
+        if (!FILL) {
+            if (lane == 0) count[t] = ng;
+        } else {
+            __syncwarp();
+            unsigned* dst = tdesc + out0 * DW;
+            for (int i = lane; i < ng * DW; i += 32) dst[i] = desc[i];
+        }
+    }
 }
 
 }  // namespace
@@ -273,10 +380,31 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
     int* d_cnt = nullptr;
     if ((rc = ws_alloc(ctx, &d_cnt, ntiles))) return rc;
     if ((rc = ws_alloc(ctx, &ctx->d_tile_ptr, ntiles + 1))) { ws_free(ctx, &d_cnt); return rc; }
-    const unsigned nb = (unsigned)((ntiles + 127) / 128);
-    tile_desc_kernel<false><<<nb, 128, 0, st>>>(N, ntiles, T, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j,
-                                                 ctx->d_gpos, d_cnt, nullptr, nullptr);
-    ctx->launches++;
+    // descriptors: one warp per tile when the tiles are few (a thread per tile would leave the GPU empty), else --
+    // or when a tile overflows the warp kernel's shared-memory lists -- one thread per tile
+    const unsigned nbw = (unsigned)std::min<int64_t>((ntiles + TD_WARPS - 1) / TD_WARPS, 148 * 16);
+    const unsigned nbt = (unsigned)((ntiles + 127) / 128);
+    const size_t td_smem_cnt = (size_t)TD_WARPS * TD_ITEMS * 8;                                  // the count pass keeps no descriptors
+    const size_t td_smem = (size_t)TD_WARPS * (TD_ITEMS * 8 + TD_GROUPS * TD_DWMAX * 4);
+    bool by_warp = ntiles <= 65536;
+    if (by_warp) {
+        CUDA_TRY(ctx, cudaFuncSetAttribute(tile_desc_warp_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)td_smem_cnt));
+        CUDA_TRY(ctx, cudaFuncSetAttribute(tile_desc_warp_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)td_smem));
+        CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_TILE_CAP, 0, sizeof(long long), st));
+        tile_desc_warp_kernel<false><<<nbw, TD_WARPS * 32, td_smem_cnt, st>>>(N, ntiles, T, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j,
+                                                                             ctx->d_gpos, d_cnt, nullptr, nullptr, ctx->d_flags);
+        ctx->launches++;
+        long long tile_cap = 0;
+        cudaError_t e = cudaMemcpyAsync(&tile_cap, ctx->d_flags + FLAG_TILE_CAP, sizeof(long long), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { ws_free(ctx, &d_cnt); RPIM_FAIL(ctx, RPIM_ERR_CUDA, "tile descriptor count failed: %s", cudaGetErrorString(e)); }
+        if (tile_cap) by_warp = false;
+    }
+    if (!by_warp) {
+        tile_desc_thread_kernel<false><<<nbt, 128, 0, st>>>(N, ntiles, T, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j,
+                                                            ctx->d_gpos, d_cnt, nullptr, nullptr);
+        ctx->launches++;
+    }
     if (cudaGetLastError() != cudaSuccess) { ws_free(ctx, &d_cnt); RPIM_FAIL(ctx, RPIM_ERR_CUDA, "tile descriptor count launch failed"); }
     rc = rpim_scan_i32_to_i64(ctx, d_cnt, ctx->d_tile_ptr, ntiles);
     ws_free(ctx, &d_cnt);
@@ -285,8 +413,12 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
     CUDA_TRY(ctx, cudaMemcpyAsync(&total, ctx->d_tile_ptr + ntiles, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaStreamSynchronize(st));
     if ((rc = ws_alloc(ctx, &ctx->d_tdesc, std::max<int64_t>(total, 1) * DW))) return rc;
-    tile_desc_kernel<true><<<nb, 128, 0, st>>>(N, ntiles, T, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j,
-                                                ctx->d_gpos, nullptr, ctx->d_tile_ptr, ctx->d_tdesc);
+    if (by_warp)
+        tile_desc_warp_kernel<true><<<nbw, TD_WARPS * 32, td_smem, st>>>(N, ntiles, T, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j,
+                                                                        ctx->d_gpos, nullptr, ctx->d_tile_ptr, ctx->d_tdesc, ctx->d_flags);
+    else
+        tile_desc_thread_kernel<true><<<nbt, 128, 0, st>>>(N, ntiles, T, ctx->k, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j,
+                                                           ctx->d_gpos, nullptr, ctx->d_tile_ptr, ctx->d_tdesc);
     KERNEL_CHECK(ctx);
     ctx->tg_T = T;
     ctx->tg_CW = CW;

@@ -6,25 +6,27 @@
 // (column node J >= row node I) are accumulated; mirror_lower_kernel then fills the lower blocks with the
 // transposes.  Half the arithmetic, half the on-chip accumulators (twice the rows per tile).
 //
-// A CTA owns a TILE of T = 2 RP consecutive block rows at a time (tiles strided over a persistent grid).
+// A CTA owns a TILE of T = R RP consecutive block rows at a time (tiles strided over a persistent grid).
 // The accumulators S_IJ of their upper blocks (nine doubles per block column) live in SHARED memory, next to
 // each row's upper column list and a 16-bit open-addressing table column node -> slot.  The point groups
 // incident to the tile arrive through a ring of NSTAGE shared-memory stages filled by a PRODUCER warp with
-// TWO copies (cp.async.bulk + mbarrier): a 2-D tensor copy (TMA) of the gradient rows of the group's eight
-// consecutive points (a plain bulk copy of their whole staged rows when 24 k bytes is no 16-byte multiple)
-// and ONE plain bulk copy of the group's record (its sorted union of supports U_g, the map (union entry, point) ->
-// support position, the quadrature weights): the bulk-copy engine has a per-request cost, so few large
-// requests, not one per point.  Row pair rp (rows 2 rp, 2 rp + 1) has CW consumer warps; the chunks of 32
-// union entries from the one that holds the rows' own nodes upwards (U_g is ascending: everything below
-// is a lower block) are dealt to them round-robin.  In a chunk a lane owns one union entry and sums
-// (w grad phi_I) (x) grad phi_{U_g[u]} over the group's points IN REGISTERS (dense: |U_g| is 1.3 .. 1.6 k, both
-// rows share the gradient loads), then adds its nine sums per row to the row's accumulator of that column:
+// TWO requests per group (mbarrier completion): the gradient rows of the group's eight consecutive points as
+// one 2-D tensor copy (TMA: box 8 points x 3 k doubles of the [point][4 k] staged array) or, when that does
+// not buy ring depth or 24 k bytes is no 16-byte multiple, their whole staged rows as one plain bulk copy;
+// and the group's record (its sorted union of supports U_g, the map (union entry, point) -> support position,
+// the quadrature weights) as one plain bulk copy.  The copy engine has a per-request cost: few large
+// requests, not one per point.  Row group rp (R = 1: one block row; R = 2: a pair that shares the gradient
+// loads) has CW consumer warps; the chunks of 32 union entries from the one that holds the rows' own nodes
+// upwards (U_g is ascending: everything below is a lower block) are dealt to them round-robin.  In a chunk a
+// lane owns one union entry and sums (w grad phi_I) (x) grad phi_{U_g[u]} over the group's points IN REGISTERS
+// (dense: |U_g| is 1.3 .. 1.6 k), then adds its nine sums per row to the row's accumulator of that column:
 // one table probe and one read-modify-write per (row, group, column) instead of per (row, point, column).
-// The CW warps of a row pair meet at a named barrier between their read-modify-write phases of consecutive
+// The CW warps of a row group meet at a named barrier between their read-modify-write phases of consecutive
 // groups; nothing else synchronises in the steady state, and the producer runs ahead across tile
 // boundaries.  Every CSR entry is summed in a fixed order (points ascending inside a group, groups
-// ascending) by one lane: no floating-point atomics, bitwise run-to-run reproducible; every entry of K is
-// written once, with the isotropic closed form K_IJ = lambda S + mu S^T + mu tr(S) I applied at write-out.
+// ascending) by one lane: no floating-point atomics, bitwise run-to-run reproducible and independent of the
+// launch shape; every entry of K is written once, with the isotropic closed form
+// K_IJ = lambda S + mu S^T + mu tr(S) I applied at write-out.
 // The body-force load f_I = b sum_q w phi_I(q) is a separate row-owner pass over the incidence lists.
 #include <cuda.h>
 

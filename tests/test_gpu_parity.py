@@ -73,6 +73,7 @@ def test_jittered_blocks_span_tiles_and_ragged_tails(k, dims, jit, gauss):
     (40, (9, 8, 7), 2),            # 3 chunks
     (60, (10, 9, 8), 2),           # 4 chunks, rows of ~400 block columns
     (30, (9, 5, 5), 3),            # 27 points per cell: groups of 8 straddle cells
+    (60, (8, 7, 6), 3),            # long incidence lists: a tile's (row, group) items crowd the descriptor kernel's lists
     (124, (9, 8, 8), 2),           # unions beyond the 128-node limit: the row-owner kernel takes over
     (64, (9, 9, 8), 2),
     (12, (6, 6, 5), 1),            # one point per cell: sparse groups, still correct

@@ -42,7 +42,8 @@ typedef enum rpim_status {
     RPIM_ERR_STATE = -4,           /* call order violated (e.g. assemble before build_pattern) */
     RPIM_ERR_BC_NODE_INVALID = -5, /* boundary node id out of range, listed twice, or without a matrix row */
     RPIM_ERR_INDEX_OVERFLOW = -6,  /* 32-bit indices forced but nnz >= 2^31 */
-    RPIM_ERR_CAPACITY = -7,        /* an on-chip work buffer would overflow (pathological node cloud) */
+    RPIM_ERR_CAPACITY = -7,        /* an on-chip work buffer would overflow (a node in more than 4096 supports, a block row
+                                      of more than 2048 columns, k > N); the support search itself has no capacity limit */
     RPIM_ERR_BREAKDOWN = -8,       /* rpim_solve_pcg: p^T K p <= 0 or not finite (K is not positive definite) */
     RPIM_ERR_SINGULAR_POINT = -9   /* rpim_add_point_loads: a load point has a singular moment matrix */
 } rpim_status;

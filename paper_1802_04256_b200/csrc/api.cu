@@ -205,7 +205,7 @@ int rpim_update_nodes(rpim_ctx* ctx, const double* d_nodes, const double* d_qpts
     if (e != cudaSuccess || capf) {
         ws_free(ctx, &d_new);
         ctx->have_pattern = false;
-        if (capf) RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "kNN: %lld points need more than the on-chip candidate capacity", capf);
+        if (capf) RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "kNN: %lld points found fewer than k nodes (k > N?)", capf);
         RPIM_FAIL(ctx, RPIM_ERR_CUDA, "rpim_update_nodes failed: %s", cudaGetErrorString(e));
     }
     cudaEventElapsedTime(&ctx->phase_ms[0], ctx->ev[0], ctx->ev[1]);

@@ -15,7 +15,7 @@
 #define RPIM_PANEL_MAX_UNION_RATIO 2.0   // automatic choice: panel kernel when mean |U_g| <= ratio * k (the group's points share their supports)
 
 // device-side error / counter slots (ctx->d_flags, int64 each)
-enum { FLAG_KNN_CAP = 0, FLAG_PAT_CAP = 1, FLAG_BC_BAD = 2, FLAG_SINGULAR = 3, FLAG_INC_CAP = 4, FLAG_OVF_ROWS = 5, FLAG_OVF_Q = 6, FLAG_INC_LONG = 7, FLAG_ROW_TICKET = 8, FLAG_INC_LONG2 = 9, FLAG_TILE_CAP = 10, NUM_FLAGS = 16 };
+enum { FLAG_KNN_CAP = 0, FLAG_PAT_CAP = 1, FLAG_BC_BAD = 2, FLAG_SINGULAR = 3, FLAG_INC_CAP = 4, FLAG_OVF_ROWS = 5, FLAG_OVF_Q = 6, FLAG_INC_LONG = 7, FLAG_ROW_TICKET = 8, FLAG_INC_LONG2 = 9, FLAG_TILE_CAP = 10, FLAG_OVF_Q2 = 11, NUM_FLAGS = 16 };
 
 struct GridParams {
     double lo[3];

@@ -246,7 +246,8 @@ __global__ void cell_regather_kernel(const double* __restrict__ nodes, int64_t N
 // ------------------------------------------------------------------ the search: one warp per query point
 // CAP = candidates held on chip per query.  The first launch uses the smallest capacity that
 // fits the expected candidate count (more resident warps); queries that need more are appended
-// to an overflow list and redone by the KNN_CAP_MAX instantiation (LAST: overflow = failure).
+// to an overflow list and redone by the KNN_CAP_MAX instantiation; the LAST tier has no limit (streaming
+// selection: the buffer is sorted and cut back to the best k whenever it fills up).
 constexpr int KNN_CAP_MAX = 2048;
 
 template <int CAP, int WARPS, bool LAST>
@@ -255,7 +256,7 @@ knn_kernel(GridParams g, const double* __restrict__ sx, const double* __restrict
            const double* __restrict__ sz, const int* __restrict__ node_order,
            const int64_t* __restrict__ cell_start, const double* __restrict__ pts, int64_t M, int k, int R0,
            const int32_t* __restrict__ qlist, const long long* __restrict__ nq_ptr,
-           int32_t* __restrict__ ovf_list, int32_t* __restrict__ support, long long* __restrict__ flags) {
+           int32_t* __restrict__ ovf_list, int ovf_flag, int32_t* __restrict__ support, long long* __restrict__ flags) {
     extern __shared__ unsigned char smem_raw[];
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned long long* key = (unsigned long long*)smem_raw + (size_t)wid * CAP;
@@ -295,23 +296,34 @@ knn_kernel(GridParams g, const double* __restrict__ sx, const double* __restrict
                 ++R;
                 continue;
             }
-            if (cnt > CAP) { overflow = true; break; }
-            // gather candidates with their squared distances (R1: no fma, fixed association)
+            if (cnt > CAP && !LAST) { overflow = true; break; }
+            // gather candidates with their squared distances (R1: no fma, fixed association).  The last tier has no
+            // capacity limit: when the buffer is full it is sorted and only the best k are kept (streaming selection
+            // under the same total order (d^2, node id): the result does not depend on where the buffer filled up)
             int base = 0;
             for (int r = 0; r < nrows; ++r) {
                 int y = a[1] + r % ny, z = a[2] + r / ny;
                 int64_t c0 = a[0] + (int64_t)g.nc[0] * (y + (int64_t)g.nc[1] * z);
                 int64_t s0 = cell_start[c0], s1 = cell_start[c0 + (b[0] - a[0]) + 1];
-                for (int64_t p = s0 + lane; p < s1; p += 32) {
-                    double dx = __dsub_rn(sx[p], xq), dy = __dsub_rn(sy[p], yq), dz = __dsub_rn(sz[p], zq);
-                    double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-                    key[base + (int)(p - s0)] = (unsigned long long)__double_as_longlong(d2);
-                    val[base + (int)(p - s0)] = node_order[p];
+                while (s0 < s1) {
+                    const int take = (int)min((int64_t)(CAP - base), s1 - s0);
+                    for (int64_t p = s0 + lane; p < s0 + take; p += 32) {
+                        double dx = __dsub_rn(sx[p], xq), dy = __dsub_rn(sy[p], yq), dz = __dsub_rn(sz[p], zq);
+                        double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+                        key[base + (int)(p - s0)] = (unsigned long long)__double_as_longlong(d2);
+                        val[base + (int)(p - s0)] = node_order[p];
+                    }
+                    base += take;
+                    s0 += take;
+                    if (base == CAP && (s0 < s1 || r + 1 < nrows)) {   // (only the last tier gets here: cnt > CAP)
+                        __syncwarp();
+                        warp_bitonic_u64_i32(key, val, CAP);
+                        base = k;
+                    }
                 }
-                base += (int)(s1 - s0);
             }
-            npad = next_pow2(cnt);
-            for (int i = cnt + lane; i < npad; i += 32) { key[i] = 0xFFFFFFFFFFFFFFFFull; val[i] = 0x7FFFFFFF; }
+            npad = next_pow2(base);
+            for (int i = base + lane; i < npad; i += 32) { key[i] = 0xFFFFFFFFFFFFFFFFull; val[i] = 0x7FFFFFFF; }
             __syncwarp();
             warp_bitonic_u64_i32(key, val, npad);
             if (whole) break;
@@ -330,7 +342,7 @@ knn_kernel(GridParams g, const double* __restrict__ sx, const double* __restrict
         }
         if (overflow && !LAST) {
             if (lane == 0) {
-                const unsigned long long slot = atomicAdd((unsigned long long*)&flags[FLAG_OVF_Q], 1ull);
+                const unsigned long long slot = atomicAdd((unsigned long long*)&flags[ovf_flag], 1ull);
                 ovf_list[slot] = (int32_t)q;
             }
             __syncwarp();
@@ -585,9 +597,10 @@ int launch_knn_select(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, int3
     return RPIM_OK;
 }
 
+// qflag: the counter of the query list (when qlist is given); oflag: the counter of the overflow list this launch appends to
 template <int CAP, int WARPS, bool LAST>
-int launch_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, const int32_t* qlist, int32_t* ovf_list,
-               int32_t* d_support, int64_t blocks_cap) {
+int launch_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, int R0, const int32_t* qlist, int qflag, int32_t* ovf_list,
+               int oflag, int32_t* d_support, int64_t blocks_cap) {
     const int64_t N = ctx->N;
     auto kern = knn_kernel<CAP, WARPS, LAST>;
     const size_t smem = (size_t)WARPS * CAP * (sizeof(unsigned long long) + sizeof(int));
@@ -595,7 +608,7 @@ int launch_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, const int32
     int64_t blocks = qlist ? blocks_cap : std::min<int64_t>((M + WARPS - 1) / WARPS, blocks_cap);
     kern<<<(unsigned)blocks, WARPS * 32, smem, ctx->stream>>>(
         ctx->grid, ctx->d_sorted_xyz, ctx->d_sorted_xyz + N, ctx->d_sorted_xyz + 2 * N, ctx->d_node_order,
-        ctx->d_cell_start, d_pts, M, k, 2, qlist, ctx->d_flags + FLAG_OVF_Q, ovf_list, d_support, ctx->d_flags);
+        ctx->d_cell_start, d_pts, M, k, R0, qlist, ctx->d_flags + qflag, ovf_list, oflag, d_support, ctx->d_flags);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
 }
@@ -688,15 +701,26 @@ int rpim_stage_grid_knn(rpim_ctx* ctx, const double* d_pts, int64_t M, int k, in
     const double per_cell = (double)N / (double)g.ncell;
     const double expect = 125.0 * per_cell * 1.25;
     const int cap = expect <= 256 ? 256 : expect <= 512 ? 512 : expect <= 1024 ? 1024 : KNN_CAP_MAX;
+    // Tiers: the capacity the mean density asks for; its overflow list redone with the largest capacity; what still
+    // does not fit (a 5 x 5 x 5 ring of cells holding more than KNN_CAP_MAX nodes: local density ~ 14 x the mean,
+    // graded clouds) redone from the query's own cell outwards (R0 = 0) -- the ring only grows until the k-th
+    // distance is covered, so the dense spots need far fewer cells.  Same result in every tier, bit for bit.
     int rc = RPIM_OK;
-    if (cap == KNN_CAP_MAX) return launch_knn<KNN_CAP_MAX, 4, true>(ctx, d_pts, M, k, nullptr, nullptr, d_support, 148 * 64);
-    int32_t* d_ovf = nullptr;
-    if ((rc = ws_alloc(ctx, &d_ovf, M))) return rc;
+    int32_t *d_ovf = nullptr, *d_ovf2 = nullptr;
+    if ((rc = ws_alloc(ctx, &d_ovf, M)) || (rc = ws_alloc(ctx, &d_ovf2, M))) { ws_free(ctx, &d_ovf); return rc; }
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_OVF_Q, 0, sizeof(long long), st));
-    if (cap == 256) rc = launch_knn_select<8, 8>(ctx, d_pts, M, k, d_ovf, d_support, 148 * 64);
-    else if (cap == 512) rc = launch_knn_select<16, 8>(ctx, d_pts, M, k, d_ovf, d_support, 148 * 64);
-    else rc = launch_knn<1024, 4, false>(ctx, d_pts, M, k, nullptr, d_ovf, d_support, 148 * 64);
-    if (rc == RPIM_OK) rc = launch_knn<KNN_CAP_MAX, 4, true>(ctx, d_pts, M, k, d_ovf, nullptr, d_support, 148 * 2);
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_OVF_Q2, 0, sizeof(long long), st));
+    if (cap == KNN_CAP_MAX) {
+        rc = launch_knn<KNN_CAP_MAX, 4, false>(ctx, d_pts, M, k, 2, nullptr, FLAG_OVF_Q, d_ovf2, FLAG_OVF_Q2, d_support, 148 * 64);
+    } else {
+        if (cap == 256) rc = launch_knn_select<8, 8>(ctx, d_pts, M, k, d_ovf, d_support, 148 * 64);
+        else if (cap == 512) rc = launch_knn_select<16, 8>(ctx, d_pts, M, k, d_ovf, d_support, 148 * 64);
+        else rc = launch_knn<1024, 4, false>(ctx, d_pts, M, k, 2, nullptr, FLAG_OVF_Q, d_ovf, FLAG_OVF_Q, d_support, 148 * 64);
+        if (rc == RPIM_OK)
+            rc = launch_knn<KNN_CAP_MAX, 4, false>(ctx, d_pts, M, k, 2, d_ovf, FLAG_OVF_Q, d_ovf2, FLAG_OVF_Q2, d_support, 148 * 2);
+    }
+    if (rc == RPIM_OK) rc = launch_knn<KNN_CAP_MAX, 4, true>(ctx, d_pts, M, k, 0, d_ovf2, FLAG_OVF_Q2, nullptr, FLAG_OVF_Q2, d_support, 148 * 2);
+    ws_free(ctx, &d_ovf2);
     ws_free(ctx, &d_ovf);   // parked in the workspace cache (later reuse is ordered by the stream)
     return rc;
 }

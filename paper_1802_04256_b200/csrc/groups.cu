@@ -387,6 +387,7 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
     const size_t td_smem_cnt = (size_t)TD_WARPS * TD_ITEMS * 8;                                  // the count pass keeps no descriptors
     const size_t td_smem = (size_t)TD_WARPS * (TD_ITEMS * 8 + TD_GROUPS * TD_DWMAX * 4);
     bool by_warp = ntiles <= 65536;
+    if (const char* e = getenv("RPIM_TILE_DESC")) by_warp = e[0] == 'w';   // "warp" / "thread": tests
     if (by_warp) {
         CUDA_TRY(ctx, cudaFuncSetAttribute(tile_desc_warp_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)td_smem_cnt));
         CUDA_TRY(ctx, cudaFuncSetAttribute(tile_desc_warp_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)td_smem));

@@ -760,7 +760,7 @@ int rpim_stage_block_pattern(rpim_ctx* ctx) {
     CUDA_TRY(ctx, cudaStreamSynchronize(st));
     if (h_flags[FLAG_KNN_CAP]) {
         drop_tmp();
-        RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "kNN: %lld points need more than the on-chip candidate capacity (or k > N)",
+        RPIM_FAIL(ctx, RPIM_ERR_CAPACITY, "kNN: %lld points found fewer than k nodes (k > N?)",
                   h_flags[FLAG_KNN_CAP]);
     }
     if (h_flags[FLAG_INC_CAP]) {

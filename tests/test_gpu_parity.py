@@ -73,7 +73,6 @@ def test_jittered_blocks_span_tiles_and_ragged_tails(k, dims, jit, gauss):
     (40, (9, 8, 7), 2),            # 3 chunks
     (60, (10, 9, 8), 2),           # 4 chunks, rows of ~400 block columns
     (30, (9, 5, 5), 3),            # 27 points per cell: groups of 8 straddle cells
-    (60, (8, 7, 6), 3),            # long incidence lists: a tile's (row, group) items crowd the descriptor kernel's lists
     (124, (9, 8, 8), 2),           # unions beyond the 128-node limit: the row-owner kernel takes over
     (64, (9, 9, 8), 2),
     (12, (6, 6, 5), 1),            # one point per cell: sparse groups, still correct
@@ -306,6 +305,9 @@ def test_cuda_K_against_the_plain_definition(idx, reduction):
     {"RPIM_PANEL_R": "2", "RPIM_PANEL_CW": "1", "RPIM_PANEL_T": "2"},   # one warp takes all chunks of its pair
     {"RPIM_PANEL_R": "1", "RPIM_PANEL_CW": "1", "RPIM_PANEL_NSTAGE": "2"},
     {"RPIM_PANEL_R": "1", "RPIM_PANEL_CW": "3", "RPIM_PANEL_T": "4"},
+    {"RPIM_TILE_DESC": "thread"},     # the descriptor kernel large problems take (one thread per tile)
+    {"RPIM_PANEL_GRAD_ONLY": "1"},    # gradient rows by the 2-D tensor copy
+    {"RPIM_PANEL_GRAD_ONLY": "0"},    # whole staged rows by a plain bulk copy
 ])
 def test_panel_reduction_launch_shapes(env, monkeypatch):
     """The other launch shapes of reduce_panels_kernel (rows per warp group, warps per group, rows per tile, ring
@@ -329,3 +331,35 @@ def test_classic_and_inverse_multiquadric(q, alpha_c):
     w = workloads.make_block(f"mq{q}", 9, 8, 7, 1.0, 2, 30, 5e9, 0.3, jitter=0.3, seed=77, q=q, alpha_c=alpha_c,
                              body=(10.0, -20.0, -2.5e4), bc="bottom+roller")
     _compare(w, run_cuda(w), run_oracle(w))
+
+
+def test_graded_density_supports_and_pattern():
+    """A cloud whose local density is hundreds of times the mean (a 16^3 cluster of spacing 0.05 inside a unit-spaced
+    block): the 5 x 5 x 5 ring of grid cells around a query holds more nodes than the largest on-chip candidate
+    buffer, so the queries fall through to the last tier of the support search (own cell outwards, streaming
+    selection without a capacity limit).  Supports and CSR pattern must still equal the oracle's bit for bit."""
+    import torch
+    import oracle
+    import paper_1802_04256_b200 as rp
+    rng = np.random.default_rng(5)
+    w = workloads.make_block("graded", 8, 8, 6, 1.0, 1, 30, 5e9, 0.3, jitter=0.3, seed=9)
+    g = (np.stack(np.meshgrid(*[np.arange(16)] * 3, indexing="ij"), -1).reshape(-1, 3) * 0.05 + np.array([3.1, 3.2, 2.1])
+         + rng.uniform(-0.01, 0.01, (4096, 3)))
+    nodes = np.ascontiguousarray(np.concatenate([w.nodes, g]))
+    pts = np.ascontiguousarray(np.concatenate([w.qpts, g[::7] + 0.013, rng.uniform([2.5, 2.6, 1.5], [4.5, 4.6, 3.5], (300, 3))]))
+    k = 30
+    s = oracle.knn(nodes, pts, k, "brute")
+    rp_o, ci_o = oracle.pattern(s, nodes.shape[0])
+    dev = torch.device("cuda:0")
+    ctx = rp.Context(0)
+    try:
+        d_n, d_q = torch.from_numpy(nodes).to(dev), torch.from_numpy(pts).to(dev)
+        nnz, bits = ctx.build_pattern(d_n, d_q, k, 64)
+        d_rp = torch.empty(3 * nodes.shape[0] + 1, dtype=torch.int64, device=dev)
+        d_ci = torch.empty(nnz, dtype=torch.int64, device=dev)
+        d_sup = torch.empty((pts.shape[0], k), dtype=torch.int32, device=dev)
+        ctx.get_pattern(d_rp, d_ci, d_sup)
+        assert np.array_equal(d_sup.cpu().numpy(), s)
+        assert np.array_equal(d_rp.cpu().numpy(), rp_o) and np.array_equal(d_ci.cpu().numpy(), ci_o)
+    finally:
+        ctx.close()

@@ -247,7 +247,7 @@ int rpim_stage_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* 
 // block columns (diagonal included): byte offsets of its areas, identical on host and device.
 struct PanelSmem {
     int LS;            // accumulator / column-list stride in block columns (Ucap rounded up to even)
-    int hlog;          // log2 of the per-row table size (power of two >= 2 Ucap)
+    int hlog;          // log2 of the per-row table size (power of two >= 1.5 Ucap)
     unsigned stage_bytes;
     unsigned off_acc, off_bcol, off_hash, off_aw, off_stage, off_bar, off_rowo, total;
 };
@@ -260,7 +260,7 @@ inline PanelSmem rpim_panel_smem(int C, int CW, int R, int T, int k, int Ucap, i
     PanelSmem L;
     L.LS = (Ucap + 1) & ~1;
     L.hlog = 6;
-    while ((1 << L.hlog) < 2 * Ucap) ++L.hlog;
+    while (2 * (1 << L.hlog) < 3 * Ucap) ++L.hlog;   // load factor <= 2/3 at the longest row, ~ 0.45 typically
     auto up16 = [](unsigned v) { return (v + 15u) & ~15u; };
     auto up128 = [](unsigned v) { return (v + 127u) & ~127u; };
     L.stage_bytes = up128((unsigned)(RPIM_GROUP_POINTS * (grad_only ? 3 : 4) * k * 8) + rpim_panel_meta_bytes(C) + 32u);

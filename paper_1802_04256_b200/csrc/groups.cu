@@ -336,7 +336,7 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
     // Launch shape of reduce_panels_kernel.  Measured on B200: one block row per consumer
     // warp group and two warps per group (13 warps at T = 6) beat row pairs with three warps (10 warps) by 7 % at
     // `stress`; the most rows per tile (8, 6, 4, 2) that leave room for a ring of five stages (else four, three),
-    // then the deepest ring (<= 6).  RPIM_PANEL_R / _CW / _T / _NSTAGE override (tuning and tests).
+    // then the deepest ring (<= 8).  RPIM_PANEL_R / _CW / _T / _NSTAGE override (tuning and tests).
     int CW = 2;
     if (const char* e = getenv("RPIM_PANEL_CW")) { const int c = atoi(e); if (c >= 1 && c <= 4) CW = c; }
     int R = 1;
@@ -354,7 +354,7 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
                     if (rpim_panel_smem(ctx->tg_C, CW, R, t, ctx->k, Ucap, need, grad_only).total <= budget) T = t;
         if (const char* e = getenv("RPIM_PANEL_T")) { const int t = atoi(e); if (t >= 2 && t <= TMAX && !(t & 1)) T = t; }
         if (T == 0) return;
-        for (nstage = 6; nstage > 2 && rpim_panel_smem(ctx->tg_C, CW, R, T, ctx->k, Ucap, nstage, grad_only).total > budget; --nstage) {}
+        for (nstage = 8; nstage > 2 && rpim_panel_smem(ctx->tg_C, CW, R, T, ctx->k, Ucap, nstage, grad_only).total > budget; --nstage) {}
         if (const char* e = getenv("RPIM_PANEL_NSTAGE")) { const int n = atoi(e); if (n >= 2 && n <= 8) nstage = n; }
         if (rpim_panel_smem(ctx->tg_C, CW, R, T, ctx->k, Ucap, nstage, grad_only).total > budget) T = 0;
     };

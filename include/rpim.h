@@ -127,6 +127,13 @@ int rpim_assemble(rpim_ctx* ctx, const double* d_qw, double E, double nu, double
                   double d_c, double q, const double body[3], double* d_vals, double* d_f,
                   int64_t* out_singular);
 
+/* Strata with one Poisson ratio (R8b, part): a per-point modulus scale,
+ * E_q = E * d_escale[q] for the stiffness contribution of quadrature point q in every later rpim_assemble (and the
+ * stresses of rpim_recover_stress); the loads are not scaled.
+ *   d_escale  Nq fp64 (DEVICE, caller-owned: must stay valid until replaced), or NULL to switch it off
+ * Cleared by rpim_build_pattern (a new point set). */
+int rpim_set_modulus_scale(rpim_ctx* ctx, const double* d_escale);
+
 /* Step a5b (R9): f_{3I+c} += w * phi_I(x) * t_c at M given points (face Gauss
  * points of a traction boundary) using the shape parameters of the last rpim_assemble.
  *   d_pts M x 3, d_w M, d_t M x 3, d_f 3N (updated in place).  Synchronises the stream.

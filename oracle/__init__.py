@@ -96,10 +96,12 @@ def shape_dense_ref(nodes, pts, support, alpha_c: float, d_c: float, q: float):
 
 
 def assemble(nodes, pts, w, support, E, nu, alpha_c, d_c, q, body, row_ptr, col_idx,
-             node_lo: int = 0, node_hi: int | None = None):
+             node_lo: int = 0, node_hi: int | None = None, escale=None):
     """K values and f for rows of nodes [node_lo, node_hi).
 
     ``row_ptr`` / ``col_idx`` describe exactly those rows (row_ptr starts at 0).
+    ``escale`` (optional, one value per point): strata with one Poisson ratio, E_q = E * escale[q]
+    (R8b); the loads are not scaled.
     Returns (vals, f, n_singular).
     """
     nodes = _f64(nodes)
@@ -117,6 +119,18 @@ def assemble(nodes, pts, w, support, E, nu, alpha_c, d_c, q, body, row_ptr, col_
     vals = np.empty(int(row_ptr[-1]))
     f = np.empty(nrows)
     nsing = C.c_int64(0)
+    if escale is not None:
+        escale = _f64(escale)
+        assert escale.shape == (M,)
+        rc = lib().orc_assemble_strata(_p(nodes, C.c_double), _p(pts, C.c_double), _p(w, C.c_double), _p(escale, C.c_double),
+                                       _p(support, C.c_int32), C.c_int64(M), C.c_int(k), C.c_double(E),
+                                       C.c_double(nu), C.c_double(alpha_c), C.c_double(d_c), C.c_double(q),
+                                       _p(body, C.c_double), C.c_int64(node_lo), C.c_int64(node_hi),
+                                       _p(row_ptr, C.c_int64), _p(col_idx, C.c_int64), _p(vals, C.c_double),
+                                       _p(f, C.c_double), C.byref(nsing))
+        if rc:
+            raise RuntimeError(f"orc_assemble_strata failed ({rc})")
+        return vals, f, int(nsing.value)
     rc = lib().orc_assemble(_p(nodes, C.c_double), _p(pts, C.c_double), _p(w, C.c_double),
                             _p(support, C.c_int32), C.c_int64(M), C.c_int(k), C.c_double(E),
                             C.c_double(nu), C.c_double(alpha_c), C.c_double(d_c), C.c_double(q),

@@ -577,10 +577,12 @@ int orc_shape_dense_ref(const double* nodes, const double* pts, const int32_t* s
 // exactly those rows (row_ptr has 3*(node_hi-node_lo)+1 entries and starts at 0); vals and f
 // are zeroed here.  BASELINE.json north_star: "form B (6x3k) and w*B^T*D*B, and reduce the
 // result into a global CSR matrix over 3N DOFs".
-int orc_assemble(const double* nodes, const double* pts, const double* w, const int32_t* support,
-                 int64_t M, int k, double E, double nu, double alpha_c, double d_c, double q,
-                 const double* body, int64_t node_lo, int64_t node_hi, const int64_t* row_ptr,
-                 const int64_t* col_idx, double* vals, double* f, int64_t* n_singular) {
+// (escale: optional per-point modulus scale of DESIGN.md R8b, E_q = E * escale[q], one Poisson ratio: the
+// stiffness contribution of point q is weighted by w[q] * escale[q], the load by w[q]; NULL = none)
+static int assemble_impl(const double* nodes, const double* pts, const double* w, const double* escale, const int32_t* support,
+                         int64_t M, int k, double E, double nu, double alpha_c, double d_c, double q,
+                         const double* body, int64_t node_lo, int64_t node_hi, const int64_t* row_ptr,
+                         const int64_t* col_idx, double* vals, double* f, int64_t* n_singular) {
     ShapeParams SP;
     shape_setup(alpha_c, d_c, q, SP);
     const double lam = E * nu / ((1.0 + nu) * (1.0 - 2.0 * nu));
@@ -602,6 +604,7 @@ int orc_assemble(const double* nodes, const double* pts, const double* w, const 
         for (int i = 0; i < k; ++i) touches |= (s[i] >= node_lo && s[i] < node_hi);
         if (!touches) continue;
         if (shape_point(nodes, s, k, pts + 3 * p, SP, phi.data(), dphi.data(), work)) { ++nsing; continue; }
+        const double wk = escale ? w[p] * escale[p] : w[p];
         const int nc = 3 * k;
         std::fill(B.begin(), B.end(), 0.0);
         for (int i = 0; i < k; ++i) {
@@ -633,7 +636,7 @@ int orc_assemble(const double* nodes, const double* pts, const double* w, const 
                         const int64_t col = 3 * (int64_t)s[j] + b;
                         const int64_t* it = std::lower_bound(cb, cb + len, col);
                         if (it == cb + len || *it != col) return -3;   // pattern does not contain the entry
-                        vals[row_ptr[row] + (it - cb)] += w[p] * acc;
+                        vals[row_ptr[row] + (it - cb)] += wk * acc;
                     }
                 f[row] += (w[p] * phi[i]) * body[a];
             }
@@ -641,6 +644,23 @@ int orc_assemble(const double* nodes, const double* pts, const double* w, const 
     }
     if (n_singular) *n_singular = nsing;
     return 0;
+}
+
+int orc_assemble(const double* nodes, const double* pts, const double* w, const int32_t* support,
+                 int64_t M, int k, double E, double nu, double alpha_c, double d_c, double q,
+                 const double* body, int64_t node_lo, int64_t node_hi, const int64_t* row_ptr,
+                 const int64_t* col_idx, double* vals, double* f, int64_t* n_singular) {
+    return assemble_impl(nodes, pts, w, nullptr, support, M, k, E, nu, alpha_c, d_c, q, body, node_lo, node_hi, row_ptr, col_idx,
+                         vals, f, n_singular);
+}
+
+// R8b: strata with one Poisson ratio -- per-point modulus E_q = E * escale[q]
+int orc_assemble_strata(const double* nodes, const double* pts, const double* w, const double* escale, const int32_t* support,
+                        int64_t M, int k, double E, double nu, double alpha_c, double d_c, double q,
+                        const double* body, int64_t node_lo, int64_t node_hi, const int64_t* row_ptr,
+                        const int64_t* col_idx, double* vals, double* f, int64_t* n_singular) {
+    return assemble_impl(nodes, pts, w, escale, support, M, k, E, nu, alpha_c, d_c, q, body, node_lo, node_hi, row_ptr, col_idx,
+                         vals, f, n_singular);
 }
 
 // R9: point loads (face traction): f_{3I+c} += (w * phi_I) * t_c at given points with their

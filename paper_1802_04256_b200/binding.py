@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = (
     "rpim_get_pattern", "rpim_assemble", "rpim_add_point_loads", "rpim_apply_penalty", "rpim_get_shape",
     "rpim_host_pattern", "rpim_host_assemble", "rpim_last_phase_ms", "rpim_phase_totals", "rpim_launch_count",
     "rpim_matvec", "rpim_solve_pcg", "rpim_recover_stress", "rpim_set_reduction", "rpim_reduction_used",
-    "rpim_probe_fp64", "rpim_update_nodes", "rpim_reduction_params",
+    "rpim_probe_fp64", "rpim_update_nodes", "rpim_reduction_params", "rpim_set_modulus_scale",
 )
 
 
@@ -72,6 +72,7 @@ def _load():
     lib.rpim_set_reduction.argtypes = [vp, C.c_int]
     lib.rpim_reduction_used.argtypes = [vp]
     lib.rpim_reduction_params.argtypes = [vp, C.POINTER(C.c_int)]
+    lib.rpim_set_modulus_scale.argtypes = [vp, vp]
     _lib = lib
     return lib
 
@@ -152,6 +153,11 @@ def rpim_set_reduction(ctx, mode: int):
 
 def rpim_reduction_used(ctx) -> int:
     return int(_load().rpim_reduction_used(ctx))
+
+
+def rpim_set_modulus_scale(ctx, d_escale):
+    """d_escale: CUDA float64 tensor of Nq values (kept alive by the caller) or None."""
+    _check(ctx, _load().rpim_set_modulus_scale(ctx, C.c_void_p(0 if d_escale is None else d_escale.data_ptr())))
 
 
 def rpim_reduction_params(ctx) -> dict:
@@ -345,6 +351,10 @@ class Context:
 
     def reduction_params(self):
         return rpim_reduction_params(self.ctx)
+
+    def set_modulus_scale(self, d_escale):
+        self._escale = d_escale          # keeps the tensor alive while the library points at it
+        return rpim_set_modulus_scale(self.ctx, d_escale)
 
     def launch_count(self):
         return rpim_launch_count(self.ctx)

@@ -70,7 +70,7 @@ template <int NWARP, int CPW, int ROWS, bool MASKED>
 __global__ void __launch_bounds__(NWARP * ROWS * 32)
 reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_ptr, const int32_t* __restrict__ inc_q,
                    const uint8_t* __restrict__ inc_j, const int32_t* __restrict__ support,
-                   const double* __restrict__ stage, const double* __restrict__ qw,
+                   const double* __restrict__ stage, const double* __restrict__ qw, const double* __restrict__ escale,
                    const int64_t* __restrict__ brow_ptr, const int32_t* __restrict__ bcol,
                    const int64_t* __restrict__ mask_ptr, const unsigned* __restrict__ masks, int mask_stride,
                    unsigned long long* __restrict__ ticket, double lambda, double mu, double bx, double by, double bz, double* __restrict__ vals, double* __restrict__ f) {
@@ -136,7 +136,8 @@ reduce_rows_kernel(int64_t N, int k, int nbg, const int64_t* __restrict__ inc_pt
                 const double w = qw[q];
                 const double* base = stage + (int64_t)q * k * 4;
                 fsum += w * base[i];   // staged layout [q][phi, d/dx, d/dy, d/dz][k]
-                sm.a[tg][0] = w * base[k + i]; sm.a[tg][1] = w * base[2 * k + i]; sm.a[tg][2] = w * base[3 * k + i];
+                const double wk = escale ? w * escale[q] : w;   // R8b: the stiffness weight carries the point's modulus scale
+                sm.a[tg][0] = wk * base[k + i]; sm.a[tg][1] = wk * base[2 * k + i]; sm.a[tg][2] = wk * base[3 * k + i];
                 sm.qbase[tg] = base;
                 if constexpr (MASKED) {
                     const unsigned* mw = mrow + (p - pa) * mstep;
@@ -286,7 +287,7 @@ __global__ void __launch_bounds__(256)
 accumulate_generic_kernel(int64_t N, int k, int Lcap, const int64_t* __restrict__ inc_ptr,
                           const int32_t* __restrict__ inc_q, const uint8_t* __restrict__ inc_j,
                           const int32_t* __restrict__ support, const double* __restrict__ stage,
-                          const double* __restrict__ qw, const int64_t* __restrict__ brow_ptr,
+                          const double* __restrict__ qw, const double* __restrict__ escale, const int64_t* __restrict__ brow_ptr,
                           const int32_t* __restrict__ bcol, double lambda, double mu, double bx, double by,
                           double bz, double* __restrict__ vals, double* __restrict__ f) {
     extern __shared__ double smem_d[];
@@ -308,7 +309,8 @@ accumulate_generic_kernel(int64_t N, int k, int Lcap, const int64_t* __restrict_
             const int i = inc_j[p];
             const double w = qw[q];
             const double* st = stage + q * 4 * (int64_t)k;
-            const double wgx = w * st[k + i], wgy = w * st[2 * k + i], wgz = w * st[3 * k + i];
+            const double wk = escale ? w * escale[q] : w;
+            const double wgx = wk * st[k + i], wgy = wk * st[2 * k + i], wgz = wk * st[3 * k + i];
             fI += w * st[i];
             const int32_t* sp = support + q * k;
             for (int j = lane; j < k; j += 32) {
@@ -452,7 +454,7 @@ static int accumulate_generic(rpim_ctx* ctx, const double* d_qw, double lambda, 
     int64_t blocks = (ctx->N + warps - 1) / warps;
     blocks = std::min<int64_t>(blocks, 148LL * per_sm * 8);
     accumulate_generic_kernel<<<(unsigned)blocks, warps * 32, smem, ctx->stream>>>(
-        ctx->N, ctx->k, Lcap, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_support, ctx->d_stage, d_qw,
+        ctx->N, ctx->k, Lcap, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_support, ctx->d_stage, d_qw, ctx->d_escale,
         ctx->d_brow_ptr, ctx->d_bcol, lambda, mu, body[0], body[1], body[2], d_vals, d_f);
     KERNEL_CHECK(ctx);
     return RPIM_OK;
@@ -488,7 +490,7 @@ int launch_reduce_rows_m(rpim_ctx* ctx, const double* d_qw, double lambda, doubl
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_ROW_TICKET, 0, sizeof(long long), ctx->stream));
     blocks = std::min<int64_t>(blocks, (int64_t)sms * per_sm);
     kern<<<(unsigned)blocks, NWARP * ROWS * 32, smem, ctx->stream>>>(
-        ctx->N, ctx->k, nbg, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_support, ctx->d_stage, d_qw,
+        ctx->N, ctx->k, nbg, ctx->d_inc_ptr, ctx->d_inc_q, ctx->d_inc_j, ctx->d_support, ctx->d_stage, d_qw, ctx->d_escale,
         ctx->d_brow_ptr, ctx->d_bcol, ctx->d_mask_ptr, ctx->d_masks, ctx->mask_stride,
         (unsigned long long*)(ctx->d_flags + FLAG_ROW_TICKET), lambda, mu, body[0], body[1], body[2], d_vals, d_f);
     KERNEL_CHECK(ctx);

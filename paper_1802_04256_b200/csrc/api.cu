@@ -95,6 +95,13 @@ int rpim_set_reduction(rpim_ctx* ctx, int mode) {
     return RPIM_OK;
 }
 
+int rpim_set_modulus_scale(rpim_ctx* ctx, const double* d_escale) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    if (!ctx->have_pattern) RPIM_FAIL(ctx, RPIM_ERR_STATE, "rpim_set_modulus_scale before rpim_build_pattern");
+    ctx->d_escale = d_escale;
+    return RPIM_OK;
+}
+
 int rpim_reduction_used(const rpim_ctx* ctx) { return ctx && ctx->have_pattern ? (ctx->have_tiles ? 2 : 1) : 0; }
 
 int rpim_reduction_params(const rpim_ctx* ctx, int out[10]) {
@@ -126,6 +133,7 @@ int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const do
     ws_free(ctx, &ctx->d_stage);
     ws_free(ctx, &ctx->d_singular);
     ctx->d_nodes = d_nodes; ctx->d_qpts = d_qpts; ctx->N = N; ctx->Nq = Nq; ctx->k = k;
+    ctx->d_escale = nullptr;
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags, 0, NUM_FLAGS * sizeof(long long), st));
     int rc;
     if ((rc = ws_alloc(ctx, &ctx->d_support, Nq * k))) return rc;

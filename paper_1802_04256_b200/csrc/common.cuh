@@ -111,6 +111,7 @@ struct rpim_ctx {
     double* d_stage = nullptr;
     uint8_t* d_singular = nullptr;   // Nq
     ShapeParams sp{};
+    const double* d_escale = nullptr;   // optional per-point modulus scale (caller-owned), R8b
     bool have_sp = false;
 
     // misc

@@ -75,11 +75,14 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, i
 }
 
 // quadrature weights of every group into the group's record (once per rpim_assemble: the weights are its input)
+// (times the point's modulus scale of DESIGN.md R8b when there is one: the record's weights only feed the stiffness)
 __global__ void panel_weights_kernel(int64_t Nq, int64_t G, unsigned meta_bytes, unsigned off_w, const double* __restrict__ qw,
-                                     unsigned char* __restrict__ gmeta) {
+                                     const double* __restrict__ escale, unsigned char* __restrict__ gmeta) {
     const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= G * GB) return;
-    reinterpret_cast<double*>(gmeta + (q / GB) * meta_bytes + off_w)[q % GB] = q < Nq ? qw[q] : 0.0;
+    double w = 0.0;
+    if (q < Nq) w = escale ? qw[q] * escale[q] : qw[q];
+    reinterpret_cast<double*>(gmeta + (q / GB) * meta_bytes + off_w)[q % GB] = w;
 }
 
 // R = block rows per consumer warp (2: a row pair shares the gradient loads; 1: twice the warps), RP = row groups
@@ -441,7 +444,7 @@ int rpim_stage_accumulate_panels(rpim_ctx* ctx, const double* d_qw, double lambd
         A.grad_only = 1;
     }
     const unsigned meta = rpim_panel_meta_bytes(ctx->tg_C);
-    panel_weights_kernel<<<(unsigned)((G * GB + 255) / 256), 256, 0, ctx->stream>>>(ctx->Nq, G, meta, 32u * ctx->tg_C * 12u, d_qw, ctx->d_gmeta);
+    panel_weights_kernel<<<(unsigned)((G * GB + 255) / 256), 256, 0, ctx->stream>>>(ctx->Nq, G, meta, 32u * ctx->tg_C * 12u, d_qw, ctx->d_escale, ctx->d_gmeta);
     KERNEL_CHECK(ctx);
     const int wpb = 8;
     load_rows_kernel<<<(unsigned)((ctx->N + wpb - 1) / wpb), wpb * 32, 0, ctx->stream>>>(

@@ -225,7 +225,7 @@ norm2_kernel(int64_t n, const double* __restrict__ v, double* __restrict__ part)
 // sigma (Voigt xx yy zz xy yz zx) = D eps, eps = sum_I B_I u_I with the staged gradients; one warp per point
 __global__ void __launch_bounds__(SV_THREADS)
 stress_kernel(int64_t Nq, int k, const int32_t* __restrict__ support, const double* __restrict__ stage,
-              const double* __restrict__ u, double lambda, double mu, double* __restrict__ sigma) {
+              const double* __restrict__ u, const double* __restrict__ escale, double lambda0, double mu0, double* __restrict__ sigma) {
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int64_t q = (int64_t)blockIdx.x * (SV_THREADS / 32) + wid; q < Nq; q += (int64_t)gridDim.x * (SV_THREADS / 32)) {
         double e[6] = {0, 0, 0, 0, 0, 0};   // exx eyy ezz gxy gyz gzx (engineering shear)
@@ -246,6 +246,8 @@ stress_kernel(int64_t Nq, int k, const int32_t* __restrict__ support, const doub
 #pragma unroll
             for (int d = 16; d > 0; d >>= 1) e[c] += __shfl_xor_sync(0xffffffffu, e[c], d);
         if (lane == 0) {
+            const double sc = escale ? escale[q] : 1.0;   // R8b: the point's modulus scale
+            const double lambda = escale ? lambda0 * sc : lambda0, mu = escale ? mu0 * sc : mu0;
             const double tr = (e[0] + e[1]) + e[2];
             double* s = sigma + 6 * q;
             s[0] = fma(2.0 * mu, e[0], lambda * tr);
@@ -379,7 +381,7 @@ int rpim_recover_stress(rpim_ctx* ctx, const double* d_u, double E, double nu, d
     const double lambda = E * nu / ((1.0 + nu) * (1.0 - 2.0 * nu));
     const double mu = E / (2.0 * (1.0 + nu));
     const unsigned nb = (unsigned)std::min<int64_t>((ctx->Nq + 7) / 8, 148 * 16);
-    stress_kernel<<<nb, SV_THREADS, 0, ctx->stream>>>(ctx->Nq, ctx->k, ctx->d_support, ctx->d_stage, d_u, lambda, mu,
+    stress_kernel<<<nb, SV_THREADS, 0, ctx->stream>>>(ctx->Nq, ctx->k, ctx->d_support, ctx->d_stage, d_u, ctx->d_escale, lambda, mu,
                                                       d_sigma);
     KERNEL_CHECK(ctx);
     return RPIM_OK;

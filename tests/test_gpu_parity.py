@@ -363,3 +363,50 @@ def test_graded_density_supports_and_pattern():
         assert np.array_equal(d_rp.cpu().numpy(), rp_o) and np.array_equal(d_ci.cpu().numpy(), ci_o)
     finally:
         ctx.close()
+
+
+@pytest.mark.parametrize("reduction", [1, 2])
+def test_strata_modulus_scale(reduction):
+    """DESIGN.md R8b (part): per-point modulus scale E_q = E s_q with one Poisson ratio, both
+    reduction kernels, against the oracle; the loads do not change; rpim_recover_stress scales with s_q; switching
+    the scale off restores the unscaled matrix bit for bit."""
+    import torch
+    import oracle
+    import paper_1802_04256_b200 as rp
+    w = workloads.make_block("strata", 9, 8, 7, 1.0, 2, 30, 5e9, 0.3, jitter=0.3, seed=41, body=(10.0, -20.0, -2.5e4))
+    rng = np.random.default_rng(8)
+    esc = np.where(w.qpts[:, 2] < 3.0, 4.0, 0.5) * rng.uniform(0.9, 1.1, w.Nq)
+    s = oracle.knn(w.nodes, w.qpts, w.k, "grid")
+    rpo, cio = oracle.pattern(s, w.N)
+    vo, fo, _ = oracle.assemble(w.nodes, w.qpts, w.qw, s, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, rpo, cio, escale=esc)
+    rows = np.repeat(np.arange(3 * w.N), np.diff(rpo))
+    km = np.abs(vo[rows == cio]).max()
+    dev = torch.device("cuda:0")
+    ctx = rp.Context(0)
+    try:
+        ctx.set_reduction(reduction)
+        d_n, d_q, d_w = (torch.from_numpy(a).to(dev) for a in (w.nodes, w.qpts, w.qw))
+        nnz, bits = ctx.build_pattern(d_n, d_q, w.k, 64)
+        assert ctx.reduction_used() == reduction and nnz == rpo[-1]
+        d_vals = torch.empty(nnz, dtype=torch.float64, device=dev)
+        d_f = torch.empty(3 * w.N, dtype=torch.float64, device=dev)
+        ctx.assemble(d_w, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f)
+        v_plain, f_plain = d_vals.cpu().numpy().copy(), d_f.cpu().numpy().copy()
+        d_e = torch.from_numpy(esc).to(dev)
+        ctx.set_modulus_scale(d_e)
+        ctx.assemble(d_w, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f)
+        assert np.abs(d_vals.cpu().numpy() - vo).max() <= TOL * km
+        assert np.array_equal(d_f.cpu().numpy(), f_plain) and np.abs(f_plain - fo).max() <= TOL * np.abs(fo).max()
+        # stresses: sigma(s) = s_q * sigma(1) for the same displacement field
+        d_u = torch.from_numpy(rng.uniform(-1e-3, 1e-3, 3 * w.N)).to(dev)
+        d_s1 = torch.empty((w.Nq, 6), dtype=torch.float64, device=dev)
+        d_s0 = torch.empty_like(d_s1)
+        ctx.recover_stress(d_u, w.E, w.nu, d_s1)
+        ctx.set_modulus_scale(None)
+        ctx.recover_stress(d_u, w.E, w.nu, d_s0)
+        s0, s1 = d_s0.cpu().numpy(), d_s1.cpu().numpy()
+        assert np.abs(s1 - esc[:, None] * s0).max() <= 1e-12 * np.abs(s1).max()
+        ctx.assemble(d_w, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f)
+        assert np.array_equal(d_vals.cpu().numpy(), v_plain)
+    finally:
+        ctx.close()

@@ -397,3 +397,41 @@ def test_other_multiquadric_exponents(q, alpha_c, dense_tol):
     pr, dr = oracle.shape_dense_ref(w.nodes, pts, s, w.alpha_c, w.d_c, w.q)
     assert np.abs(phi - pr).max() / np.abs(pr).max() < dense_tol
     assert np.abs(dphi - dr).max() / np.abs(dr).max() < dense_tol
+
+
+# ------------------------------------------------------------------ R8b: strata with one Poisson ratio (per-point modulus scale)
+def test_modulus_scale_is_linear_and_keeps_the_invariants():
+    """K(s) = sum_q s_q K_q: exact scaling by a power of two, additivity in s, symmetry and the rigid-body null
+    space for any s >= 0; the loads do not depend on s; a two-layer bar equals the sum of its layers' matrices."""
+    w = workloads.make_block("strata", 7, 6, 6, 1.0, 2, 30, 5e9, 0.3, jitter=0.3, seed=3, body=(1.0, -2.0, -3.0))
+    s = oracle.knn(w.nodes, w.qpts, w.k, "grid")
+    rp, ci = oracle.pattern(s, w.N)
+    args = (w.nodes, w.qpts, w.qw, s, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, rp, ci)
+    v0, f0, _ = oracle.assemble(*args)
+    v1, f1, _ = oracle.assemble(*args, escale=np.ones(w.Nq))
+    v2, f2, _ = oracle.assemble(*args, escale=np.full(w.Nq, 2.0))
+    assert np.array_equal(v0, v1) and np.array_equal(f0, f1)
+    assert np.array_equal(2.0 * v0, v2) and np.array_equal(f0, f2)
+    rng = np.random.default_rng(4)
+    sa, sb = rng.uniform(0.2, 3.0, w.Nq), rng.uniform(0.2, 3.0, w.Nq)
+    va, _, _ = oracle.assemble(*args, escale=sa)
+    vb, _, _ = oracle.assemble(*args, escale=sb)
+    vab, fab, _ = oracle.assemble(*args, escale=sa + sb)
+    rows = np.repeat(np.arange(3 * w.N), np.diff(rp))
+    km = np.abs(vab[rows == ci]).max()
+    assert np.abs(va + vb - vab).max() <= 1e-14 * km and np.array_equal(fab, f0)
+    import scipy.sparse as sp
+    K = sp.csr_matrix((va, ci, rp), shape=(3 * w.N, 3 * w.N))
+    assert abs(K - K.T).max() <= 1e-15 * km
+    r = w.nodes - w.nodes.mean(0)
+    for c in range(3):
+        t = np.zeros((w.N, 3)); t[:, c] = 1.0
+        e = np.zeros(3); e[c] = 1.0
+        for m in (t, np.cross(e, r)):
+            assert np.abs(K @ m.reshape(-1)).max() <= 1e-12 * km * np.abs(m).max()
+    # two layers: stiff below z = 2.5, soft above
+    lay = np.where(w.qpts[:, 2] < 2.5, 4.0, 0.5)
+    vl, _, _ = oracle.assemble(*args, escale=lay)
+    vlo, _, _ = oracle.assemble(*args, escale=np.where(lay == 4.0, 1.0, 0.0))
+    vhi, _, _ = oracle.assemble(*args, escale=np.where(lay == 0.5, 1.0, 0.0))
+    assert np.abs(4.0 * vlo + 0.5 * vhi - vl).max() <= 1e-14 * km

@@ -155,6 +155,35 @@ int rpim_apply_penalty(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* 
                        const double* d_u_bar, int64_t m, double alpha, int alpha_is_relative,
                        double* d_vals, double* d_f, double* out_alpha_used);
 
+/* Stage 2 without any device allocation: same arguments, same checks and bitwise the same K, f and alpha_used as
+ * rpim_apply_penalty, for callers that cannot let the library reach cudaMalloc at this point of their program:
+ *   - a solver that has already handed (nearly) all of the GPU's memory to its own pool -- at the `stress`
+ *     configuration K, col_idx and the staged shape functions take 174 of 180 GB, and a late cudaMalloc can fail;
+ *   - a time-stepping or serving loop that runs other streams on the same device: cudaMalloc and cudaFree
+ *     synchronise the whole device and would stall them;
+ *   - several solver instances sharing one GPU under a device-memory budget that has to be accounted for byte by
+ *     byte: what this call uses is fixed and known when the library is built.
+ * rpim_apply_penalty takes its scratch memory (partial maxima of the diagonal, one bit per node for the
+ * duplicate check, a counter) from the context's workspace and so may allocate; this call keeps the same scratch
+ * in a fixed array inside the library image (about 0.5 MiB, held by every GPU that loads librpim until the
+ * process exits) and calls no cudaMalloc, cudaFree or allocating library routine.
+ *   Limit: at most RPIM_STATIC_PENALTY_MAX_NODES nodes in the context's pattern (rpim_apply_penalty_static_max_nodes
+ *     returns the same number); a larger problem is refused with RPIM_ERR_CAPACITY and nothing is touched.  The
+ *     length m of the boundary list is not limited.
+ *   First call on a device: looks up the array's device address (once per device, with that device current) and
+ *     may make the CUDA runtime load the library's kernels; make that first call during start-up, before any
+ *     stream capture begins.
+ *   Sharing: all contexts on a device use the one array, and it keeps the previous call's contents (the call
+ *     clears what it needs to find at zero).  Two calls that overlap on the GPU -- different contexts or streams
+ *     of one device -- race on it and give wrong results: serialise them.  Calls on different devices are
+ *     independent.
+ * Synchronises the stream once, like rpim_apply_penalty. */
+#define RPIM_STATIC_PENALTY_MAX_NODES 4194304
+int rpim_apply_penalty_static(rpim_ctx* ctx, const int64_t* d_bc_nodes, const uint8_t* d_bc_mask,
+                              const double* d_u_bar, int64_t m, double alpha, int alpha_is_relative,
+                              double* d_vals, double* d_f, double* out_alpha_used);
+int64_t rpim_apply_penalty_static_max_nodes(void);
+
 /* Stage 3 ("solve the system ... then the stresses").
  *
  * rpim_matvec: y = K x with K in the layout rpim_assemble / rpim_apply_penalty leave in d_vals (the

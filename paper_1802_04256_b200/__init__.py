@@ -15,6 +15,8 @@ from .binding import (  # noqa: F401
     rpim_assemble,
     rpim_add_point_loads,
     rpim_apply_penalty,
+    rpim_apply_penalty_static,
+    rpim_apply_penalty_static_max_nodes,
     rpim_get_shape,
     rpim_host_pattern,
     rpim_host_assemble,

@@ -19,6 +19,7 @@ EXPORTED_SYMBOLS = (
     "rpim_host_pattern", "rpim_host_assemble", "rpim_last_phase_ms", "rpim_phase_totals", "rpim_launch_count",
     "rpim_matvec", "rpim_solve_pcg", "rpim_recover_stress", "rpim_set_reduction", "rpim_reduction_used",
     "rpim_probe_fp64", "rpim_update_nodes", "rpim_reduction_params", "rpim_set_modulus_scale",
+    "rpim_apply_penalty_static", "rpim_apply_penalty_static_max_nodes",
 )
 
 
@@ -59,6 +60,9 @@ def _load():
     lib.rpim_assemble.argtypes = [vp, vp, dbl, dbl, dbl, dbl, dbl, C.POINTER(dbl), vp, vp, C.POINTER(i64)]
     lib.rpim_add_point_loads.argtypes = [vp, vp, vp, vp, i64, vp]
     lib.rpim_apply_penalty.argtypes = [vp, vp, vp, vp, i64, dbl, C.c_int, vp, vp, C.POINTER(dbl)]
+    lib.rpim_apply_penalty_static.argtypes = [vp, vp, vp, vp, i64, dbl, C.c_int, vp, vp, C.POINTER(dbl)]
+    lib.rpim_apply_penalty_static_max_nodes.argtypes = []
+    lib.rpim_apply_penalty_static_max_nodes.restype = i64
     lib.rpim_get_shape.argtypes = [vp, vp, vp, vp]
     lib.rpim_host_pattern.argtypes = [vp, vp, i64, vp, i64, C.c_int, C.c_int, C.POINTER(i64), C.POINTER(C.c_int)]
     lib.rpim_host_assemble.argtypes = [vp, vp, dbl, dbl, dbl, dbl, dbl, C.POINTER(dbl), vp, vp, vp, i64, dbl,
@@ -229,6 +233,25 @@ def rpim_apply_penalty(ctx, d_bc_nodes, d_bc_mask, d_u_bar, alpha, alpha_is_rela
     return float(used.value)
 
 
+def rpim_apply_penalty_static(ctx, d_bc_nodes, d_bc_mask, d_u_bar, alpha, alpha_is_relative, d_vals, d_f):
+    """rpim_apply_penalty for callers that must not allocate device memory (see include/rpim.h): same arguments
+    and results, scratch memory in a fixed array inside the library, at most
+    ``rpim_apply_penalty_static_max_nodes()`` nodes.  Returns alpha_used."""
+    import torch
+    used = C.c_double(0.0)
+    m = 0 if d_bc_nodes is None else d_bc_nodes.shape[0]
+    rc = _load().rpim_apply_penalty_static(ctx, _dptr(d_bc_nodes, torch.int64), _dptr(d_bc_mask, torch.uint8),
+                                           _dptr(d_u_bar, torch.float64), m, float(alpha),
+                                           int(bool(alpha_is_relative)), _dptr(d_vals, torch.float64),
+                                           _dptr(d_f, torch.float64), C.byref(used))
+    _check(ctx, rc)
+    return float(used.value)
+
+
+def rpim_apply_penalty_static_max_nodes() -> int:
+    return int(_load().rpim_apply_penalty_static_max_nodes())
+
+
 def rpim_get_shape(ctx, d_phi=None, d_dphi=None, d_singular=None):
     _check(ctx, _load().rpim_get_shape(ctx, _dptr(d_phi), _dptr(d_dphi), _dptr(d_singular)))
 
@@ -315,6 +338,9 @@ class Context:
 
     def apply_penalty(self, d_bc_nodes, d_bc_mask, d_u_bar, alpha, relative, d_vals, d_f):
         return rpim_apply_penalty(self.ctx, d_bc_nodes, d_bc_mask, d_u_bar, alpha, relative, d_vals, d_f)
+
+    def apply_penalty_static(self, d_bc_nodes, d_bc_mask, d_u_bar, alpha, relative, d_vals, d_f):
+        return rpim_apply_penalty_static(self.ctx, d_bc_nodes, d_bc_mask, d_u_bar, alpha, relative, d_vals, d_f)
 
     def get_shape(self, d_phi=None, d_dphi=None, d_singular=None):
         return rpim_get_shape(self.ctx, d_phi, d_dphi, d_singular)

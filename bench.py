@@ -216,6 +216,32 @@ def max_over_ranks(ms_local: float, world: int, device=None) -> float:
     return float(t.item())
 
 
+def rank_allreduce(world: int, device=None):
+    """allreduce(array, "min" | "max") over the ranks for partition.verify_shard (None for a single rank)."""
+    if world <= 1:
+        return None
+    import torch
+    import torch.distributed as dist
+
+    def red(a, op):
+        t = torch.from_numpy(np.ascontiguousarray(a))
+        t = t.to(device) if device is not None else t
+        dist.all_reduce(t, op=dist.ReduceOp.MIN if op == "min" else dist.ReduceOp.MAX)
+        return t.cpu().numpy()
+    return red
+
+
+def check_shard(shard, w_local, support_local, nq_job: int, world: int, device=None):
+    """--shard is only valid when the halo bounds every support radius on every rank and every point of the domain
+    is taken by some rank (partition.py); otherwise owned rows are silently incomplete: refuse to time that."""
+    from paper_1802_04256_b200 import partition as pt
+    ok, missing = pt.verify_shard(shard, w_local.nodes, w_local.qpts, support_local, nq_job, rank_allreduce(world, device))
+    if not ok or missing:
+        raise RuntimeError(f"--shard: halo {shard.halo:.4g} is not valid for this cloud (support radius bound holds on "
+                           f"every rank: {ok}; quadrature points taken by no rank: {missing}); owned rows would be "
+                           "incomplete -- use a larger halo")
+
+
 def job_value(points_per_rank: int, world: int, ms_step: float) -> float:
     """Whole-job throughput: the quadrature points all ranks processed per second."""
     return world * points_per_rank / (ms_step * 1e-3)
@@ -274,6 +300,11 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
 
     # first pass sizes the outputs (pattern is data dependent)
     nnz, bits = ctx.build_pattern(d_nodes, d_qpts, w.k, w.index_bits)
+    if shard is not None:
+        d_sup = torch.empty((w.Nq, w.k), dtype=torch.int32, device=dev)
+        ctx.get_pattern(None, None, d_sup)
+        check_shard(shard, w, d_sup.cpu().numpy(), nq_job, world, dev)
+        del d_sup
     idt = torch.int32 if bits == 32 else torch.int64
     d_rp = torch.empty(3 * w.N + 1, dtype=idt, device=dev)
     d_ci = torch.empty(nnz, dtype=idt, device=dev)

@@ -11,9 +11,11 @@ Row-owner partition with redundant halo work and NO data-path exchange:
     nodes of a taken point among the taken nodes are its k nearest nodes among ALL nodes.  The owned rows of the
     rank's sub-problem are then complete and -- supports ascending, points in ascending order -- bit-identical to
     the same rows of the undivided problem; the rows of halo nodes are partial and are discarded;
-  * the bound is VERIFIED after the support search (`support_radius_ok`): on the sub-cloud the k-th neighbour
-    distance can only be larger than the true one, so `max <= halo` on every rank proves the premise for every
-    point (each point is taken by at least one rank);
+  * the bound has to be VERIFIED after the support search, and `verify_shard` does it (the tests and
+    `bench.py --shard` call it and refuse to go on otherwise): on the sub-cloud the k-th neighbour distance can
+    only be larger than the true one, so `max <= halo` on every rank (`support_radius_ok`) proves the premise
+    for every point that some rank has taken -- and that every point IS taken by at least one rank is checked
+    too, since a point farther than `halo` from every slab's box would otherwise be dropped silently;
   * the only collective of the path is allreduce(max) of one double: alpha = penalty * max_i K_ii.  A halo row's
     partial diagonal never exceeds its complete value (every contribution to a diagonal entry is >= 0), which
     the owning rank holds, so max over ranks of the local maxima is the global maximum.
@@ -74,6 +76,23 @@ def support_radius_ok(sub_nodes: np.ndarray, sub_pts: np.ndarray, support_local:
     """max over the taken points of the distance to the farthest node of the support found on the sub-cloud."""
     d = sub_nodes[support_local] - sub_pts[:, None, :]
     return bool(np.sqrt((d * d).sum(axis=2)).max() <= halo)
+
+
+def verify_shard(shard: Shard, sub_nodes: np.ndarray, sub_pts: np.ndarray, support_local: np.ndarray, nq_total: int,
+                 allreduce=None):
+    """The two premises of the docstring above, checked after the support search of every rank: (1) `halo` bounds
+    the support radius found on the sub-cloud (`support_radius_ok`) on EVERY rank, (2) every quadrature point of
+    the domain is taken by at least one rank.  `allreduce(array, op)` with op in {"min", "max"} reduces a float64
+    / uint8 numpy array over the ranks and returns the result (None: single rank).  Returns
+    (all ranks' halo bound holds, number of points no rank has taken); a caller must not use the owned rows
+    unless the result is (True, 0)."""
+    ok = np.array([1.0 if support_radius_ok(sub_nodes, sub_pts, support_local, shard.halo) else 0.0])
+    taken = np.zeros(nq_total, dtype=np.uint8)
+    taken[shard.point_ids] = 1
+    if allreduce is not None:
+        ok = allreduce(ok, "min")
+        taken = allreduce(taken, "max")
+    return bool(ok[0] == 1.0), int(nq_total - int(taken.sum(dtype=np.int64)))
 
 
 def local_bc(shard: Shard, bc_nodes: np.ndarray, bc_mask: np.ndarray, bc_ubar: np.ndarray):

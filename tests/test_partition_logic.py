@@ -44,9 +44,16 @@ def _worker(rank, world, port, out_dir):
         w = _problem()
         sh = pt.make_shard(w.nodes, w.qpts, w.k, rank, world)
         nodes, pts, s, rp, ci, vals, f = _rank_assemble(w, sh)
-        ok = pt.support_radius_ok(nodes, pts, s, sh.halo)
+        import bench
+        ok, missing = pt.verify_shard(sh, nodes, pts, s, w.Nq, bench.rank_allreduce(world))   # as bench.py --shard does
+        assert missing == 0
         flag = torch.tensor([1.0 if ok else 0.0], dtype=torch.float64)
-        dist.all_reduce(flag, op=dist.ReduceOp.MIN)          # every rank must confirm the halo bound
+        # points that no rank takes (here: every rank forgets every other one of its own; on this small block the
+        # halos make both ranks take all points, so the odd ones are lost) are seen by EVERY rank
+        cut = pt.Shard(sh.rank, sh.world, sh.row_lo, sh.row_hi, sh.node_ids, sh.point_ids[::2], sh.own_lo, sh.own_hi,
+                       sh.halo)
+        ok2, missing2 = pt.verify_shard(cut, nodes, pts[::2], s[::2], w.Nq, bench.rank_allreduce(world))
+        assert ok2 and missing2 > 0
         rows = np.repeat(np.arange(len(rp) - 1), np.diff(rp))
         local_max = float(vals[rows == ci].max())             # over ALL local rows, partial halo rows included
         t = torch.tensor([local_max], dtype=torch.float64)
@@ -110,6 +117,18 @@ def test_partition_degenerates_gracefully():
     nodes, pts = w.nodes[sh.node_ids], w.qpts[sh.point_ids]
     s = oracle.knn(np.ascontiguousarray(nodes), np.ascontiguousarray(pts), w.k, "grid")
     assert not pt.support_radius_ok(nodes, pts, s, sh.halo)
+    # bench.py --shard refuses to time such a partition: the halo bound fails, and with so small a halo the two
+    # ranks together do not even take every point
+    import bench
+    ok, missing = pt.verify_shard(sh, nodes, pts, s, w.Nq)
+    assert not ok and missing > 0
+    import pytest
+    with pytest.raises(RuntimeError, match="halo"):
+        import dataclasses
+        bench.check_shard(sh, dataclasses.replace(w, nodes=nodes, qpts=pts), s, w.Nq, 1)
+    good = pt.make_shard(w.nodes, w.qpts, w.k, 0, 1)
+    s_all = oracle.knn(w.nodes, w.qpts, w.k, "grid")
+    assert pt.verify_shard(good, w.nodes, w.qpts, s_all, w.Nq) == (True, 0)
 
 
 def test_bench_shard_workload_covers_the_domain_once():

@@ -80,6 +80,21 @@ int rpim_set_reduction(rpim_ctx* ctx, int mode);
 int rpim_reduction_used(const rpim_ctx* ctx);
 int rpim_reduction_params(const rpim_ctx* ctx, int out[10]);
 
+/* Tuning / test knob: force parts of the panel kernel's launch shape instead of the automatic choice (every
+ * argument: 0 = automatic).  The result does not depend on it -- the order of summation per matrix entry is the
+ * same for every shape -- only the speed does.  The library reads no environment variable.
+ *   rows_per_tile    2, 4, 6 or 8 block rows per CTA tile (ignored when a row has more than 1024 upper columns)
+ *   warps_per_group  1..4 consumer warps per row group (at most 3 with one row per group)
+ *   rows_per_group   1 or 2 block rows per consumer warp group
+ *   ring_stages      2..8 stages of the group ring
+ *   staging          1 = gradient rows by a 2-D tensor copy (needs an even k <= 84), 2 = whole staged rows by a plain bulk copy
+ *   tile_desc        1 = tile descriptors by one warp per tile, 2 = by one thread per tile
+ * A shape that does not fit the shared memory falls back to the row-owner kernel (rpim_reduction_used tells).
+ * Out-of-range values give RPIM_ERR_INVALID_ARG and change nothing.  Takes effect at the next
+ * rpim_build_pattern / rpim_update_nodes; rpim_reduction_params reports the shape in use. */
+int rpim_set_panel_shape(rpim_ctx* ctx, int rows_per_tile, int warps_per_group, int rows_per_group, int ring_stages,
+                         int staging, int tile_desc);
+
 /* Stage 0 (R1, R2; hot-path steps a1, a2): exact k-nearest-neighbour supports on a
  * uniform cell grid and the CSR pattern of the 3N x 3N stiffness matrix.
  *   d_nodes  N x 3 field-node coordinates        d_qpts  Nq x 3 quadrature points
@@ -197,7 +212,8 @@ int64_t rpim_apply_penalty_static_max_nodes(void);
  * be NULL) report what was reached, out_rel_resid being the TRUE ||f - K u||_2 / ||f||_2 of the returned
  * iterate, recomputed with one more product -- not converging is not an error.  If p^T K p <= 0 or is not
  * finite (K is not positive definite: singular points, unconstrained components) the iteration stops at
- * the next look and RPIM_ERR_BREAKDOWN is returned, outputs filled.  f = 0 returns u = 0.  All reductions
+ * the next look and RPIM_ERR_BREAKDOWN is returned, outputs filled.  f = 0 returns u = 0; a load vector that is
+ * not finite (NaN, Inf) also returns RPIM_ERR_BREAKDOWN, with d_u untouched.  All reductions
  * have a fixed order: the iterates are bitwise reproducible.  Synchronises the stream.
  *
  * rpim_recover_stress: sigma = D B u at every quadrature point of the last rpim_assemble (its staged

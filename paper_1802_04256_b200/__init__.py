@@ -24,6 +24,7 @@ from .binding import (  # noqa: F401
     rpim_phase_totals,
     rpim_launch_count,
     rpim_matvec,
+    rpim_set_panel_shape,
     rpim_solve_pcg,
     rpim_recover_stress,
     rpim_workspace_bytes,

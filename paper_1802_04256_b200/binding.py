@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = (
     "rpim_host_pattern", "rpim_host_assemble", "rpim_last_phase_ms", "rpim_phase_totals", "rpim_launch_count",
     "rpim_matvec", "rpim_solve_pcg", "rpim_recover_stress", "rpim_set_reduction", "rpim_reduction_used",
     "rpim_probe_fp64", "rpim_update_nodes", "rpim_reduction_params", "rpim_set_modulus_scale",
-    "rpim_apply_penalty_static", "rpim_apply_penalty_static_max_nodes",
+    "rpim_apply_penalty_static", "rpim_apply_penalty_static_max_nodes", "rpim_set_panel_shape",
 )
 
 
@@ -77,6 +77,7 @@ def _load():
     lib.rpim_reduction_used.argtypes = [vp]
     lib.rpim_reduction_params.argtypes = [vp, C.POINTER(C.c_int)]
     lib.rpim_set_modulus_scale.argtypes = [vp, vp]
+    lib.rpim_set_panel_shape.argtypes = [vp] + [C.c_int] * 6
     _lib = lib
     return lib
 
@@ -153,6 +154,13 @@ def rpim_probe_fp64(ctx):
 
 def rpim_set_reduction(ctx, mode: int):
     _check(ctx, _load().rpim_set_reduction(ctx, int(mode)))
+
+
+def rpim_set_panel_shape(ctx, rows_per_tile=0, warps_per_group=0, rows_per_group=0, ring_stages=0, staging=0,
+                         tile_desc=0):
+    """Force parts of the panel kernel's launch shape (0 = automatic); see include/rpim.h."""
+    _check(ctx, _load().rpim_set_panel_shape(ctx, int(rows_per_tile), int(warps_per_group), int(rows_per_group),
+                                             int(ring_stages), int(staging), int(tile_desc)))
 
 
 def rpim_reduction_used(ctx) -> int:
@@ -371,6 +379,9 @@ class Context:
 
     def set_reduction(self, mode):
         return rpim_set_reduction(self.ctx, mode)
+
+    def set_panel_shape(self, **shape):
+        return rpim_set_panel_shape(self.ctx, **shape)
 
     def reduction_used(self):
         return rpim_reduction_used(self.ctx)

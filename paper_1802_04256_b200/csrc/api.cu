@@ -95,6 +95,21 @@ int rpim_set_reduction(rpim_ctx* ctx, int mode) {
     return RPIM_OK;
 }
 
+int rpim_set_panel_shape(rpim_ctx* ctx, int rows_per_tile, int warps_per_group, int rows_per_group, int ring_stages,
+                         int staging, int tile_desc) {
+    if (!ctx) return RPIM_ERR_INVALID_ARG;
+    const bool ok = (rows_per_tile == 0 || (rows_per_tile >= 2 && rows_per_tile <= 8 && !(rows_per_tile & 1))) &&
+                    (warps_per_group >= 0 && warps_per_group <= 4) && (rows_per_group >= 0 && rows_per_group <= 2) &&
+                    (ring_stages == 0 || (ring_stages >= 2 && ring_stages <= 8)) && (staging >= 0 && staging <= 2) &&
+                    (tile_desc >= 0 && tile_desc <= 2);
+    if (!ok)
+        RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "rpim_set_panel_shape: rows_per_tile in {0,2,4,6,8}, warps_per_group 0..4, "
+                  "rows_per_group 0..2, ring_stages 0 or 2..8, staging 0..2, tile_desc 0..2");
+    ctx->ov_T = rows_per_tile; ctx->ov_CW = warps_per_group; ctx->ov_R = rows_per_group;
+    ctx->ov_nstage = ring_stages; ctx->ov_grad = staging; ctx->ov_tdesc = tile_desc;
+    return RPIM_OK;
+}
+
 int rpim_set_modulus_scale(rpim_ctx* ctx, const double* d_escale) {
     if (!ctx) return RPIM_ERR_INVALID_ARG;
     if (!ctx->have_pattern) RPIM_FAIL(ctx, RPIM_ERR_STATE, "rpim_set_modulus_scale before rpim_build_pattern");
@@ -198,10 +213,14 @@ int rpim_update_nodes(rpim_ctx* ctx, const double* d_nodes, const double* d_qpts
     if ((rc = rpim_stage_grid_refresh(ctx, &rebuild, &moved))) { ctx->have_pattern = false; return rc; }
     int32_t* d_new = nullptr;
     if ((rc = ws_alloc(ctx, &d_new, Nq * k))) { ctx->have_pattern = false; return rc; }
-    CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_flags + FLAG_KNN_CAP, 0, sizeof(long long), st));
-    if ((rc = rpim_stage_grid_knn(ctx, ctx->d_qpts, Nq, k, d_new, rebuild))) { ws_free(ctx, &d_new); ctx->have_pattern = false; return rc; }
+    // from here on the grid and d_nodes are the new ones: every failure gives d_new back and drops the pattern
+    auto drop = [&]() { ws_free(ctx, &d_new); ctx->have_pattern = false; };
+    cudaError_t e0 = cudaMemsetAsync(ctx->d_flags + FLAG_KNN_CAP, 0, sizeof(long long), st);
+    if (e0 != cudaSuccess) { drop(); RPIM_FAIL(ctx, RPIM_ERR_CUDA, "rpim_update_nodes: memset failed: %s", cudaGetErrorString(e0)); }
+    if ((rc = rpim_stage_grid_knn(ctx, ctx->d_qpts, Nq, k, d_new, rebuild))) { drop(); return rc; }
     unsigned long long* d_changed = (unsigned long long*)ctx->d_scratch;
-    CUDA_TRY(ctx, cudaMemsetAsync(d_changed, 0, sizeof(unsigned long long), st));
+    e0 = cudaMemsetAsync(d_changed, 0, sizeof(unsigned long long), st);
+    if (e0 != cudaSuccess) { drop(); RPIM_FAIL(ctx, RPIM_ERR_CUDA, "rpim_update_nodes: memset failed: %s", cudaGetErrorString(e0)); }
     support_diff_kernel<<<(unsigned)((Nq + 255) / 256), 256, 0, st>>>(ctx->d_support, d_new, Nq, k, d_changed);
     ctx->launches++;
     unsigned long long changed = 0;

@@ -96,6 +96,8 @@ struct rpim_ctx {
     int tg_CW = 0;                   // consumer warps per row group
     bool tg_grad_only = false;       // the groups' staged rows travel as a 2-D tensor copy of the gradient rows only
     int tg_R = 2;                    // block rows per row group (2: a pair shares the gradient loads; 1: twice the warps)
+    // rpim_set_panel_shape: forced launch shape of the panel reduction (0 = automatic), read by rpim_stage_tiles
+    int ov_T = 0, ov_CW = 0, ov_R = 0, ov_nstage = 0, ov_grad = 0 /*1 tensor copy, 2 plain*/, ov_tdesc = 0 /*1 warp, 2 thread*/;
     int max_ulen = 0;                // most upper block columns (diagonal included) of a row
     double tg_mean_union = 0.0;      // mean |U_g| of the last statistics pass
     int64_t ntiles = 0;

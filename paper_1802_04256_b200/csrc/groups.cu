@@ -336,11 +336,9 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
     // Launch shape of reduce_panels_kernel.  Measured on B200: one block row per consumer
     // warp group and two warps per group (13 warps at T = 6) beat row pairs with three warps (10 warps) by 7 % at
     // `stress`; the most rows per tile (8, 6, 4, 2) that leave room for a ring of five stages (else four, three),
-    // then the deepest ring (<= 8).  RPIM_PANEL_R / _CW / _T / _NSTAGE override (tuning and tests).
-    int CW = 2;
-    if (const char* e = getenv("RPIM_PANEL_CW")) { const int c = atoi(e); if (c >= 1 && c <= 4) CW = c; }
-    int R = 1;
-    if (const char* e = getenv("RPIM_PANEL_R")) { const int r = atoi(e); if (r == 1 || r == 2) R = r; }
+    // then the deepest ring (<= 8).  rpim_set_panel_shape overrides any of them (tuning and tests; validated there).
+    int CW = ctx->ov_CW ? ctx->ov_CW : 2;
+    int R = ctx->ov_R ? ctx->ov_R : 1;
     if (R == 1 && CW > 3) CW = 3;
     const unsigned budget = 227u * 1024u;
     // rows per tile and ring depth for one way of staging the groups' rows
@@ -352,10 +350,10 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
             for (int need = 5; need >= 3 && T == 0; --need)
                 for (int t = TMAX; t >= 2 && T == 0; t -= 2)
                     if (rpim_panel_smem(ctx->tg_C, CW, R, t, ctx->k, Ucap, need, grad_only).total <= budget) T = t;
-        if (const char* e = getenv("RPIM_PANEL_T")) { const int t = atoi(e); if (t >= 2 && t <= TMAX && !(t & 1)) T = t; }
+        if (ctx->ov_T && Ucap <= 1024) T = ctx->ov_T;   // (the row-length guard holds for a forced T as well)
         if (T == 0) return;
         for (nstage = 8; nstage > 2 && rpim_panel_smem(ctx->tg_C, CW, R, T, ctx->k, Ucap, nstage, grad_only).total > budget; --nstage) {}
-        if (const char* e = getenv("RPIM_PANEL_NSTAGE")) { const int n = atoi(e); if (n >= 2 && n <= 8) nstage = n; }
+        if (ctx->ov_nstage) nstage = ctx->ov_nstage;
         if (rpim_panel_smem(ctx->tg_C, CW, R, T, ctx->k, Ucap, nstage, grad_only).total > budget) T = 0;
     };
     // Whole staged rows by one plain bulk copy, or the gradient rows only by a 2-D tensor copy (three quarters of
@@ -369,8 +367,8 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
         choose(true, Tg, ng);
         if (Tg > T || (Tg == T && ng > nstage)) { T = Tg; nstage = ng; grad_only = true; }
     }
-    if (const char* e = getenv("RPIM_PANEL_GRAD_ONLY")) {
-        const bool want = atoi(e) != 0;
+    if (ctx->ov_grad) {
+        const bool want = ctx->ov_grad == 1;
         if (want != grad_only && (!want || rpim_panel_grad_only(ctx->k))) { grad_only = want; choose(grad_only, T, nstage); }
     }
     if (T == 0) { ctx->tg_C = 0; return RPIM_OK; }   // rows too long to keep two of them on chip
@@ -387,7 +385,7 @@ int rpim_stage_tiles(rpim_ctx* ctx) {
     const size_t td_smem_cnt = (size_t)TD_WARPS * TD_ITEMS * 8;                                  // the count pass keeps no descriptors
     const size_t td_smem = (size_t)TD_WARPS * (TD_ITEMS * 8 + TD_GROUPS * TD_DWMAX * 4);
     bool by_warp = ntiles <= 65536;
-    if (const char* e = getenv("RPIM_TILE_DESC")) by_warp = e[0] == 'w';   // "warp" / "thread": tests
+    if (ctx->ov_tdesc) by_warp = ctx->ov_tdesc == 1;   // rpim_set_panel_shape: tests
     if (by_warp) {
         CUDA_TRY(ctx, cudaFuncSetAttribute(tile_desc_warp_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)td_smem_cnt));
         CUDA_TRY(ctx, cudaFuncSetAttribute(tile_desc_warp_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)td_smem));

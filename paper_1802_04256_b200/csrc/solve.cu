@@ -315,7 +315,14 @@ int rpim_solve_pcg(rpim_ctx* ctx, const double* d_vals, const double* d_f, doubl
     int it = 0;
     double rel = 0.0;
     bool breakdown = false;
-    if (!(ff > 0.0)) {
+    if (!std::isfinite(ff)) {
+        // a NaN or Inf in the load vector is not "f = 0": report it instead of a converged solve (d_u untouched)
+        if (out_iters) *out_iters = 0;
+        if (out_rel_resid) *out_rel_resid = ff;
+        ctx->err = "rpim_solve_pcg: the load vector is not finite (||f||^2 is NaN or Inf)";
+        return fail(RPIM_ERR_BREAKDOWN);
+    }
+    if (ff == 0.0) {
         // f = 0: the solution of the definite system is u = 0, whatever the initial guess was
         if (cudaMemsetAsync(d_u, 0, (size_t)n * sizeof(double), st) != cudaSuccess) { ctx->err = "memset failed"; return fail(RPIM_ERR_CUDA); }
     } else {

@@ -5,12 +5,19 @@ Row-owner partition with redundant halo work and NO data-path exchange:
 
   * rank r owns the block rows (nodes) [N r / W, N (r+1) / W): contiguous id ranges, i.e. spatial slabs for a
     spatially coherent numbering;
-  * it takes every quadrature point within `halo` of the bounding box of its owned nodes, and every node within
-    2 * `halo` of that box.  If `halo` bounds the support radius (distance from a point to its k-th nearest node)
-    of every point, then (a) every point whose support touches an owned row is taken, and (b) the k nearest
-    nodes of a taken point among the taken nodes are its k nearest nodes among ALL nodes.  The owned rows of the
-    rank's sub-problem are then complete and -- supports ascending, points in ascending order -- bit-identical to
-    the same rows of the undivided problem; the rows of halo nodes are partial and are discarded;
+  * it takes every quadrature point within `halo` of the bounding box of its owned nodes -- in whole groups of 8
+    consecutive global ids, see below -- and every node within `halo` of the farthest taken point's distance
+    from that box (2 * `halo` when no group sticks out).  If `halo` bounds the support radius (distance from a
+    point to its k-th nearest node) of every point, then (a) every point whose support touches an owned row is
+    taken, and (b) the k nearest nodes of a taken point among the taken nodes are its k nearest nodes among ALL
+    nodes.  The owned rows of the rank's sub-problem are then complete; the rows of halo nodes are partial and
+    are discarded;
+  * rounding: with supports ascending and points in ascending order the row-owner kernel (and the oracle) add
+    a row's contributions point by point in the same order as on the undivided problem: owned rows are
+    bit-identical.  The panel kernel first sums the points of a group of 8 consecutive LOCAL ids in registers;
+    because points are taken in whole global groups (`make_shard(group=8)`), local groups are the undivided
+    problem's groups and its owned rows are bit-identical too (tests/test_gpu_sharded.py runs both kernels).
+    With `group=1` that kernel's owned rows agree only to rounding;
   * the bound has to be VERIFIED after the support search, and `verify_shard` does it (the tests and
     `bench.py --shard` call it and refuse to go on otherwise): on the sub-cloud the k-th neighbour distance can
     only be larger than the true one, so `max <= halo` on every rank (`support_radius_ok`) proves the premise
@@ -54,15 +61,35 @@ def halo_estimate(nodes: np.ndarray, k: int, safety: float = 2.2) -> float:
     return safety * (3.0 * k / (4.0 * np.pi)) ** (1.0 / 3.0) * h
 
 
-def make_shard(nodes: np.ndarray, qpts: np.ndarray, k: int, rank: int, world: int, halo: float | None = None) -> Shard:
-    N = nodes.shape[0]
+POINT_GROUP = 8   # the panel reduction sums the points of a group of 8 consecutive ids in registers first
+
+
+def _box_distance(x: np.ndarray, blo: np.ndarray, bhi: np.ndarray) -> np.ndarray:
+    """Chebyshev distance of every row of x to the axis-aligned box [blo, bhi] (0 inside)."""
+    return np.maximum(np.maximum(blo - x, x - bhi), 0.0).max(axis=1)
+
+
+def make_shard(nodes: np.ndarray, qpts: np.ndarray, k: int, rank: int, world: int, halo: float | None = None,
+               group: int = POINT_GROUP) -> Shard:
+    """`group`: points are taken in whole groups of `group` consecutive global ids (a group with one point within
+    `halo` of the box is taken entirely).  The shard's local groups of `group` consecutive points are then the
+    undivided problem's groups, so a reduction that sums group-wise (the panel kernel) rounds the owned rows exactly
+    as it does on the undivided problem.  The node halo grows accordingly: `halo` beyond the farthest taken point."""
+    N, Nq = nodes.shape[0], qpts.shape[0]
     lo, hi = owned_rows(N, rank, world)
     if halo is None:
         halo = halo_estimate(nodes, k)
     own = nodes[lo:hi]
     blo, bhi = own.min(axis=0), own.max(axis=0)
-    take_p = np.all((qpts >= blo - halo) & (qpts <= bhi + halo), axis=1)
-    take_n = np.all((nodes >= blo - 2.0 * halo) & (nodes <= bhi + 2.0 * halo), axis=1)
+    dist_p = _box_distance(qpts, blo, bhi)
+    take_p = dist_p <= halo
+    if group > 1:
+        G = -(-Nq // group)
+        pad = np.zeros(G * group, dtype=bool)
+        pad[:Nq] = take_p
+        take_p = np.repeat(pad.reshape(G, group).any(axis=1), group)[:Nq]
+    reach = max(float(halo), float(dist_p[take_p].max())) if take_p.any() else float(halo)
+    take_n = _box_distance(nodes, blo, bhi) <= reach + halo      # every taken point's support (radius <= halo)
     take_n[lo:hi] = True
     node_ids = np.nonzero(take_n)[0].astype(np.int64)
     point_ids = np.nonzero(take_p)[0].astype(np.int64)

@@ -5,7 +5,7 @@ from __future__ import annotations
 import numpy as np
 
 
-def run_cuda(w, *, penalty=True, loads=True, index_bits=None, want_shape=True, ctx=None, reduction=0):
+def run_cuda(w, *, penalty=True, loads=True, index_bits=None, want_shape=True, ctx=None, reduction=0, panel_shape=None):
     import torch
     import paper_1802_04256_b200 as rp
 
@@ -16,6 +16,7 @@ def run_cuda(w, *, penalty=True, loads=True, index_bits=None, want_shape=True, c
     out = {}
     try:
         ctx.set_reduction(reduction)
+        ctx.set_panel_shape(**(panel_shape or {}))
         d_nodes = torch.from_numpy(w.nodes).to(dev)
         d_qpts = torch.from_numpy(w.qpts).to(dev)
         d_qw = torch.from_numpy(w.qw).to(dev)
@@ -29,7 +30,8 @@ def run_cuda(w, *, penalty=True, loads=True, index_bits=None, want_shape=True, c
         d_vals = torch.full((nnz,), float("nan"), dtype=torch.float64, device=dev)
         d_f = torch.full((3 * w.N,), float("nan"), dtype=torch.float64, device=dev)
         nsing = ctx.assemble(d_qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, d_vals, d_f)
-        out.update(nnz=nnz, bits=bits, nsing=nsing, phase_ms=ctx.phase_ms(), reduction_used=ctx.reduction_used())
+        out.update(nnz=nnz, bits=bits, nsing=nsing, phase_ms=ctx.phase_ms(), reduction_used=ctx.reduction_used(),
+                   reduction_params=ctx.reduction_params())
         if want_shape:
             d_phi = torch.empty((w.Nq, w.k), dtype=torch.float64, device=dev)
             d_dphi = torch.empty((w.Nq, 3, w.k), dtype=torch.float64, device=dev)
@@ -202,6 +204,31 @@ def gpu_invariants(ctx, w, d_nodes, d_vals, d_f):
     lever = float(np.abs(w.nodes - xc).max()) * max(np.abs(expect).max(), 1e-300)
     out["torque_err"] = float(np.abs(tq - texp).max() / lever)
     out["qw_err"] = float(abs(w.qw.sum() - w.volume) / w.volume)
+    # energy identity for linear fields (the oracle's own pin in test_oracle_pins.py):
+    # v^T K u = Vol * eps_v^T D eps_u.  Unlike symmetry and the rigid-body modes -- which every single point's
+    # w B^T D B satisfies on its own -- this one moves when a point (1 / Nq of the energy) is dropped or doubled.
+    lam, mu = w.E * w.nu / ((1 + w.nu) * (1 - 2 * w.nu)), w.E / (2 * (1 + w.nu))
+    D = np.zeros((6, 6))
+    D[:3, :3] = lam
+    D[np.arange(3), np.arange(3)] += 2 * mu
+    D[np.arange(3, 6), np.arange(3, 6)] = mu
+
+    def voigt(H):
+        e = 0.5 * (H + H.T)
+        return np.array([e[0, 0], e[1, 1], e[2, 2], 2 * e[0, 1], 2 * e[1, 2], 2 * e[2, 0]])
+    rng = np.random.default_rng(3)
+    worst = 0.0
+    Ku = torch.empty_like(x)
+    for _ in range(6):
+        Hu, Hv = rng.standard_normal((3, 3)), rng.standard_normal((3, 3))
+        u = (r @ torch.from_numpy(Hu.T).to(dev)).contiguous().view(-1)      # (centred coordinates: a rigid shift of u)
+        v = (r @ torch.from_numpy(Hv.T).to(dev)).contiguous().view(-1)
+        ctx.matvec(d_vals, u, Ku)
+        got = float(torch.dot(v, Ku))
+        expect = w.volume * voigt(Hv) @ D @ voigt(Hu)
+        scale = w.volume * np.abs(D).max() * np.abs(Hu).max() * np.abs(Hv).max()
+        worst = max(worst, abs(got - expect) / scale)
+    out["energy_err"] = float(worst)
     return out
 
 

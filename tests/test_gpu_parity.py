@@ -300,26 +300,29 @@ def test_cuda_K_against_the_plain_definition(idx, reduction):
     assert err <= DEF_TOL[w.k] and (ferr <= DEF_TOL[w.k] or np.abs(fr).max() == 0.0)
 
 
-@pytest.mark.parametrize("env", [
-    {"RPIM_PANEL_R": "2", "RPIM_PANEL_CW": "3"},                        # row pairs sharing the gradient loads
-    {"RPIM_PANEL_R": "2", "RPIM_PANEL_CW": "1", "RPIM_PANEL_T": "2"},   # one warp takes all chunks of its pair
-    {"RPIM_PANEL_R": "1", "RPIM_PANEL_CW": "1", "RPIM_PANEL_NSTAGE": "2"},
-    {"RPIM_PANEL_R": "1", "RPIM_PANEL_CW": "3", "RPIM_PANEL_T": "4"},
-    {"RPIM_TILE_DESC": "thread"},     # the descriptor kernel large problems take (one thread per tile)
-    {"RPIM_PANEL_GRAD_ONLY": "1"},    # gradient rows by the 2-D tensor copy
-    {"RPIM_PANEL_GRAD_ONLY": "0"},    # whole staged rows by a plain bulk copy
+@pytest.mark.parametrize("shape", [
+    dict(rows_per_group=2, warps_per_group=3),                       # row pairs sharing the gradient loads
+    dict(rows_per_group=2, warps_per_group=1, rows_per_tile=2),      # one warp takes all chunks of its pair
+    dict(rows_per_group=1, warps_per_group=1, ring_stages=2),
+    dict(rows_per_group=1, warps_per_group=3, rows_per_tile=4),
+    dict(tile_desc=2),     # the descriptor kernel large problems take (one thread per tile)
+    dict(staging=1),       # gradient rows by the 2-D tensor copy
+    dict(staging=2),       # whole staged rows by a plain bulk copy
 ])
-def test_panel_reduction_launch_shapes(env, monkeypatch):
+def test_panel_reduction_launch_shapes(shape):
     """The other launch shapes of reduce_panels_kernel (rows per warp group, warps per group, rows per tile, ring
-    depth; rpim_build_pattern reads the RPIM_PANEL_* overrides): same bars, and bitwise the same K as the default
+    depth, staging; forced through rpim_set_panel_shape): same bars, and bitwise the same K as the default
     shape (the order of summation per entry does not depend on the launch shape)."""
     w = workloads.make_block("shape60", 10, 9, 8, 1.0, 2, 60, 5e9, 0.3, jitter=0.3, seed=360,
                              body=(10.0, -20.0, -2.5e4), bc="bottom+roller")
     g0, o = run_cuda(w, reduction=2), run_oracle(w)
-    for kk, v in env.items():
-        monkeypatch.setenv(kk, v)
-    g = run_cuda(w, reduction=2)
+    g = run_cuda(w, reduction=2, panel_shape=shape)
     assert g["reduction_used"] == 2
+    used = g["reduction_params"]
+    for key, name in (("rows_per_tile", "rows_per_tile"), ("warps_per_group", "warps_per_row_group"),
+                      ("rows_per_group", "rows_per_warp_group"), ("ring_stages", "ring_stages")):
+        assert key not in shape or used[name] == shape[key], (key, used)
+    assert "staging" not in shape or used["tensor_copy_staging"] == (1 if shape["staging"] == 1 else 0)
     _compare(w, g, o)
     assert np.array_equal(g["vals"], g0["vals"]) and np.array_equal(g["f"], g0["f"])
 

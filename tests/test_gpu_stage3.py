@@ -135,3 +135,11 @@ def test_pcg_reports_the_true_residual_handles_zero_load_and_flags_breakdown():
         with pytest.raises(rp.RpimError) as e:
             ctx.solve_pcg(-vals, f, u, 1e-10, 10000)
         assert e.value.code == -8
+        # a load vector with a NaN is not "f = 0": no converged solve is reported, and the guess is left alone
+        fn = f.clone()
+        fn[5] = float("nan")
+        u = torch.full_like(f, 3.0)
+        with pytest.raises(rp.RpimError) as e:
+            ctx.solve_pcg(vals, fn, u, 1e-10, 100)
+        assert e.value.code == -8 and "finite" in str(e.value)
+        assert bool((u == 3.0).all())

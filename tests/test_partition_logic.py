@@ -91,6 +91,8 @@ def test_two_ranks_shard_one_domain_and_stitch_back_to_the_undivided_matrix(tmp_
         assert np.isin(S[r["point_ids"]].ravel(), r["node_ids"]).all()       # halo of nodes is a superset
         assert np.array_equal(r["node_ids"][r["support"]], S[r["point_ids"]])  # sub-cloud search = true supports
         assert float(r["halo_ok"]) == 1.0
+        gid, cnt = np.unique(r["point_ids"] // 8, return_counts=True)          # points come in whole groups of 8
+        assert np.all(cnt[gid < w.Nq // 8] == 8)
         a, b = int(rp[3 * lo]), int(rp[3 * hi])
         assert np.array_equal(r["orp"], rp[3 * lo:3 * hi + 1] - a)            # owned rows: pattern bit-exact
         assert np.array_equal(r["gcol"], ci[a:b])

@@ -534,6 +534,10 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
         out["fp64_probe"] = ctx.probe_fp64()
     except Exception as ex:
         out["fp64_probe"] = {"error": repr(ex)[:200]}
+    try:
+        out["fp64_dmma_probe"] = ctx.probe_fp64_dmma()
+    except Exception as ex:
+        out["fp64_dmma_probe"] = {"error": repr(ex)[:200]}
     ctx.close()
     torch.cuda.empty_cache()
     return out
@@ -616,6 +620,13 @@ def main():
     if rank == 0:
         roofline = r["roofline"]
         roofline["fp64_probe"] = r["fp64_probe"]
+        # scalars beside the nested records (a flat reader keeps these): measured sustained DFMA and FP64 mma.sync
+        # rates on this device, and the dominant kernel's fraction of the MEASURED DFMA rate next to `frac`
+        # (which stays against the derived peak, `peak_source`)
+        roofline["fp64_probe_tflops"] = r["fp64_probe"].get("tflops")
+        roofline["fp64_dmma_probe_tflops"] = r["fp64_dmma_probe"].get("tflops")
+        if roofline.get("bound") == "alu" and roofline["fp64_probe_tflops"]:
+            roofline["frac_of_measured_fp64"] = roofline["achieved"] / roofline["fp64_probe_tflops"]
         line = {
             "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,

@@ -257,6 +257,11 @@ int rpim_phase_totals(rpim_ctx* ctx, double out_ms[5], int64_t out_calls[2], int
  * best launch.  Synchronises the stream. */
 int rpim_probe_fp64(rpim_ctx* ctx, double* out_tflops, double* out_ms);
 
+/* The same measurement for the FP64 tensor-core instruction sm_100a has (warp-level mma.sync m8n8k4; tcgen05 has no
+ * FP64 kind): eight independent accumulator chains per warp, 2 x 8 x 8 x 4 flops per instruction.  It answers SURVEY.md
+ * section 8(d) "measure DMMA against DFMA" for the B^T D B contraction; DESIGN.md section 5 has the outcome. */
+int rpim_probe_fp64_dmma(rpim_ctx* ctx, double* out_tflops, double* out_ms);
+
 /* Number of kernels this library has launched on the context since creation. */
 int64_t rpim_launch_count(const rpim_ctx* ctx);
 

@@ -20,6 +20,7 @@ EXPORTED_SYMBOLS = (
     "rpim_matvec", "rpim_solve_pcg", "rpim_recover_stress", "rpim_set_reduction", "rpim_reduction_used",
     "rpim_probe_fp64", "rpim_update_nodes", "rpim_reduction_params", "rpim_set_modulus_scale",
     "rpim_apply_penalty_static", "rpim_apply_penalty_static_max_nodes", "rpim_set_panel_shape",
+    "rpim_probe_fp64_dmma",
 )
 
 
@@ -73,6 +74,7 @@ def _load():
     lib.rpim_solve_pcg.argtypes = [vp, vp, vp, vp, dbl, C.c_int, C.POINTER(C.c_int), C.POINTER(dbl)]
     lib.rpim_recover_stress.argtypes = [vp, vp, dbl, dbl, vp]
     lib.rpim_probe_fp64.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]
+    lib.rpim_probe_fp64_dmma.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl)]
     lib.rpim_set_reduction.argtypes = [vp, C.c_int]
     lib.rpim_reduction_used.argtypes = [vp]
     lib.rpim_reduction_params.argtypes = [vp, C.POINTER(C.c_int)]
@@ -149,6 +151,13 @@ def rpim_probe_fp64(ctx):
     """{"tflops": sustained FP64 fma rate, "ms": duration of the best launch}."""
     tf, ms = C.c_double(0.0), C.c_double(0.0)
     _check(ctx, _load().rpim_probe_fp64(ctx, C.byref(tf), C.byref(ms)))
+    return {"tflops": float(tf.value), "ms": float(ms.value)}
+
+
+def rpim_probe_fp64_dmma(ctx):
+    """{"tflops": sustained FP64 mma.sync m8n8k4 rate, "ms": duration of the best launch}."""
+    tf, ms = C.c_double(0.0), C.c_double(0.0)
+    _check(ctx, _load().rpim_probe_fp64_dmma(ctx, C.byref(tf), C.byref(ms)))
     return {"tflops": float(tf.value), "ms": float(ms.value)}
 
 
@@ -376,6 +385,9 @@ class Context:
 
     def probe_fp64(self):
         return rpim_probe_fp64(self.ctx)
+
+    def probe_fp64_dmma(self):
+        return rpim_probe_fp64_dmma(self.ctx)
 
     def set_reduction(self, mode):
         return rpim_set_reduction(self.ctx, mode)

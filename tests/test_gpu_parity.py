@@ -203,6 +203,13 @@ def test_error_codes():
             ctx.apply_penalty(bad, None, torch.zeros((2, 3), dtype=torch.float64, device=dev), 1.0, False, vals, f)
         assert e.value.code == -5
         assert ctx.workspace_bytes() > 0
+        # rpim_set_panel_shape: out-of-range values are refused and change nothing
+        for bad_shape in (dict(rows_per_tile=3), dict(rows_per_tile=10), dict(warps_per_group=5), dict(rows_per_group=3),
+                          dict(ring_stages=1), dict(ring_stages=9), dict(staging=3), dict(tile_desc=-1)):
+            with pytest.raises(rp.RpimError) as e:
+                ctx.set_panel_shape(**bad_shape)
+            assert e.value.code == -1
+        ctx.set_panel_shape()                      # all automatic
 
 
 def test_host_buffer_entry_points_match_device_path():

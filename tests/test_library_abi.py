@@ -50,3 +50,20 @@ def test_product_never_imports_oracle_and_vice_versa():
                     src = open(os.path.join(dirpath, fn)).read()
                     for inc in re.findall(r'#include\s+"([^"]+)"', src):
                         assert banned not in inc and "oracle" not in inc.lower() or sub == "oracle", (fn, inc)
+
+
+def test_library_code_reads_no_environment_variable():
+    """The launch shape of a C-ABI library must not depend on the caller's environment (rpim_set_panel_shape is
+    the explicit knob): none of the library's own object files references getenv.  (librpim.so as a whole does --
+    the statically linked CUDA runtime reads CUDA_* variables -- so the objects are what is checked.)"""
+    import glob
+    import subprocess
+    from paper_1802_04256_b200 import build
+    build.build()
+    objs = sorted(glob.glob(os.path.join(ROOT, "paper_1802_04256_b200", "csrc", "build", "*.o")))
+    assert len(objs) >= 10
+    for o in objs:
+        und = subprocess.run(["nm", "-u", o], capture_output=True, text=True, check=True).stdout
+        assert "getenv" not in und, os.path.basename(o)
+    for src in glob.glob(os.path.join(ROOT, "paper_1802_04256_b200", "csrc", "*.cu*")):
+        assert "getenv" not in open(src).read(), os.path.basename(src)

@@ -299,6 +299,8 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
     d_bcu = torch.from_numpy(w.bc_ubar).to(dev)
 
     # first pass sizes the outputs (pattern is data dependent)
+    if getattr(args, "index_bits", 0):
+        w.index_bits = args.index_bits      # 6432 = RPIM_INDEX_MIXED: int64 row_ptr, int32 col_idx (not the default)
     nnz, bits = ctx.build_pattern(d_nodes, d_qpts, w.k, w.index_bits)
     if shard is not None:
         d_sup = torch.empty((w.Nq, w.k), dtype=torch.int32, device=dev)
@@ -306,8 +308,9 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
         check_shard(shard, w, d_sup.cpu().numpy(), nq_job, world, dev)
         del d_sup
     idt = torch.int32 if bits == 32 else torch.int64
+    cdt = torch.int64 if bits == 64 else torch.int32
     d_rp = torch.empty(3 * w.N + 1, dtype=idt, device=dev)
-    d_ci = torch.empty(nnz, dtype=idt, device=dev)
+    d_ci = torch.empty(nnz, dtype=cdt, device=dev)
     d_vals = torch.empty(nnz, dtype=torch.float64, device=dev)
     d_f = torch.empty(3 * w.N, dtype=torch.float64, device=dev)
 
@@ -491,7 +494,7 @@ def bench_config(name, args, steps, warmup, dev, rank, local_rank, world, peaks,
             h_nodes, h_qpts, h_qw = pin(w.nodes), pin(w.qpts), pin(w.qw)
             h_bcn, h_bcm, h_bcu = pin(w.bc_nodes), pin(w.bc_mask), pin(w.bc_ubar)
             h_rp = torch.empty(3 * w.N + 1, dtype=idt, pin_memory=True).numpy()
-            h_ci = torch.empty(nnz, dtype=idt, pin_memory=True).numpy()
+            h_ci = torch.empty(nnz, dtype=cdt, pin_memory=True).numpy()
             h_vals = torch.empty(nnz, dtype=torch.float64, pin_memory=True).numpy()
             h_f = torch.empty(3 * w.N, dtype=torch.float64, pin_memory=True).numpy()
             assert h_rp.dtype == np_idt
@@ -569,6 +572,9 @@ def main():
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard ONE domain of the config into row slabs with halos (strong scaling, allreduce(max) of "
                          "the penalty scale) instead of N independent replicas")
+    ap.add_argument("--index-bits", type=int, default=0, choices=[0, 32, 64, 6432],
+                    help="0: the config's own rule (BASELINE.json: 64-bit iff nnz > 2^31 - 1); 6432 = RPIM_INDEX_MIXED "
+                         "(int64 row_ptr, int32 col_idx): a side measurement, never the default")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="do not also time `large` when the headline is `stress`")

@@ -50,6 +50,12 @@ typedef enum rpim_status {
 
 #define RPIM_MAX_K 124  /* moment systems up to 128 x 128 */
 
+/* index_bits value for CSR arrays of mixed width: row_ptr int64_t (offsets up to nnz), col_idx int32_t (DOF ids
+ * below 3 N < 2^31, which rpim_build_pattern guarantees).  Where nnz > 2^31 - 1 forces 64-bit offsets this halves
+ * col_idx: 31 GB less HBM and 31 GB less to copy at the `stress` configuration.  Never
+ * chosen automatically: index_bits = 0 keeps BASELINE.json's rule (both arrays 64-bit iff nnz > 2^31 - 1). */
+#define RPIM_INDEX_MIXED 6432
+
 /* Create a context on CUDA device `device`; all work goes to `cuda_stream` (a cudaStream_t,
  * may be NULL for the default stream).  Fails with RPIM_ERR_CUDA when no device exists. */
 int rpim_create(rpim_ctx** out_ctx, int device, void* cuda_stream);
@@ -99,8 +105,9 @@ int rpim_set_panel_shape(rpim_ctx* ctx, int rows_per_tile, int warps_per_group, 
  * uniform cell grid and the CSR pattern of the 3N x 3N stiffness matrix.
  *   d_nodes  N x 3 field-node coordinates        d_qpts  Nq x 3 quadrature points
  *   k        support size (4 <= k <= min(N, RPIM_MAX_K))
- *   index_bits  0 = auto (64 iff nnz > 2^31 - 1), 32 or 64: width of row_ptr AND col_idx
- *   out_nnz, out_index_bits  host scalars (number of stored scalar entries, chosen width)
+ *   index_bits  0 = auto (64 iff nnz > 2^31 - 1), 32 or 64: width of row_ptr AND col_idx;
+ *               RPIM_INDEX_MIXED: row_ptr 64-bit, col_idx 32-bit
+ *   out_nnz, out_index_bits  host scalars (number of stored scalar entries; chosen width: 32, 64 or RPIM_INDEX_MIXED)
  * Synchronises the stream. */
 int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const double* d_qpts,
                        int64_t Nq, int k, int index_bits, int64_t* out_nnz, int* out_index_bits);
@@ -121,7 +128,8 @@ int rpim_update_nodes(rpim_ctx* ctx, const double* d_nodes, const double* d_qpts
                       int* out_pattern_rebuilt, int64_t* out_nnz);
 
 /* Write the pattern built by rpim_build_pattern.
- *   d_row_ptr  3N+1 entries, d_col_idx  nnz entries, both int32_t or int64_t per index_bits
+ *   d_row_ptr  3N+1 entries, d_col_idx  nnz entries, both int32_t or int64_t per index_bits (RPIM_INDEX_MIXED:
+ *              d_row_ptr int64_t, d_col_idx int32_t; the same widths hold for h_row_ptr / h_col_idx of rpim_host_assemble)
  *   d_support  Nq x k int32 node ids, ascending per point; may be NULL
  * Any of the three may be NULL to skip it.  Asynchronous. */
 int rpim_get_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx, int32_t* d_support);

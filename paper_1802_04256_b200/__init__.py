@@ -30,4 +30,5 @@ from .binding import (  # noqa: F401
     rpim_workspace_bytes,
     rpim_last_error,
     EXPORTED_SYMBOLS,
+    RPIM_INDEX_MIXED,
 )

@@ -24,6 +24,9 @@ EXPORTED_SYMBOLS = (
 )
 
 
+RPIM_INDEX_MIXED = 6432   # index_bits: row_ptr int64, col_idx int32 (include/rpim.h)
+
+
 class RpimError(RuntimeError):
     def __init__(self, code: int, msg: str):
         super().__init__(f"librpim error {code}: {msg}")
@@ -287,10 +290,11 @@ def rpim_host_assemble(ctx, h_qw, E, nu, alpha_c, d_c, q, body, h_bc_nodes, h_bc
     ns, used = C.c_int64(0), C.c_double(0.0)
     m = 0 if h_bc_nodes is None else h_bc_nodes.shape[0]
     idt = None if h_row_ptr is None else h_row_ptr.dtype
+    cdt = None if h_col_idx is None else h_col_idx.dtype     # RPIM_INDEX_MIXED: int64 offsets, int32 column ids
     rc = _load().rpim_host_assemble(ctx, _hptr(h_qw, np.float64), float(E), float(nu), float(alpha_c), float(d_c),
                                     float(q), b, _hptr(h_bc_nodes, np.int64), _hptr(h_bc_mask, np.uint8),
                                     _hptr(h_u_bar, np.float64), m, float(alpha), int(bool(alpha_is_relative)),
-                                    _hptr(h_row_ptr, idt), _hptr(h_col_idx, idt), _hptr(h_vals, np.float64),
+                                    _hptr(h_row_ptr, idt), _hptr(h_col_idx, cdt), _hptr(h_vals, np.float64),
                                     _hptr(h_f, np.float64), C.byref(ns), C.byref(used))
     _check(ctx, rc)
     return int(ns.value), float(used.value)

@@ -140,7 +140,8 @@ int rpim_build_pattern(rpim_ctx* ctx, const double* d_nodes, int64_t N, const do
     if (!ctx) return RPIM_ERR_INVALID_ARG;
     if (!d_nodes || !d_qpts || N <= 0 || Nq <= 0) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "null pointer or empty input");
     if (k < 4 || k > RPIM_MAX_K || k > N) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "k = %d must satisfy 4 <= k <= min(N, %d)", k, RPIM_MAX_K);
-    if (index_bits != 0 && index_bits != 32 && index_bits != 64) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "index_bits must be 0, 32 or 64");
+    if (index_bits != 0 && index_bits != 32 && index_bits != 64 && index_bits != RPIM_INDEX_MIXED)
+        RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "index_bits must be 0, 32, 64 or RPIM_INDEX_MIXED (%d)", RPIM_INDEX_MIXED);
     if (N > 700000000 || Nq * (int64_t)k > 0x7fffffff00LL || Nq > 0x7fffffff) RPIM_FAIL(ctx, RPIM_ERR_INVALID_ARG, "problem too large for 32-bit node / point ids");
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
@@ -569,7 +570,8 @@ int rpim_host_assemble(rpim_ctx* ctx, const double* h_qw, double E, double nu, d
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
     const int64_t nnz = 9 * ctx->nnzb, n3 = 3 * ctx->N;
-    const size_t iw = ctx->index_bits / 8;
+    // width of a row_ptr entry / of a col_idx entry (RPIM_INDEX_MIXED: 64-bit offsets, 32-bit column ids)
+    const size_t iw = ctx->index_bits == 32 ? 4 : 8, iwc = ctx->index_bits == 64 ? 8 : 4;
     // device buffers of the call live in the context's workspace (cached across calls: no cudaMalloc / cudaFree
     // per step); the index arrays go back to the host on a side stream while the values are assembled
     int rc = RPIM_OK;
@@ -582,7 +584,7 @@ int rpim_host_assemble(rpim_ctx* ctx, const double* h_qw, double E, double nu, d
         if (h_bc_mask && (rc = ws_alloc(ctx, &ctx->hb_bm, m))) return rc;
     }
     if (h_row_ptr && (rc = ws_alloc(ctx, &ctx->hb_rp, (int64_t)((n3 + 1) * iw)))) return rc;
-    if (h_col_idx && (rc = ws_alloc(ctx, &ctx->hb_ci, (int64_t)(std::max<int64_t>(nnz, 1) * iw)))) return rc;
+    if (h_col_idx && (rc = ws_alloc(ctx, &ctx->hb_ci, (int64_t)(std::max<int64_t>(nnz, 1) * iwc)))) return rc;
     if (!ctx->side_stream) {
         CUDA_TRY(ctx, cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking));
         CUDA_TRY(ctx, cudaEventCreateWithFlags(&ctx->side_ev[0], cudaEventDisableTiming));
@@ -598,7 +600,7 @@ int rpim_host_assemble(rpim_ctx* ctx, const double* h_qw, double E, double nu, d
     CUDA_TRY(ctx, cudaEventRecord(ctx->side_ev[0], st));
     CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->side_stream, ctx->side_ev[0], 0));
     if (h_row_ptr) CUDA_TRY(ctx, cudaMemcpyAsync(h_row_ptr, ctx->hb_rp, (size_t)(n3 + 1) * iw, cudaMemcpyDeviceToHost, ctx->side_stream));
-    if (h_col_idx) CUDA_TRY(ctx, cudaMemcpyAsync(h_col_idx, ctx->hb_ci, (size_t)nnz * iw, cudaMemcpyDeviceToHost, ctx->side_stream));
+    if (h_col_idx) CUDA_TRY(ctx, cudaMemcpyAsync(h_col_idx, ctx->hb_ci, (size_t)nnz * iwc, cudaMemcpyDeviceToHost, ctx->side_stream));
     CUDA_TRY(ctx, cudaEventRecord(ctx->side_ev[1], ctx->side_stream));
     rc = rpim_assemble(ctx, ctx->hb_qw, E, nu, alpha_c, d_c, q, body, ctx->hb_vals, ctx->hb_f, out_singular);
     if (rc == RPIM_OK)

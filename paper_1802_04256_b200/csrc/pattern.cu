@@ -925,7 +925,10 @@ int rpim_stage_emit_pattern(rpim_ctx* ctx, void* d_row_ptr, void* d_col_idx) {
     const int64_t N = ctx->N;
     const unsigned nbr = (unsigned)((N + 1 + 255) / 256);
     const unsigned nbc = (unsigned)std::min<int64_t>((N + 7) / 8, 148 * 32);
-    if (ctx->index_bits == 32) {
+    if (ctx->index_bits == RPIM_INDEX_MIXED) {   // 64-bit row offsets, 32-bit column ids (3 N < 2^31 always holds)
+        if (d_row_ptr) { emit_rowptr_kernel<int64_t><<<nbr, 256, 0, st>>>(N, ctx->d_brow_ptr, (int64_t*)d_row_ptr); KERNEL_CHECK(ctx); }
+        if (d_col_idx) { emit_colidx_kernel<int32_t><<<nbc, 256, 0, st>>>(N, ctx->d_brow_ptr, ctx->d_bcol, (int32_t*)d_col_idx); KERNEL_CHECK(ctx); }
+    } else if (ctx->index_bits == 32) {
         if (d_row_ptr) { emit_rowptr_kernel<int32_t><<<nbr, 256, 0, st>>>(N, ctx->d_brow_ptr, (int32_t*)d_row_ptr); KERNEL_CHECK(ctx); }
         if (d_col_idx) { emit_colidx_kernel<int32_t><<<nbc, 256, 0, st>>>(N, ctx->d_brow_ptr, ctx->d_bcol, (int32_t*)d_col_idx); KERNEL_CHECK(ctx); }
     } else {

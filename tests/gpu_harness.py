@@ -23,8 +23,9 @@ def run_cuda(w, *, penalty=True, loads=True, index_bits=None, want_shape=True, c
         bits_req = w.index_bits if index_bits is None else index_bits
         nnz, bits = ctx.build_pattern(d_nodes, d_qpts, w.k, bits_req)
         idt = torch.int32 if bits == 32 else torch.int64
+        cdt = torch.int64 if bits == 64 else torch.int32           # RPIM_INDEX_MIXED (6432): int64 offsets, int32 ids
         d_rp = torch.empty(3 * w.N + 1, dtype=idt, device=dev)
-        d_ci = torch.empty(nnz, dtype=idt, device=dev)
+        d_ci = torch.empty(nnz, dtype=cdt, device=dev)
         d_sup = torch.empty((w.Nq, w.k), dtype=torch.int32, device=dev)
         ctx.get_pattern(d_rp, d_ci, d_sup)
         d_vals = torch.full((nnz,), float("nan"), dtype=torch.float64, device=dev)

@@ -111,6 +111,25 @@ def test_run_to_run_bitwise_determinism_and_index_width():
     for key in ("vals", "f", "vals0", "phi", "dphi"):
         assert np.array_equal(a[key], b[key]) and np.array_equal(a[key], c[key])
     assert a["launches"] > 0
+    # mixed widths (RPIM_INDEX_MIXED): 64-bit row offsets, 32-bit column ids, same pattern and values; also through
+    # the host-buffer entry points
+    import paper_1802_04256_b200 as rp
+    m = run_cuda(w, index_bits=rp.RPIM_INDEX_MIXED)
+    assert m["bits"] == rp.RPIM_INDEX_MIXED and m["row_ptr"].dtype == np.int64 and m["col_idx"].dtype == np.int32
+    assert np.array_equal(m["row_ptr"], b["row_ptr"]) and np.array_equal(m["col_idx"], b["col_idx"])
+    assert np.array_equal(m["vals"], b["vals"]) and np.array_equal(m["f"], b["f"])
+    with rp.Context(0) as ctx:
+        nnz, bits = ctx.host_pattern(w.nodes, w.qpts, w.k, rp.RPIM_INDEX_MIXED)
+        assert bits == rp.RPIM_INDEX_MIXED and nnz == b["nnz"]
+        rpa, cia = np.full(3 * w.N + 1, -1, np.int64), np.full(nnz, -1, np.int32)
+        vals, f = np.empty(nnz), np.empty(3 * w.N)
+        ctx.host_assemble(w.qw, w.E, w.nu, w.alpha_c, w.d_c, w.q, w.body, w.bc_nodes, w.bc_mask, w.bc_ubar,
+                          w.penalty_alpha, True, rpa, cia, vals, f)
+        assert np.array_equal(rpa, b["row_ptr"]) and np.array_equal(cia, b["col_idx"])
+        assert np.array_equal(vals, b["vals"]) and np.array_equal(f, b["f"])
+        with pytest.raises(rp.RpimError) as e:
+            ctx.host_pattern(w.nodes, w.qpts, w.k, 48)
+        assert e.value.code == -1
 
 
 def test_shuffled_node_numbering():
